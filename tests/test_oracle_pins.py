@@ -1,0 +1,465 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (all -m "not gpu").
+
+Each test names the passage of PAPER.md (arXiv 2401.17074) or the DESIGN.md reading it pins.
+Nothing here is produced by the CUDA path.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from paper_2401_17074_b200 import workloads as W
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+CS2 = 1.0 / 3.0
+DIRS = [(cx, cy, cz) for cz in (-1, 0, 1) for cy in (-1, 0, 1) for cx in (-1, 0, 1)]
+
+
+def rand_M(rng, amp_u=0.1, amp_pi=0.01):
+    M = np.empty(10)
+    M[0] = 1.0 + rng.uniform(-0.2, 0.2)
+    M[1:4] = rng.uniform(-amp_u, amp_u, 3)
+    M[4:10] = rng.uniform(-amp_pi, amp_pi, 6)
+    return M
+
+
+def Pi_of(M):
+    return np.array([[M[4], M[7], M[8]], [M[7], M[5], M[9]], [M[8], M[9], M[6]]])
+
+
+# ---------------------------------------------------------------------------------------------
+# P1 / P2: moment reproduction.  Pins w_i, H2, H3, the 1/(n! cs^2n) prefactors, readings A1-A4, A6.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+def test_P1_moments_order_0_1_2(oracle_mod, mode):
+    """sum f* = rho; sum c f* = rho u (+ rho g); sum cc f* = rho cs2 I + rho uu + (1-w) Pi.
+    (PAPER.md:45 'linear and local summations', Eq. 12, Eq. 14, Eq. 17)"""
+    rng = np.random.default_rng(11)
+    for _ in range(20):
+        M = rand_M(rng)
+        omega = rng.uniform(0.3, 1.99)
+        g = rng.uniform(-1e-3, 1e-3, 3) if _ % 2 else np.zeros(3)
+        rho, u, Pi = M[0], M[1:4], Pi_of(M)
+        f = np.array([oracle_mod.fstar(M, c, omega, g, mode) for c in DIRS])
+        c = np.array(DIRS, dtype=float)
+        assert abs(f.sum() - rho) < 1e-15 * 4
+        np.testing.assert_allclose(c.T @ f, rho * (u + g), atol=5e-16)
+        S = np.einsum("i,ia,ib->ab", f, c, c)
+        np.testing.assert_allclose(S, rho * CS2 * np.eye(3) + rho * np.outer(u, u) + (1 - omega) * Pi, atol=5e-16)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_P2_third_moments(oracle_mod, mode):
+    """sum c_a c_b c_g f* = rho u_a u_b u_g + (1-w) a3_abg + cs2 rho (u_a d_bg + u_b d_ag + u_g d_ab)
+    for every index triple except a=b=g (H3_aaa = 0 on this lattice).  Pins H3, 1/(6 cs^6), the
+    three-term symmetrised a3 of Eq. 17 (reading A4) and 'third-order equilibrium term once' (A1).
+    (PAPER.md:140 Eq. 15, :150 Eq. 17)"""
+    rng = np.random.default_rng(12)
+    d = np.eye(3)
+    for _ in range(10):
+        M = rand_M(rng)
+        omega = rng.uniform(0.3, 1.99)
+        rho, u, Pi = M[0], M[1:4], Pi_of(M)
+        f = np.array([oracle_mod.fstar(M, c, omega, (0, 0, 0), mode) for c in DIRS])
+        c = np.array(DIRS, dtype=float)
+        Q = np.einsum("i,ia,ib,ig->abg", f, c, c, c)
+        a3 = (np.einsum("ab,g->abg", Pi, u) + np.einsum("a,bg->abg", u, Pi) + np.einsum("b,ag->abg", u, Pi))
+        want = (rho * np.einsum("a,b,g->abg", u, u, u) + (1 - omega) * a3
+                + CS2 * rho * (np.einsum("a,bg->abg", u, d) + np.einsum("b,ag->abg", u, d) + np.einsum("g,ab->abg", u, d)))
+        for a, b, g in itertools.product(range(3), repeat=3):
+            if a == b == g:
+                # the lattice cannot carry c^3: sum c_a^3 f = sum c_a f
+                assert abs(Q[a, a, a] - rho * u[a]) < 1e-15
+            else:
+                assert abs(Q[a, b, g] - want[a, b, g]) < 1e-16 * 5, (a, b, g)
+
+
+def test_P2b_dropped_terms_would_fail(oracle_mod):
+    """Sensitivity check of P1/P2: a second-order-only population (Eq. 8) misses the third moment."""
+    M = np.array([1.1, 0.1, -0.07, 0.05, 0, 0, 0, 0, 0, 0])
+    c = np.array(DIRS, dtype=float)
+    f = np.array([oracle_mod.fstar(M, ci, 1.0, (0, 0, 0), 1) for ci in DIRS])
+    w = np.array([np.prod([2 / 3 if k == 0 else 1 / 6 for k in ci]) for ci in DIRS])
+    cu = c @ M[1:4]
+    f2 = w * M[0] * (1 + 3 * cu + 4.5 * cu * cu - 1.5 * (M[1:4] @ M[1:4]))      # Eq. 2
+    Q3 = np.einsum("i,i,i,i->", f, c[:, 0], c[:, 0], c[:, 1])
+    Q2 = np.einsum("i,i,i,i->", f2, c[:, 0], c[:, 0], c[:, 1])
+    want = M[0] * M[1] ** 2 * M[2] + CS2 * M[0] * M[2]
+    assert abs(Q3 - want) < 1e-16 and abs(Q2 - want) > 1e-4
+
+
+def test_tau1_is_pure_equilibrium(oracle_mod):
+    """omega = 1: f* = f_eq, independent of Pi (Eq. 5)."""
+    rng = np.random.default_rng(3)
+    M = rand_M(rng)
+    M0 = M.copy(); M0[4:] = 0
+    for c in DIRS:
+        assert oracle_mod.fstar(M, c, 1.0) == oracle_mod.fstar(M0, c, 1.0)
+
+
+def test_rest_state_weights(oracle_mod):
+    """rho = 1, u = 0, Pi = 0: f*_i = w_i, the D3Q27 weights 8/27, 2/27, 1/54, 1/216 by shell (Fig. 2)."""
+    M = np.zeros(10); M[0] = 1
+    shell = {0: 8 / 27, 1: 2 / 27, 2: 1 / 54, 3: 1 / 216}
+    for c in DIRS:
+        assert abs(oracle_mod.fstar(M, c, 0.7, (0, 0, 0), 0) - shell[sum(abs(k) for k in c)]) < 1e-17
+
+
+# ---------------------------------------------------------------------------------------------
+# P9: brute-force tensor mode == closed-form mode, on states incl. every boundary kind
+# ---------------------------------------------------------------------------------------------
+def _mk(oracle_mod, w):
+    o = oracle_mod.Oracle(w.nx, w.ny, w.nz, w.tau)
+    for f, k in w.faces.items():
+        if w.inlet is not None and f == w.inlet.face:
+            o.set_face(f, k, w.inlet.u_plane, w.inlet.noise_amp, w.inlet.seed, w.inlet.noise_mask)
+        else:
+            o.set_face(f, k)
+    o.set_force(w.g)
+    o.set_moments(w.moments)
+    return o
+
+
+def test_P9_brute_vs_closed_fstar(oracle_mod):
+    rng = np.random.default_rng(5)
+    for _ in range(50):
+        M = rand_M(rng); om = rng.uniform(0.2, 1.99); g = rng.uniform(-1e-2, 1e-2, 3)
+        for c in DIRS:
+            a = oracle_mod.fstar(M, c, om, g, 0); b = oracle_mod.fstar(M, c, om, g, 1)
+            assert abs(a - b) < 2e-16
+
+
+@pytest.mark.parametrize("shape", [(3, 3, 3), (4, 3, 5), (6, 5, 7)])
+def test_P9_brute_vs_closed_step_all_bc(oracle_mod, shape):
+    nx, ny, nz = shape
+    w = W.random_state(nx, ny, nz, seed=21)
+    # walls in y + force, periodic x, open z (inlet lo / outlet hi)
+    w.faces = {W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK,
+               W.FACE_ZLO: W.BC_VELOCITY_INLET, W.FACE_ZHI: W.BC_OUTLET_ZERO_GRADIENT}
+    up = np.random.default_rng(2).uniform(-0.03, 0.03, (3, ny, nx))
+    w.inlet = W.Inlet(W.FACE_ZLO, up, 0.05, 9, 0b111)
+    w.g = (1e-4, -2e-4, 3e-4)
+    a = _mk(oracle_mod, w); b = _mk(oracle_mod, w)
+    a.step(3, 0); b.step(3, 1)
+    assert np.abs(a.get_moments() - b.get_moments()).max() < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# P3: uniform flow is a fixed point
+# ---------------------------------------------------------------------------------------------
+def test_P3_uniform_flow_fixed_point(oracle_mod):
+    M = np.zeros((10, 4, 5, 6)); M[0] = 1.07; M[1] = 0.05; M[2] = -0.03; M[3] = 0.02
+    o = oracle_mod.Oracle(6, 5, 4, 0.6); o.set_moments(M); o.step(5)
+    R = o.get_moments()
+    assert np.abs(R[:4] - M[:4]).max() < 5e-16
+    assert np.abs(R[4:]).max() < 5e-16
+
+
+# ---------------------------------------------------------------------------------------------
+# P4: equivalence with a classic two-lattice population code (independent numpy implementation)
+# ---------------------------------------------------------------------------------------------
+class PopulationLB:
+    """Recursive-regularised BGK on D3Q27 with explicit populations, collide then push-stream
+    (Eq. 1, 5, 12, 14, 16, 17).  Walls in y: halfway bounce-back.  Written independently of the
+    oracle with explicit Hermite tensors and einsum."""
+
+    def __init__(self, M, tau, g, walls_y=False):
+        self.c = np.array(DIRS, dtype=int)
+        cf = self.c.astype(float)
+        self.w = np.prod(np.where(self.c == 0, 2 / 3, 1 / 6), axis=1)
+        d = np.eye(3)
+        self.H2 = np.einsum("ia,ib->iab", cf, cf) - CS2 * d[None]
+        self.H3 = (np.einsum("ia,ib,ig->iabg", cf, cf, cf)
+                   - CS2 * (np.einsum("ig,ab->iabg", cf, d) + np.einsum("ia,bg->iabg", cf, d)
+                            + np.einsum("ib,ag->iabg", cf, d)))
+        self.cf = cf
+        self.omega = 1.0 / tau
+        self.g = np.asarray(g, float)
+        self.walls_y = walls_y
+        rho, u = M[0], M[1:4]
+        Pi = np.array([[M[4], M[7], M[8]], [M[7], M[5], M[9]], [M[8], M[9], M[6]]])
+        self.f = self.feq(rho, u) + self.fneq_reg(Pi, u)            # pre-collision
+
+    def feq(self, rho, u):
+        cu = np.einsum("ia,a...->i...", self.cf, u)
+        e2 = np.einsum("iab,a...,b...->i...", self.H2, u, u)
+        e3 = np.einsum("iabg,a...,b...,g...->i...", self.H3, u, u, u)
+        wb = self.w.reshape((-1,) + (1,) * (u.ndim - 1))
+        return wb * rho[None] * (1 + cu / CS2 + e2 / (2 * CS2**2) + e3 / (6 * CS2**3))
+
+    def fneq_reg(self, a2, u):
+        a3 = (np.einsum("ab...,g...->abg...", a2, u) + np.einsum("a...,bg...->abg...", u, a2)
+              + np.einsum("b...,ag...->abg...", u, a2))
+        n2 = np.einsum("iab,ab...->i...", self.H2, a2)
+        n3 = np.einsum("iabg,abg...->i...", self.H3, a3)
+        wb = self.w.reshape((-1,) + (1,) * (u.ndim - 1))
+        return wb * (n2 / (2 * CS2**2) + n3 / (6 * CS2**3))
+
+    def moments(self):
+        f = self.f
+        rho = f.sum(0)
+        u = np.einsum("ia,i...->a...", self.cf, f) / rho
+        fneq = f - self.feq(rho, u)
+        a2 = np.einsum("iab,i...->ab...", self.H2, fneq)             # Eq. 12
+        return rho, u, a2
+
+    def step(self):
+        rho, u, a2 = self.moments()
+        wb = self.w.reshape(-1, 1, 1, 1)
+        cg = (self.cf @ self.g).reshape(-1, 1, 1, 1)
+        post = self.feq(rho, u) + (1 - self.omega) * self.fneq_reg(a2, u) + wb * rho[None] * cg / CS2
+        new = np.empty_like(post)
+        for i, (cx, cy, cz) in enumerate(self.c):
+            new[i] = np.roll(post[i], shift=(cz, cy, cx), axis=(0, 1, 2))   # f_i(x + c_i) = post_i(x)
+        if self.walls_y:
+            opp = {tuple(c): i for i, c in enumerate(self.c)}
+            for i, (cx, cy, cz) in enumerate(self.c):
+                ib = opp[(-cx, -cy, -cz)]
+                if cy == 1:
+                    new[i][:, 0, :] = post[ib][:, 0, :]
+                elif cy == -1:
+                    new[i][:, -1, :] = post[ib][:, -1, :]
+        self.f = new
+
+    def M(self):
+        rho, u, a2 = self.moments()
+        return np.stack([rho, u[0], u[1], u[2], a2[0, 0], a2[1, 1], a2[2, 2], a2[0, 1], a2[0, 2], a2[1, 2]])
+
+
+@pytest.mark.parametrize("walls", [False, True])
+def test_P4_population_code_equivalence(oracle_mod, walls):
+    """TSLB moments == moments of the explicit collide-and-stream code at every step (Eq. 5-6:
+    the thread-safe form is the regularised LB 'in disguise').  Pins pull direction, source-site
+    semantics of the force term (reading A11) and the bounce-back convention (A12)."""
+    w = W.random_state(6, 5, 7, seed=4, tau=0.62)
+    g = (2e-4, -1e-4, 3e-4)
+    o = oracle_mod.Oracle(6, 5, 7, w.tau)
+    if walls:
+        o.set_face(W.FACE_YLO, W.BC_BOUNCE_BACK); o.set_face(W.FACE_YHI, W.BC_BOUNCE_BACK)
+    o.set_force(g); o.set_moments(w.moments)
+    p = PopulationLB(w.moments, w.tau, g, walls_y=walls)
+    assert np.abs(p.M() - w.moments).max() < 1e-15        # initial populations carry the moments
+    for s in range(5):
+        o.step(1); p.step()
+        assert np.abs(o.get_moments() - p.M()).max() < 5e-15, s
+
+
+# ---------------------------------------------------------------------------------------------
+# P5: mass conservation; momentum budget with force
+# ---------------------------------------------------------------------------------------------
+def test_P5_mass_and_momentum_budget_periodic(oracle_mod):
+    w = W.random_state(8, 7, 6, seed=8, tau=0.55)
+    g = np.array([1e-4, 2e-4, -3e-4])
+    o = oracle_mod.Oracle(8, 7, 6, w.tau); o.set_force(g); o.set_moments(w.moments)
+    d0 = o.diagnostics()
+    for s in range(20):
+        o.step(1)
+        d = o.diagnostics()
+        assert abs(d[0] - d0[0]) < 1e-12 * d0[0]
+        # first-order (Luo) forcing: momentum grows by g * mass per step
+        np.testing.assert_allclose(d[1:4], d0[1:4] + (s + 1) * g * d0[0], atol=1e-12)
+
+
+def test_P5_mass_closed_channel(oracle_mod):
+    w = W.channel(8, 12, 6, steps=50, dtype="f64")
+    o = _mk(oracle_mod, w)
+    m0 = o.diagnostics()[0]
+    o.step(50)
+    assert abs(o.diagnostics()[0] - m0) < 1e-12 * m0
+
+
+# ---------------------------------------------------------------------------------------------
+# P6: viscous decay, nu = cs2 (tau - 1/2)
+# ---------------------------------------------------------------------------------------------
+def _amp(M, M0):
+    return float((M[1:4] * M0[1:4]).sum() / (M0[1:4] ** 2).sum())
+
+
+def test_P6_taylor_green_2d_decay(oracle_mod):
+    """2-D Taylor-Green vortex: velocity amplitude ~ exp(-2 nu k^2 t) (the law quoted in north_star)."""
+    w = W.taylor_green_2d(32, 4, tau=0.8, U0=0.01, steps=100)
+    o = _mk(oracle_mod, w); o.step(100)
+    nu = CS2 * (w.tau - 0.5); k = 2 * np.pi / 32
+    nu_eff = -np.log(_amp(o.get_moments(), w.moments)) / (2 * k * k * 100)
+    assert abs(nu_eff / nu - 1) < 0.02
+
+
+def test_P6_config0_decay(oracle_mod):
+    """configs[0]: wave vector (k,k,k) -> amplitude ~ exp(-3 nu k^2 t) (reading A20)."""
+    w = W.config0()
+    o = _mk(oracle_mod, w); o.step(100)
+    nu = CS2 * (w.tau - 0.5); k = 2 * np.pi / 32
+    nu_eff = -np.log(_amp(o.get_moments(), w.moments)) / (3 * k * k * 100)
+    assert abs(nu_eff / nu - 1) < 0.02
+    # wrong tau->nu maps (tau/3, (tau-1)/3) are off by > 60 %
+    assert abs(nu_eff / (CS2 * w.tau) - 1) > 0.3
+
+
+# ---------------------------------------------------------------------------------------------
+# P7 / P8: steady forced Poiseuille flow between halfway bounce-back walls
+# ---------------------------------------------------------------------------------------------
+@pytest.fixture(scope="module")
+def poiseuille(oracle_mod):
+    ny, tau, g = 16, 0.8, 1e-6
+    M = np.zeros((10, 3, ny, 3)); M[0] = 1
+    o = oracle_mod.Oracle(3, ny, 3, tau)
+    o.set_face(W.FACE_YLO, W.BC_BOUNCE_BACK); o.set_face(W.FACE_YHI, W.BC_BOUNCE_BACK)
+    o.set_force((g, 0, 0)); o.set_moments(M)
+    o.step(30000)
+    return o.get_moments(), ny, tau, g
+
+
+def test_P7_poiseuille_parabola(poiseuille):
+    M, ny, tau, g = poiseuille
+    nu = CS2 * (tau - 0.5)
+    ux = M[1][1, :, 1]
+    d2 = ux[2:] - 2 * ux[1:-1] + ux[:-2]
+    np.testing.assert_allclose(d2, -g / nu, rtol=1e-6)             # curvature: nu = cs2 (tau - 1/2)
+    j = np.arange(ny)
+    para = (g / (2 * nu)) * (j + 0.5) * (ny - 0.5 - j)             # walls half a cell outside nodes 0, ny-1
+    slip = ux - para
+    assert np.ptp(slip) < 1e-6 * ux.max()                          # constant offset only
+    assert abs(slip.mean()) < 0.02 * ux.max()                      # wall position: halfway (reading A12)
+    assert np.abs(M[2]).max() < 1e-14 and np.abs(M[3]).max() < 1e-14
+
+
+def test_P8_shear_stress(poiseuille):
+    """Pi_neq_xy = -(tau/3) rho du_x/dy  (sign/scale of the stored non-equilibrium flux)."""
+    M, ny, tau, g = poiseuille
+    ux = M[1][1, :, 1]; rho = M[0][1, :, 1]; pxy = M[7][1, :, 1]
+    dudy = 0.5 * (ux[2:] - ux[:-2])
+    np.testing.assert_allclose(pxy[1:-1], -(tau / 3) * rho[1:-1] * dudy, rtol=1e-4)
+
+
+# ---------------------------------------------------------------------------------------------
+# Lattice symmetries: the step commutes with axis permutations and reflections
+# ---------------------------------------------------------------------------------------------
+def _permute(M, perm):
+    """Relabel axes: new axis a is old axis perm[a] (array axes are z,y,x = 2,1,0)."""
+    vec = [1, 2, 3]
+    ten = {(0, 0): 4, (1, 1): 5, (2, 2): 6, (0, 1): 7, (0, 2): 8, (1, 2): 9}
+    out = np.empty_like(M)
+    arr_perm = tuple(2 - perm[2 - ax] for ax in range(3))          # array axis order for transpose
+    tr = lambda A: np.transpose(A, arr_perm)
+    out[0] = tr(M[0])
+    for a in range(3):
+        out[vec[a]] = tr(M[vec[perm[a]]])
+    for (a, b), k in ten.items():
+        pa, pb = sorted((perm[a], perm[b]))
+        out[k] = tr(M[ten[(pa, pb)]])
+    return np.ascontiguousarray(out)
+
+
+def _reflect(M, ax):
+    """x_ax -> -x_ax."""
+    out = np.flip(M, axis=3 - ax).copy()                           # M axes: field, z, y, x
+    out[1 + ax] *= -1
+    for (a, b), k in {(0, 1): 7, (0, 2): 8, (1, 2): 9}.items():
+        if ax in (a, b):
+            out[k] *= -1
+    return out
+
+
+@pytest.mark.parametrize("perm", [(1, 0, 2), (2, 1, 0), (1, 2, 0)])
+def test_symmetry_axis_permutation(oracle_mod, perm):
+    w = W.random_state(5, 5, 5, seed=13, tau=0.58)
+    a = oracle_mod.Oracle(5, 5, 5, w.tau); a.set_moments(w.moments); a.step(2)
+    b = oracle_mod.Oracle(5, 5, 5, w.tau); b.set_moments(_permute(w.moments, perm)); b.step(2)
+    assert np.abs(_permute(a.get_moments(), perm) - b.get_moments()).max() < 1e-15
+
+
+@pytest.mark.parametrize("ax", [0, 1, 2])
+def test_symmetry_reflection(oracle_mod, ax):
+    w = W.random_state(4, 5, 6, seed=14, tau=0.58)
+    a = oracle_mod.Oracle(4, 5, 6, w.tau); a.set_moments(w.moments); a.step(2)
+    b = oracle_mod.Oracle(4, 5, 6, w.tau); b.set_moments(_reflect(w.moments, ax)); b.step(2)
+    assert np.abs(_reflect(a.get_moments(), ax) - b.get_moments()).max() < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# Open boundaries (readings A13-A16; physically "parity unpinned"): definitional checks only
+# ---------------------------------------------------------------------------------------------
+def test_open_faces_quiescent_stays_quiescent(oracle_mod):
+    M = np.zeros((10, 6, 5, 4)); M[0] = 1
+    o = oracle_mod.Oracle(4, 5, 6, 0.7)
+    for f in range(6):
+        o.set_face(f, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_moments(M); o.step(10)
+    R = o.get_moments()
+    assert np.abs(R - M).max() < 1e-15
+
+
+def test_ghost_fill_definition(oracle_mod):
+    """get_moments returns boundary nodes filled from x_F (clamp to [1, n-2] on open axes), inlet u imposed."""
+    w = W.random_state(5, 6, 7, seed=3)
+    up = np.random.default_rng(1).uniform(-0.02, 0.02, (3, 6, 5))
+    o = oracle_mod.Oracle(5, 6, 7, 0.7)
+    o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.0, 5, 0)
+    o.set_face(W.FACE_ZHI, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_face(W.FACE_XLO, W.BC_OUTLET_ZERO_GRADIENT); o.set_face(W.FACE_XHI, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_moments(w.moments)
+    R = o.get_moments(); M = w.moments
+    np.testing.assert_array_equal(R[:, 1:-1, :, 1:-1], M[:, 1:-1, :, 1:-1])      # interior untouched
+    np.testing.assert_array_equal(R[:, -1, :, 2], M[:, -2, :, 2])                 # outlet copies all 10
+    np.testing.assert_array_equal(R[:, 3, :, 0], M[:, 3, :, 1])
+    np.testing.assert_array_equal(R[:, -1, :, 0], M[:, -2, :, 1])                 # edge: both clamped
+    np.testing.assert_array_equal(R[0, 0], np.pad(M[0, 1, :, 1:-1], ((0, 0), (1, 1)), mode="edge"))  # rho from x_F
+    np.testing.assert_array_equal(R[1:4, 0], up)                                  # inlet wins on the edge too
+    np.testing.assert_array_equal(R[4:, 0, :, 2], M[4:, 1, :, 2])                 # Pi from x_F
+
+
+def test_inlet_noise_is_relative_and_reproducible(oracle_mod):
+    w = W.jet(12, 12, 8, steps=1, dtype="f64", D=6.0)
+    a = _mk(oracle_mod, w); b = _mk(oracle_mod, w)
+    a.step(3); b.step(3)
+    Ra, Rb = a.get_moments(), b.get_moments()
+    np.testing.assert_array_equal(Ra, Rb)
+    uz = Ra[3, 0]; up = w.inlet.u_plane[2]
+    assert np.all(uz[up == 0] == 0)
+    rel = uz[up != 0] / up[up != 0] - 1
+    assert np.abs(rel).max() <= 0.01 * (1 + 1e-12) and np.abs(rel).max() > 0.005
+    idx = (0 * 12 + 5) * 12 + 5                                   # node (5,5,0), t = 3
+    assert abs(uz[5, 5] - up[5, 5] * (1 + 0.01 * oracle_mod.noise_xi(1, 3, idx))) < 1e-18
+
+
+# ---------------------------------------------------------------------------------------------
+# Inlet-noise hash (reading A14) against the published SplitMix64 stream
+# ---------------------------------------------------------------------------------------------
+def test_mix64_published_vectors(oracle_mod):
+    want = [int(l) for l in open(os.path.join(GOLD, "splitmix64_seed1234567.txt")) if l.strip() and l[0] != "#"]
+    s = 1234567
+    for v in want:
+        s = (s + 0x9E3779B97F4A7C15) % 2**64
+        assert oracle_mod.mix64(s) == v
+
+
+def test_noise_xi_range_and_exactness(oracle_mod):
+    xs = np.array([oracle_mod.noise_xi(1, t, i) for t in range(4) for i in range(500)])
+    assert xs.min() >= -1 and xs.max() < 1
+    assert abs(xs.mean()) < 0.05 and abs(xs.std() - 1 / np.sqrt(3)) < 0.03
+    np.testing.assert_array_equal(xs, xs.astype(np.float32).astype(np.float64))   # exact in fp32
+    r = oracle_mod.noise_r24(7, 2, 99)
+    k = oracle_mod.mix64((oracle_mod.mix64(7 ^ ((0x9E3779B97F4A7C15 * 3) % 2**64)) + 99) % 2**64)
+    assert r == k >> 40 and 0 <= r < 2**24
+
+
+# ---------------------------------------------------------------------------------------------
+# Parameters the paper prints
+# ---------------------------------------------------------------------------------------------
+def test_paper_parameter_sets():
+    P = {}
+    for l in open(os.path.join(GOLD, "paper_parameters.txt")):
+        if l.strip() and l[0] != "#":
+            k, v = l.split(); P[k] = float(v)
+    # nu = cs2 (tau - 1/2), PAPER.md:51 vs :258 (tau printed to 4 digits)
+    assert abs(0.5 + 3 * P["jet_nu"] - P["jet_tau"]) < 5e-5
+    assert abs(P["jet_U"] * P["jet_D"] / P["jet_nu"] / P["jet_Re"] - 1) < 0.1
+    assert abs(P["jet_U"] * np.sqrt(3) - P["jet_Ma"]) < 0.005
+    u_tau = np.sqrt(P["chan_g"] * P["chan_H"])
+    assert abs(P["chan_H"] * u_tau / P["chan_nu"] / P["chan_Re_tau"] - 1) < 0.01
+    # BASELINE.json configs[2]/[3] use the same maps
+    w = W.channel(6, 8, 6, steps=1)
+    assert abs(w.tau - (0.5 + 3 * 0.0035 * 4 / 180)) < 1e-15 and abs(w.g[0] - 0.0035**2 / 4) < 1e-20
+    j = W.jet(8, 8, 8, steps=1)
+    assert abs(j.tau - (0.5 + 3 * 0.05 * 20 / 7000)) < 1e-15
