@@ -1,0 +1,143 @@
+/*
+ * tslb.h -- C ABI of libtslb.so: the fused per-timestep sweep of the high-order thread-safe
+ * lattice Boltzmann (TSLB) method on the D3Q27 lattice, hand-written for NVIDIA B200 (sm_100a).
+ *
+ * "PAPER.md:N" = line N of the extracted text of arXiv 2401.17074; DESIGN.md lists how garbled or
+ * silent passages are read ("reading A<n>").
+ *
+ * What the library computes (PAPER.md:68 Eq. 6, :154 Eq. 18, :45 / :126 Eq. 12, :157):
+ *   state      10 hydrodynamic moments per lattice node (rho, u[3], Pi_neq[6]) in two ping-pong
+ *              ("AB flip-flop") buffers; nothing else is stored.
+ *   one step   for every node x and each of the 27 directions c_i, the post-collision population of
+ *              the upstream node x - c_i is rebuilt from that node's moments with the third-order
+ *              Hermite-regularised expansion  f*_i = f_i^eq + (1 - 1/tau) f_i^neq  (Eq. 14, 17, 18),
+ *              pulled, and the new moments rho = sum f, rho u = sum c f, Pi = sum c c f - Pi_eq are
+ *              accumulated and written at x only ("thread-safe").  Body force, halfway
+ *              bounce-back walls, and the non-equilibrium-extrapolation velocity inlet / zero-gradient
+ *              outlet (PAPER.md:181-202 Eq. 22-23, :258) are part of the same step.
+ *
+ * Conventions
+ *   - Every call returns an int status (TSLB_OK = 0).  No exception or abort crosses this boundary;
+ *     output arguments are written only on success.  tslb_last_error() gives a message.
+ *   - Moment arrays exchanged with the caller are plain SoA  [10][nz][ny][nx], x fastest, of the
+ *     context's dtype (float or double), field order
+ *         rho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz      (Pi = NON-equilibrium momentum flux).
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are ordinary host memory
+ *     (pinned memory makes the copies asynchronous).  The library never allocates device memory:
+ *     the caller binds one workspace (tslb_workspace_bytes) and keeps it alive until destroy/rebind.
+ *   - `stream` is a borrowed cudaStream_t passed as void* (NULL = legacy default stream).  All
+ *     device work is enqueued on it and the call returns without synchronising, except the
+ *     *_host calls, which synchronise the stream before returning.
+ *   - A context is not thread-safe; distinct contexts are independent.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one fails with TSLB_ECUDA.
+ */
+#ifndef TSLB_H_
+#define TSLB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tslb_ctx tslb_ctx; /* opaque, owned by the library */
+
+enum { TSLB_F32 = 0, TSLB_F64 = 1 };
+enum { TSLB_OK = 0, TSLB_EINVAL = 1, TSLB_ENOMEM = 2, TSLB_ECUDA = 3, TSLB_ESTATE = 4 };
+enum { TSLB_FACE_XLO = 0, TSLB_FACE_XHI, TSLB_FACE_YLO, TSLB_FACE_YHI, TSLB_FACE_ZLO, TSLB_FACE_ZHI };
+enum {
+    TSLB_BC_PERIODIC = 0,             /* index wraps modulo n on that axis (both faces of the axis)   */
+    TSLB_BC_BOUNCE_BACK = 1,          /* halfway bounce-back no-slip wall half a cell outside the face */
+    TSLB_BC_VELOCITY_INLET = 2,       /* nodes ON the face: u imposed, rho and Pi_neq from x_F          */
+    TSLB_BC_OUTLET_ZERO_GRADIENT = 3, /* nodes ON the face: all 10 moments copied from x_F              */
+    TSLB_BC_BODY_FORCE = 4            /* not a face kind: sets the body acceleration g (face ignored)   */
+};
+/* Which sweep kernel tslb_step uses. AUTO picks the register-marching kernel when the lattice and the
+ * boundary set allow it and the per-direction gather kernel otherwise. */
+enum { TSLB_KERNEL_AUTO = 0, TSLB_KERNEL_GATHER = 1, TSLB_KERNEL_MARCH = 2 };
+
+/* Parameters of TSLB_BC_VELOCITY_INLET (PAPER.md:181 Eq. 22, :270; readings A13, A14).
+ * dev_u_plane: imposed velocity on the face, [3][n_b][n_a] of the context dtype, a = lower in-plane
+ * axis (fastest), b = higher in-plane axis; caller-owned and must outlive the context's use of it.
+ * Component k of node x_B at step t is  u_in,k * (1 + noise_amp * xi(seed, t, lin(x_B)))  when bit k of
+ * noise_component_mask is set, else u_in,k;  xi in [-1,1) = 2 r24 / 2^24 - 1 with r24 the top 24 bits
+ * of mix64(mix64(seed ^ (0x9E3779B97F4A7C15 * (t+1))) + lin), mix64 = SplitMix64's finaliser and
+ * lin = (z*ny + y)*nx + x. */
+typedef struct tslb_inlet_params {
+    const void *dev_u_plane;
+    double noise_amp;
+    uint64_t seed;
+    int32_t noise_component_mask;
+} tslb_inlet_params;
+
+/* Create a context for an nx x ny x nz lattice with BGK relaxation time tau (omega = 1/tau,
+ * nu = (tau - 1/2)/3).  Pure host call (no CUDA).  Defaults: all faces PERIODIC, g = 0.
+ * TSLB_EINVAL: out == NULL, a dimension < 3 or the lattice exceeds 2^31-1 nodes, tau not finite or
+ * <= 0.5, unknown dtype.  TSLB_ENOMEM: host allocation failed. */
+int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out);
+
+/* Free the context (host memory only; the workspace and inlet planes stay the caller's). NULL is a no-op. */
+void tslb_destroy(tslb_ctx *ctx);
+
+/* Bytes of device memory the context needs: two moment buffers of 10*nx*ny*nz elements plus scratch for
+ * the diagnostics reduction and the host-copy staging area.  0 if ctx == NULL. */
+size_t tslb_workspace_bytes(const tslb_ctx *ctx);
+
+/* Give the context its device memory (256-byte aligned, >= tslb_workspace_bytes, caller-owned).  First
+ * call that touches CUDA: queries the current device.  Rebinding discards the state (set_moments again).
+ * TSLB_EINVAL: NULL / misaligned / too small.  TSLB_ECUDA: no usable device. */
+int tslb_bind_workspace(tslb_ctx *ctx, void *dev_ptr, size_t bytes);
+
+/* Load the state at t = 0 from a device array [10][nz][ny][nx] of the context dtype (layout above);
+ * resets the step counter.  Enqueued on `stream`.  TSLB_ESTATE: no workspace bound. */
+int tslb_set_moments(tslb_ctx *ctx, const void *dev_src, void *stream);
+/* Same from host memory (H2D copy through the workspace's staging area, then the same conversion);
+ * synchronises `stream` before returning. */
+int tslb_set_moments_host(tslb_ctx *ctx, const void *host_src, void *stream);
+
+/* Set the kind of one face, or the body force.
+ *   PERIODIC / BOUNCE_BACK / OUTLET_ZERO_GRADIENT : params == NULL.
+ *   VELOCITY_INLET : params -> tslb_inlet_params.
+ *   BODY_FORCE     : params -> const double g[3] (acceleration; adds w_i rho c_i.g / cs^2 to the
+ *                    post-collision population of the SOURCE node, reading A11); face ignored.
+ * TSLB_EINVAL: unknown face/kind, missing params, non-finite g or noise_amp.  Consistency of the whole
+ * set (PERIODIC must be on both faces of an axis) is checked by tslb_step. */
+int tslb_set_boundary(tslb_ctx *ctx, int face, int kind, const void *params);
+
+/* Choose the sweep kernel (TSLB_KERNEL_*).  TSLB_EINVAL if MARCH is forced on a configuration it does not
+ * cover (reported by tslb_step). */
+int tslb_set_kernel(tslb_ctx *ctx, int kernel);
+/* The kernel the next tslb_step would launch (TSLB_KERNEL_GATHER or TSLB_KERNEL_MARCH), or -1. */
+int tslb_active_kernel(const tslb_ctx *ctx);
+
+/* Advance n time steps (n >= 0): n x { boundary-node fill at time t ; fused stream-collide sweep A -> B ;
+ * swap }.  Asynchronous on `stream`; no host<->device traffic.  TSLB_ESTATE before bind/set_moments,
+ * TSLB_EINVAL for n < 0 or an inconsistent boundary set, TSLB_ECUDA on a launch error. */
+int tslb_step(tslb_ctx *ctx, int n, void *stream);
+
+/* Write the current state (boundary nodes filled at the current t first) to a device array of the layout
+ * above. */
+int tslb_get_moments(tslb_ctx *ctx, void *dev_dst, void *stream);
+/* Same to host memory; synchronises `stream` before returning. */
+int tslb_get_moments_host(tslb_ctx *ctx, void *host_dst, void *stream);
+
+/* Mass sum(rho), momentum sum(rho u)[3] and kinetic energy 1/2 sum(rho |u|^2) over the nodes that are not
+ * on an open (inlet/outlet) face, accumulated in fp64 with warp-shuffle reductions and a fixed-order final
+ * pass (bitwise reproducible).  dev_out5: 5 doubles in device memory. */
+int tslb_diagnostics(tslb_ctx *ctx, double *dev_out5, void *stream);
+
+/* Steps taken since the last set_moments, or -1. */
+long long tslb_step_count(const tslb_ctx *ctx);
+/* Number of kernels this context has launched so far (all kinds), for bench.py's gpu_launches. */
+long long tslb_launch_count(const tslb_ctx *ctx);
+/* Message of the last failing call on this context (ctx-owned, valid until the next call); for
+ * ctx == NULL the message of the last failed tslb_create in this thread. */
+const char *tslb_last_error(const tslb_ctx *ctx);
+/* Library version string, e.g. "tslb-b200 0.1 (sm_100a)". */
+const char *tslb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TSLB_H_ */

@@ -1,0 +1,243 @@
+"""Thin ctypes binding of libtslb.so (include/tslb.h): argument marshalling only.
+
+Every step of the TSLB path runs in the CUDA kernels behind the C ABI; PyTorch is used for device
+memory (the workspace and the caller's moment arrays) and streams.  There is NO CPU fallback: if the
+library is missing, or a call needs a CUDA device and none is there, this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libtslb.so")
+
+TSLB_F32, TSLB_F64 = 0, 1
+TSLB_OK, TSLB_EINVAL, TSLB_ENOMEM, TSLB_ECUDA, TSLB_ESTATE = range(5)
+FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
+BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE = range(5)
+KERNEL_AUTO, KERNEL_GATHER, KERNEL_MARCH = range(3)
+KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_MARCH: "march"}
+
+# every symbol include/tslb.h declares (tests check that the library exports all of them)
+SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",
+           "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
+           "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
+           "tslb_launch_count", "tslb_last_error", "tslb_version")
+
+
+class InletParams(C.Structure):
+    _fields_ = [("dev_u_plane", C.c_void_p), ("noise_amp", C.c_double), ("seed", C.c_uint64),
+                ("noise_component_mask", C.c_int32)]
+
+
+class TSLBError(RuntimeError):
+    def __init__(self, code: int, what: str, msg: str):
+        super().__init__("%s failed (status %d): %s" % (what, code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libtslb.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            "%s is missing: build it with `python -m paper_2401_17074_b200.build` (no CPU fallback exists)" % path)
+    lib = C.CDLL(path)
+    vp, ip = C.c_void_p, C.c_int
+    lib.tslb_create.argtypes = [ip, ip, ip, C.c_double, ip, C.POINTER(vp)]
+    lib.tslb_destroy.argtypes = [vp]
+    lib.tslb_destroy.restype = None
+    lib.tslb_workspace_bytes.argtypes = [vp]
+    lib.tslb_workspace_bytes.restype = C.c_size_t
+    lib.tslb_bind_workspace.argtypes = [vp, vp, C.c_size_t]
+    lib.tslb_set_moments.argtypes = [vp, vp, vp]
+    lib.tslb_set_moments_host.argtypes = [vp, vp, vp]
+    lib.tslb_set_boundary.argtypes = [vp, ip, ip, vp]
+    lib.tslb_set_kernel.argtypes = [vp, ip]
+    lib.tslb_active_kernel.argtypes = [vp]
+    lib.tslb_step.argtypes = [vp, ip, vp]
+    lib.tslb_get_moments.argtypes = [vp, vp, vp]
+    lib.tslb_get_moments_host.argtypes = [vp, vp, vp]
+    lib.tslb_diagnostics.argtypes = [vp, vp, vp]
+    lib.tslb_step_count.argtypes = [vp]
+    lib.tslb_step_count.restype = C.c_longlong
+    lib.tslb_launch_count.argtypes = [vp]
+    lib.tslb_launch_count.restype = C.c_longlong
+    lib.tslb_last_error.argtypes = [vp]
+    lib.tslb_last_error.restype = C.c_char_p
+    lib.tslb_version.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def version() -> str:
+    return load_library().tslb_version().decode()
+
+
+def _stream_ptr(stream) -> C.c_void_p:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(int(getattr(stream, "cuda_stream", stream)))
+
+
+class TSLB:
+    """One lattice on the current CUDA device.  Mirrors the C ABI call for call."""
+
+    def __init__(self, nx: int, ny: int, nz: int, tau: float, dtype: str = "f32", bind: bool = True):
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        self.dtype = dtype
+        self.shape = (nz, ny, nx)
+        code = {"f32": TSLB_F32, "f64": TSLB_F64}.get(dtype, -1)
+        rc = self._lib.tslb_create(nx, ny, nz, float(tau), code, C.byref(self._h))
+        if rc:
+            raise TSLBError(rc, "tslb_create", self._lib.tslb_last_error(None).decode())
+        self._keep = {}       # tensors the context points at (workspace, inlet planes)
+        if bind:
+            self.bind_workspace()
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _chk(self, rc: int, what: str):
+        if rc:
+            raise TSLBError(rc, what, self._lib.tslb_last_error(self._h).decode())
+
+    @property
+    def torch_dtype(self):
+        import torch
+        return torch.float32 if self.dtype == "f32" else torch.float64
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.tslb_destroy(self._h)
+            self._h = C.c_void_p()
+            self._keep.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check_tensor(self, t, what, shape=None):
+        if not t.is_cuda:
+            raise ValueError("%s must be a CUDA tensor" % what)
+        if t.dtype != self.torch_dtype or not t.is_contiguous():
+            raise ValueError("%s must be contiguous %s" % (what, self.torch_dtype))
+        if shape is not None and tuple(t.shape) != tuple(shape):
+            raise ValueError("%s has shape %s, expected %s" % (what, tuple(t.shape), tuple(shape)))
+
+    # -- C ABI ------------------------------------------------------------------------------
+    def workspace_bytes(self) -> int:
+        return int(self._lib.tslb_workspace_bytes(self._h))
+
+    def bind_workspace(self, workspace=None):
+        import torch
+        if workspace is None:
+            if not torch.cuda.is_available():
+                raise TSLBError(TSLB_ECUDA, "tslb_bind_workspace", "no CUDA device (there is no CPU fallback)")
+            workspace = torch.empty(self.workspace_bytes(), dtype=torch.uint8, device="cuda")
+        self._chk(self._lib.tslb_bind_workspace(self._h, C.c_void_p(workspace.data_ptr()), workspace.numel()),
+                  "tslb_bind_workspace")
+        self._keep["ws"] = workspace
+
+    def set_moments(self, M, stream=None):
+        """M: CUDA tensor [10][nz][ny][nx] of the context dtype."""
+        self._check_tensor(M, "moments", (10,) + self.shape)
+        self._chk(self._lib.tslb_set_moments(self._h, C.c_void_p(M.data_ptr()), _stream_ptr(stream)), "tslb_set_moments")
+
+    def set_moments_host(self, M, stream=None):
+        """M: host tensor or numpy array [10][nz][ny][nx] of the context dtype (pinned = async copy)."""
+        ptr, keep = _host_ptr(M, self, (10,) + self.shape)
+        self._chk(self._lib.tslb_set_moments_host(self._h, ptr, _stream_ptr(stream)), "tslb_set_moments_host")
+
+    def set_boundary(self, face: int, kind: int, u_plane=None, noise_amp: float = 0.0, seed: int = 0,
+                     noise_mask: int = 0):
+        if kind == BC_VELOCITY_INLET:
+            if u_plane is None:
+                raise ValueError("VELOCITY_INLET needs u_plane")
+            self._check_tensor(u_plane, "u_plane")
+            ip = InletParams(C.c_void_p(u_plane.data_ptr()), float(noise_amp), int(seed), int(noise_mask))
+            self._chk(self._lib.tslb_set_boundary(self._h, face, kind, C.cast(C.byref(ip), C.c_void_p)),
+                      "tslb_set_boundary")
+            self._keep["inlet%d" % face] = u_plane
+        else:
+            self._chk(self._lib.tslb_set_boundary(self._h, face, kind, None), "tslb_set_boundary")
+
+    def set_body_force(self, g: Sequence[float]):
+        arr = (C.c_double * 3)(*[float(v) for v in g])
+        self._chk(self._lib.tslb_set_boundary(self._h, 0, BC_BODY_FORCE, C.cast(arr, C.c_void_p)), "tslb_set_boundary")
+
+    def set_kernel(self, kernel: int):
+        self._chk(self._lib.tslb_set_kernel(self._h, int(kernel)), "tslb_set_kernel")
+
+    def active_kernel(self) -> int:
+        return int(self._lib.tslb_active_kernel(self._h))
+
+    def step(self, n: int = 1, stream=None):
+        self._chk(self._lib.tslb_step(self._h, int(n), _stream_ptr(stream)), "tslb_step")
+
+    def get_moments(self, out=None, stream=None):
+        import torch
+        if out is None:
+            out = torch.empty((10,) + self.shape, dtype=self.torch_dtype, device="cuda")
+        self._check_tensor(out, "out", (10,) + self.shape)
+        self._chk(self._lib.tslb_get_moments(self._h, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "tslb_get_moments")
+        return out
+
+    def get_moments_host(self, out, stream=None):
+        ptr, keep = _host_ptr(out, self, (10,) + self.shape)
+        self._chk(self._lib.tslb_get_moments_host(self._h, ptr, _stream_ptr(stream)), "tslb_get_moments_host")
+        return out
+
+    def diagnostics(self, stream=None):
+        """(mass, px, py, pz, kinetic energy) as a CUDA fp64 tensor of 5."""
+        import torch
+        out = torch.empty(5, dtype=torch.float64, device="cuda")
+        self._chk(self._lib.tslb_diagnostics(self._h, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "tslb_diagnostics")
+        return out
+
+    @property
+    def step_count(self) -> int:
+        return int(self._lib.tslb_step_count(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.tslb_launch_count(self._h))
+
+
+def _host_ptr(M, ctx: TSLB, shape):
+    """Pointer to a contiguous host array (torch CPU tensor or numpy array) of the context dtype."""
+    import numpy as np
+    if hasattr(M, "data_ptr"):
+        if M.is_cuda or M.dtype != ctx.torch_dtype or not M.is_contiguous() or tuple(M.shape) != tuple(shape):
+            raise ValueError("host tensor must be contiguous CPU %s of shape %s" % (ctx.torch_dtype, tuple(shape)))
+        return C.c_void_p(M.data_ptr()), M
+    want = np.float32 if ctx.dtype == "f32" else np.float64
+    if not isinstance(M, np.ndarray) or M.dtype != want or not M.flags["C_CONTIGUOUS"] or M.shape != tuple(shape):
+        raise ValueError("host array must be C-contiguous %s of shape %s" % (want.__name__, tuple(shape)))
+    return C.c_void_p(M.ctypes.data), M
+
+
+def from_workload(w, kernel: int = KERNEL_AUTO) -> TSLB:
+    """Context configured (boundary set, force, kernel choice) for a workloads.Workload; state not loaded."""
+    import torch
+    sim = TSLB(w.nx, w.ny, w.nz, w.tau, w.dtype)
+    for face, kind in w.faces.items():
+        if w.inlet is not None and face == w.inlet.face:
+            up = torch.from_numpy(w.inlet.u_plane).to("cuda")
+            sim.set_boundary(face, kind, up, w.inlet.noise_amp, w.inlet.seed, w.inlet.noise_mask)
+        else:
+            sim.set_boundary(face, kind)
+    if any(w.g):
+        sim.set_body_force(w.g)
+    sim.set_kernel(kernel)
+    return sim

@@ -1,0 +1,372 @@
+// kernels_basic.cu -- the per-direction "gather" sweep (covers every boundary set and lattice shape),
+// the boundary-node fill, layout import/export and the diagnostics reduction.  sm_100a.
+//
+// Arithmetic follows PAPER.md:154 (Eq. 18) with the readings of DESIGN.md; contractions are reduced by
+// hand.  Internal storage is the SHIFTED form: field 0 holds drho = rho - 1
+// and populations are carried as f_i - w_i, so that fp32 rounding is relative to the perturbation and
+// not to 1.  The w_i-part is added back in closed form:
+// sum_i w_i = 1, sum_i w_i c_i = 0, sum_i w_i c_i c_i = I/3.
+#include "tslb_internal.h"
+
+namespace {
+
+template <typename T>
+struct Site {
+    T dr, ux, uy, uz, pxx, pyy, pzz, pxy, pxz, pyz;
+};
+
+template <typename T>
+__device__ __forceinline__ Site<T> load_site(const T *__restrict__ A, size_t N, size_t i)
+{
+    Site<T> s;
+    s.dr = __ldg(A + i);
+    s.ux = __ldg(A + N + i);
+    s.uy = __ldg(A + 2 * N + i);
+    s.uz = __ldg(A + 3 * N + i);
+    s.pxx = __ldg(A + 4 * N + i);
+    s.pyy = __ldg(A + 5 * N + i);
+    s.pzz = __ldg(A + 6 * N + i);
+    s.pxy = __ldg(A + 7 * N + i);
+    s.pxz = __ldg(A + 8 * N + i);
+    s.pyz = __ldg(A + 9 * N + i);
+    return s;
+}
+
+// f*_c(M) - w_c for direction (sgn*cx, sgn*cy, sgn*cz); cx,cy,cz are compile-time after unrolling.
+//   f* = w [ rho (1 + 3 c.(u+g) + 4.5((c.u)^2 - |u|^2/3) + 4.5((c.u)^3 - (c.u)|u|^2))          Eq. 14
+//          + beta (4.5 (cPc - trP/3) + 4.5 (3 cPc c.u - trP c.u - 2 cPu)) ]                      Eq. 17
+// Terms odd in c change sign with sgn (bounce-back evaluates the opposite direction at the own node).
+template <typename T>
+__device__ __forceinline__ T fstar_shifted(const Site<T> &m, int cx, int cy, int cz, T sgn, T w, T beta,
+                                           const T *g)
+{
+    const T fx = (T)cx, fy = (T)cy, fz = (T)cz;
+    const T rho = (T)1 + m.dr;
+    const T cu = fx * m.ux + fy * m.uy + fz * m.uz;
+    const T cg = fx * g[0] + fy * g[1] + fz * g[2];
+    const T uu = m.ux * m.ux + m.uy * m.uy + m.uz * m.uz;
+    const T trP = m.pxx + m.pyy + m.pzz;
+    const T cPx = fx * m.pxx + fy * m.pxy + fz * m.pxz;  // (c.P)_x
+    const T cPy = fx * m.pxy + fy * m.pyy + fz * m.pyz;
+    const T cPz = fx * m.pxz + fy * m.pyz + fz * m.pzz;
+    const T cPc = cPx * fx + cPy * fy + cPz * fz;
+    const T cPu = cPx * m.ux + cPy * m.uy + cPz * m.uz;
+    const T even_eq = (T)4.5 * cu * cu - (T)1.5 * uu;
+    const T odd_eq = (T)3 * (cu + cg) + (T)4.5 * cu * (cu * cu - uu);
+    const T even_ne = (T)4.5 * cPc - (T)1.5 * trP;
+    const T odd_ne = (T)4.5 * ((T)3 * cPc * cu - trP * cu - (T)2 * cPu);
+    return w * (m.dr + rho * (even_eq + sgn * odd_eq) + beta * (even_ne + sgn * odd_ne));
+}
+
+__device__ __forceinline__ bool is_open_kind(int k)
+{
+    return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT;
+}
+
+template <typename P>
+__device__ __forceinline__ bool on_open_face(const P &p, int x, int y, int z)
+{
+    return (x == 0 && is_open_kind(p.kind[0])) || (x == p.nx - 1 && is_open_kind(p.kind[1])) ||
+           (y == 0 && is_open_kind(p.kind[2])) || (y == p.ny - 1 && is_open_kind(p.kind[3])) ||
+           (z == 0 && is_open_kind(p.kind[4])) || (z == p.nz - 1 && is_open_kind(p.kind[5]));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Gather sweep: one thread per node, 27 upstream nodes read straight from global memory (L1/L2
+// provide the reuse).  SURVEY.md 8(a) rows a1-a8 in one kernel.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__ A, T *__restrict__ B,
+                                                            SweepParams<T> p)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= p.nx || y >= p.ny) return;
+    const size_t N = (size_t)p.nx * p.ny * p.nz;
+    const size_t ip = ((size_t)z * p.ny + y) * p.nx + x;
+    const Site<T> own = load_site(A, N, ip);
+
+    if (on_open_face(p, x, y, z)) {  // boundary nodes are not advanced: M_{t+1}(x_B) := M_t(x_B)
+        B[ip] = own.dr;
+        B[N + ip] = own.ux; B[2 * N + ip] = own.uy; B[3 * N + ip] = own.uz;
+        B[4 * N + ip] = own.pxx; B[5 * N + ip] = own.pyy; B[6 * N + ip] = own.pzz;
+        B[7 * N + ip] = own.pxy; B[8 * N + ip] = own.pxz; B[9 * N + ip] = own.pyz;
+        return;
+    }
+
+    // upstream coordinate x - c for c = -1, 0, +1 (index c+1), with periodic wrap; bounce flags
+    int sx[3], sy[3], sz[3];
+    bool bx[3], by[3], bz[3];
+    {
+        const int n[3] = {p.nx, p.ny, p.nz};
+        const int q[3] = {x, y, z};
+        int *s[3] = {sx, sy, sz};
+        bool *b[3] = {bx, by, bz};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            s[a][1] = q[a]; b[a][1] = false;
+            // c = +1 pulls from q-1
+            b[a][2] = false;
+            if (q[a] > 0) s[a][2] = q[a] - 1;
+            else if (p.kind[2 * a] == TSLB_BC_PERIODIC) s[a][2] = n[a] - 1;
+            else { s[a][2] = q[a]; b[a][2] = (p.kind[2 * a] == TSLB_BC_BOUNCE_BACK); }
+            // c = -1 pulls from q+1
+            b[a][0] = false;
+            if (q[a] < n[a] - 1) s[a][0] = q[a] + 1;
+            else if (p.kind[2 * a + 1] == TSLB_BC_PERIODIC) s[a][0] = 0;
+            else { s[a][0] = q[a]; b[a][0] = (p.kind[2 * a + 1] == TSLB_BC_BOUNCE_BACK); }
+        }
+    }
+
+    T dR = 0, Jx = 0, Jy = 0, Jz = 0, Sxx = 0, Syy = 0, Szz = 0, Sxy = 0, Sxz = 0, Syz = 0;
+#pragma unroll
+    for (int cz = -1; cz <= 1; ++cz)
+#pragma unroll
+        for (int cy = -1; cy <= 1; ++cy)
+#pragma unroll
+            for (int cx = -1; cx <= 1; ++cx) {
+                const bool bounced = bx[cx + 1] | by[cy + 1] | bz[cz + 1];
+                const T w = (T)((cx ? 1.0 / 6 : 2.0 / 3) * (cy ? 1.0 / 6 : 2.0 / 3) * (cz ? 1.0 / 6 : 2.0 / 3));
+                T f;
+                if (cx == 0 && cy == 0 && cz == 0) {
+                    f = fstar_shifted(own, 0, 0, 0, (T)1, w, p.beta, p.g);
+                } else {
+                    // halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) from the node's own moments
+                    const size_t is = bounced ? ip : ((size_t)sz[cz + 1] * p.ny + sy[cy + 1]) * p.nx + sx[cx + 1];
+                    const Site<T> m = load_site(A, N, is);
+                    f = fstar_shifted(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, p.g);
+                }
+                dR += f;                                  // arrival direction c_i in every sum
+                if (cx) Jx += (T)cx * f;
+                if (cy) Jy += (T)cy * f;
+                if (cz) Jz += (T)cz * f;
+                if (cx) Sxx += f;
+                if (cy) Syy += f;
+                if (cz) Szz += f;
+                if (cx && cy) Sxy += (T)(cx * cy) * f;
+                if (cx && cz) Sxz += (T)(cx * cz) * f;
+                if (cy && cz) Syz += (T)(cy * cz) * f;
+            }
+    // rho' = 1 + dR; u' = J / rho'; Pi' = S - rho'(I/3 + u'u') with S_aa = dS_aa + 1/3   (Eq. 12)
+    const T rho = (T)1 + dR;
+    const T inv = (T)1 / rho;
+    const T ux = Jx * inv, uy = Jy * inv, uz = Jz * inv;
+    const T third = (T)(1.0 / 3.0);
+    B[ip] = dR;
+    B[N + ip] = ux; B[2 * N + ip] = uy; B[3 * N + ip] = uz;
+    B[4 * N + ip] = Sxx - third * dR - rho * ux * ux;
+    B[5 * N + ip] = Syy - third * dR - rho * uy * uy;
+    B[6 * N + ip] = Szz - third * dR - rho * uz * uz;
+    B[7 * N + ip] = Sxy - rho * ux * uy;
+    B[8 * N + ip] = Sxz - rho * ux * uz;
+    B[9 * N + ip] = Syz - rho * uy * uz;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Boundary-node fill at time t (PAPER.md:181-196 Eq. 22-23, :202, :258; readings A13-A16):
+// every node on an INLET/OUTLET face takes all 10 moments of x_F (its coordinates on open axes
+// clamped to [1, n-2]); on an inlet face the velocity is then imposed (with seeded noise).
+// One thread per (face, in-plane position); a node on several open faces is handled by the
+// lowest-index one.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t mix64(uint64_t z)  // SplitMix64 finaliser (Vigna, public domain)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+template <typename T>
+__global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p, int plane_max)
+{
+    const int f = blockIdx.y;
+    if (!is_open_kind(p.kind[f])) return;
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n[3] = {p.nx, p.ny, p.nz};
+    const int ax = f >> 1;
+    const int a = (ax == 0) ? 1 : 0;
+    const int b = (ax == 2) ? 1 : 2;
+    if (j >= n[a] * n[b]) return;
+    int q[3];
+    q[ax] = (f & 1) ? n[ax] - 1 : 0;
+    q[a] = j % n[a];
+    q[b] = j / n[a];
+    // lowest-index open face containing this node does the work
+    for (int f2 = 0; f2 < f; ++f2) {
+        const int ax2 = f2 >> 1;
+        if (is_open_kind(p.kind[f2]) && q[ax2] == ((f2 & 1) ? n[ax2] - 1 : 0)) return;
+    }
+    int r[3] = {q[0], q[1], q[2]};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        if (r[d] == 0 && is_open_kind(p.kind[2 * d])) r[d] = 1;
+        if (r[d] == n[d] - 1 && is_open_kind(p.kind[2 * d + 1])) r[d] = n[d] - 2;
+    }
+    const size_t N = (size_t)p.nx * p.ny * p.nz;
+    const size_t ib = ((size_t)q[2] * p.ny + q[1]) * p.nx + q[0];
+    const size_t iF = ((size_t)r[2] * p.ny + r[1]) * p.nx + r[0];
+#pragma unroll
+    for (int k = 0; k < TSLB_NF; ++k) M[k * N + ib] = M[k * N + iF];
+    for (int f2 = 0; f2 < 6; ++f2) {
+        if (p.kind[f2] != TSLB_BC_VELOCITY_INLET) continue;
+        const int ax2 = f2 >> 1;
+        if (q[ax2] != ((f2 & 1) ? n[ax2] - 1 : 0)) continue;
+        const int a2 = (ax2 == 0) ? 1 : 0, b2 = (ax2 == 2) ? 1 : 2;
+        const size_t pl = (size_t)n[a2] * n[b2];
+        const size_t jj = (size_t)q[b2] * n[a2] + q[a2];
+        uint64_t k64 = mix64(p.inlet[f2].seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(p.t + 1)));
+        k64 = mix64(k64 + (uint64_t)ib);
+        const double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
+        const T *up = (const T *)p.inlet[f2].u_plane;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            double v = (double)up[k * pl + jj];
+            if (p.inlet[f2].mask & (1 << k)) v *= 1.0 + p.inlet[f2].noise_amp * xi;
+            M[(1 + k) * N + ib] = (T)v;
+        }
+        break;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// API layout <-> internal layout (field 0: rho <-> rho - 1; exact for 0.5 <= rho <= 2)
+// ---------------------------------------------------------------------------------------------
+template <typename T, int DIR>
+__global__ void convert_kernel(const T *__restrict__ src, T *__restrict__ dst, size_t N)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < TSLB_NF * N; i += stride) {
+        T v = src[i];
+        if (i < N) v = DIR > 0 ? v - (T)1 : v + (T)1;
+        dst[i] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Diagnostics: fp64 accumulation, warp shuffles, fixed-order final pass.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(TSLB_DIAG_THREADS) diag_partial_kernel(const T *__restrict__ A, FillParams p,
+                                                                          double *__restrict__ partial)
+{
+    const size_t N = (size_t)p.nx * p.ny * p.nz;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    double acc[5] = {0, 0, 0, 0, 0};
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
+        const int x = (int)(i % p.nx);
+        const size_t r = i / p.nx;
+        const int y = (int)(r % p.ny), z = (int)(r / p.ny);
+        if (on_open_face(p, x, y, z)) continue;
+        const double rho = 1.0 + (double)A[i];
+        const double ux = A[N + i], uy = A[2 * N + i], uz = A[3 * N + i];
+        acc[0] += rho; acc[1] += rho * ux; acc[2] += rho * uy; acc[3] += rho * uz;
+        acc[4] += 0.5 * rho * (ux * ux + uy * uy + uz * uz);
+    }
+    __shared__ double sh[5][TSLB_DIAG_THREADS / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const double v = warp_sum(acc[k]);
+        if (lane == 0) sh[k][wid] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 5) {
+        double v = 0;
+        for (int w = 0; w < TSLB_DIAG_THREADS / 32; ++w) v += sh[threadIdx.x][w];
+        partial[threadIdx.x * gridDim.x + blockIdx.x] = v;
+    }
+}
+
+__global__ void diag_final_kernel(const double *__restrict__ partial, int nblocks, double *__restrict__ out5)
+{
+    // one warp per quantity; lane-strided partial sums in a fixed order, then a shuffle tree
+    const int k = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double v = 0;
+    for (int b = lane; b < nblocks; b += 32) v += partial[k * nblocks + b];
+    v = warp_sum(v);
+    if (lane == 0) out5[k] = v;
+}
+
+template <typename T>
+SweepParams<T> make_params(const tslb_ctx *c)
+{
+    SweepParams<T> p;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
+    p.beta = (T)(1.0 - c->omega);
+    for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
+    return p;
+}
+
+FillParams make_fill(const tslb_ctx *c)
+{
+    FillParams p;
+    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    for (int f = 0; f < 6; ++f) { p.kind[f] = c->kind[f]; p.inlet[f] = c->inlet[f]; }
+    p.t = c->t;
+    return p;
+}
+
+}  // namespace
+
+cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st)
+{
+    dim3 block(64, 2, 1);
+    dim3 grid((c->nx + block.x - 1) / block.x, (c->ny + block.y - 1) / block.y, c->nz);
+    if (c->dtype == TSLB_F32)
+        sweep_gather_kernel<float><<<grid, block, 0, st>>>((const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur],
+                                                          make_params<float>(c));
+    else
+        sweep_gather_kernel<double><<<grid, block, 0, st>>>((const double *)c->buf[c->cur],
+                                                           (double *)c->buf[1 - c->cur], make_params<double>(c));
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st)
+{
+    bool any = false;
+    for (int f = 0; f < 6; ++f) any |= (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT);
+    if (!any) return cudaSuccess;
+    int pm = c->nx * c->ny;
+    if (c->nx * c->nz > pm) pm = c->nx * c->nz;
+    if (c->ny * c->nz > pm) pm = c->ny * c->nz;
+    dim3 block(128), grid((pm + 127) / 128, 6);
+    if (c->dtype == TSLB_F32) fill_boundary_kernel<float><<<grid, block, 0, st>>>((float *)buf, make_fill(c), pm);
+    else fill_boundary_kernel<double><<<grid, block, 0, st>>>((double *)buf, make_fill(c), pm);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+template <int DIR>
+static cudaError_t launch_convert(tslb_ctx *c, const void *src, void *dst, cudaStream_t st)
+{
+    const size_t N = tslb_sites(c);
+    size_t blocks = (TSLB_NF * N + 255) / 256;
+    if (blocks > (size_t)c->sm_count * 16) blocks = (size_t)c->sm_count * 16;
+    if (c->dtype == TSLB_F32) convert_kernel<float, DIR><<<(unsigned)blocks, 256, 0, st>>>((const float *)src, (float *)dst, N);
+    else convert_kernel<double, DIR><<<(unsigned)blocks, 256, 0, st>>>((const double *)src, (double *)dst, N);
+    c->launches++;
+    return cudaGetLastError();
+}
+cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<+1>(c, src, dst, st); }
+cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<-1>(c, src, dst, st); }
+
+cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st)
+{
+    if (c->dtype == TSLB_F32)
+        diag_partial_kernel<float><<<TSLB_DIAG_BLOCKS, TSLB_DIAG_THREADS, 0, st>>>((const float *)c->buf[c->cur], make_fill(c), c->scratch);
+    else
+        diag_partial_kernel<double><<<TSLB_DIAG_BLOCKS, TSLB_DIAG_THREADS, 0, st>>>((const double *)c->buf[c->cur], make_fill(c), c->scratch);
+    diag_final_kernel<<<1, 160, 0, st>>>(c->scratch, TSLB_DIAG_BLOCKS, dev_out5);
+    c->launches += 2;
+    return cudaGetLastError();
+}

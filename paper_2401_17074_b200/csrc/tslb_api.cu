@@ -1,0 +1,244 @@
+// tslb_api.cu -- the C ABI of include/tslb.h: context, validation, launch logic.  No arithmetic of the
+// method lives here; every step of the path runs in the kernels.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include "tslb_internal.h"
+
+namespace {
+
+thread_local char g_create_err[256] = "";
+
+int fail(tslb_ctx *c, int code, const char *fmt, const char *detail = "")
+{
+    char *dst = c ? c->err : g_create_err;
+    snprintf(dst, 256, fmt, detail);
+    return code;
+}
+
+int cuda_fail(tslb_ctx *c, const char *what, cudaError_t e)
+{
+    snprintf(c->err, sizeof c->err, "%s: %s", what, cudaGetErrorString(e));
+    return TSLB_ECUDA;
+}
+
+size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+size_t buffer_bytes(const tslb_ctx *c) { return align256(TSLB_NF * tslb_sites(c) * tslb_elem(c)); }
+
+int check_ready(tslb_ctx *c, bool need_state)
+{
+    if (!c) return TSLB_EINVAL;
+    if (!c->ws) return fail(c, TSLB_ESTATE, "no workspace bound (call tslb_bind_workspace)");
+    if (need_state && !c->have_state) return fail(c, TSLB_ESTATE, "no state loaded (call tslb_set_moments)");
+    return TSLB_OK;
+}
+
+int check_boundary_set(tslb_ctx *c)
+{
+    for (int ax = 0; ax < 3; ++ax)
+        if ((c->kind[2 * ax] == TSLB_BC_PERIODIC) != (c->kind[2 * ax + 1] == TSLB_BC_PERIODIC))
+            return fail(c, TSLB_EINVAL, "PERIODIC must be set on both faces of an axis");
+    return TSLB_OK;
+}
+
+int pick_kernel(const tslb_ctx *c, const char **why)
+{
+    const bool ok = tslb_march_supported(c, why);
+    if (c->kernel_req == TSLB_KERNEL_GATHER) return TSLB_KERNEL_GATHER;
+    if (c->kernel_req == TSLB_KERNEL_MARCH) return ok ? TSLB_KERNEL_MARCH : -1;
+    return ok ? TSLB_KERNEL_MARCH : TSLB_KERNEL_GATHER;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out)
+{
+    if (!out) return fail(nullptr, TSLB_EINVAL, "out == NULL");
+    if (nx < 3 || ny < 3 || nz < 3) return fail(nullptr, TSLB_EINVAL, "every dimension must be >= 3");
+    if ((double)nx * ny * nz > 2147483647.0) return fail(nullptr, TSLB_EINVAL, "lattice exceeds 2^31-1 nodes");
+    if (!isfinite(tau) || !(tau > 0.5)) return fail(nullptr, TSLB_EINVAL, "tau must be finite and > 0.5");
+    if (dtype != TSLB_F32 && dtype != TSLB_F64) return fail(nullptr, TSLB_EINVAL, "unknown dtype");
+    tslb_ctx *c = (tslb_ctx *)calloc(1, sizeof *c);
+    if (!c) return fail(nullptr, TSLB_ENOMEM, "host allocation failed");
+    c->nx = nx; c->ny = ny; c->nz = nz; c->dtype = dtype;
+    c->tau = tau; c->omega = 1.0 / tau;
+    c->kernel_req = TSLB_KERNEL_AUTO;
+    c->sm_count = 148;
+    *out = c;
+    return TSLB_OK;
+}
+
+void tslb_destroy(tslb_ctx *c) { free(c); }
+
+size_t tslb_workspace_bytes(const tslb_ctx *c)
+{
+    if (!c) return 0;
+    return 2 * buffer_bytes(c) + align256(5 * TSLB_DIAG_BLOCKS * sizeof(double));
+}
+
+int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
+{
+    if (!c) return TSLB_EINVAL;
+    if (!dev_ptr) return fail(c, TSLB_EINVAL, "workspace pointer is NULL");
+    if (((uintptr_t)dev_ptr & 255) != 0) return fail(c, TSLB_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < tslb_workspace_bytes(c)) return fail(c, TSLB_EINVAL, "workspace smaller than tslb_workspace_bytes");
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(c, "cudaGetDevice", e);
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(c, "cudaDeviceGetAttribute", e);
+    c->sm_count = sms > 0 ? sms : 148;
+    c->ws = dev_ptr; c->ws_bytes = bytes;
+    c->buf[0] = dev_ptr;
+    c->buf[1] = (char *)dev_ptr + buffer_bytes(c);
+    c->scratch = (double *)((char *)dev_ptr + 2 * buffer_bytes(c));
+    c->cur = 0; c->t = 0; c->have_state = 0;
+    return TSLB_OK;
+}
+
+int tslb_set_moments(tslb_ctx *c, const void *dev_src, void *stream)
+{
+    int rc = check_ready(c, false);
+    if (rc) return rc;
+    if (!dev_src) return fail(c, TSLB_EINVAL, "dev_src == NULL");
+    cudaError_t e = tslb_launch_import(c, dev_src, c->buf[0], (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
+    c->cur = 0; c->t = 0; c->have_state = 1;
+    return TSLB_OK;
+}
+
+int tslb_set_moments_host(tslb_ctx *c, const void *host_src, void *stream)
+{
+    int rc = check_ready(c, false);
+    if (rc) return rc;
+    if (!host_src) return fail(c, TSLB_EINVAL, "host_src == NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    // buffer 1 is free while the state is being replaced: use it as the staging area
+    cudaError_t e = cudaMemcpyAsync(c->buf[1], host_src, TSLB_NF * tslb_sites(c) * tslb_elem(c), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(c, "H2D copy", e);
+    e = tslb_launch_import(c, c->buf[1], c->buf[0], st);
+    if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, "cudaStreamSynchronize", e);
+    c->cur = 0; c->t = 0; c->have_state = 1;
+    return TSLB_OK;
+}
+
+int tslb_set_boundary(tslb_ctx *c, int face, int kind, const void *params)
+{
+    if (!c) return TSLB_EINVAL;
+    if (kind == TSLB_BC_BODY_FORCE) {
+        if (!params) return fail(c, TSLB_EINVAL, "BODY_FORCE needs params -> double g[3]");
+        const double *g = (const double *)params;
+        for (int a = 0; a < 3; ++a)
+            if (!isfinite(g[a])) return fail(c, TSLB_EINVAL, "body force must be finite");
+        for (int a = 0; a < 3; ++a) c->g[a] = g[a];
+        return TSLB_OK;
+    }
+    if (face < 0 || face > 5) return fail(c, TSLB_EINVAL, "unknown face");
+    if (kind < 0 || kind > TSLB_BC_OUTLET_ZERO_GRADIENT) return fail(c, TSLB_EINVAL, "unknown boundary kind");
+    if (kind == TSLB_BC_VELOCITY_INLET) {
+        if (!params) return fail(c, TSLB_EINVAL, "VELOCITY_INLET needs params -> tslb_inlet_params");
+        const tslb_inlet_params *ip = (const tslb_inlet_params *)params;
+        if (!ip->dev_u_plane) return fail(c, TSLB_EINVAL, "inlet dev_u_plane == NULL");
+        if (!isfinite(ip->noise_amp)) return fail(c, TSLB_EINVAL, "inlet noise_amp must be finite");
+        c->inlet[face].u_plane = ip->dev_u_plane;
+        c->inlet[face].noise_amp = ip->noise_amp;
+        c->inlet[face].seed = ip->seed;
+        c->inlet[face].mask = ip->noise_component_mask;
+    } else {
+        memset(&c->inlet[face], 0, sizeof c->inlet[face]);
+    }
+    c->kind[face] = kind;
+    return TSLB_OK;
+}
+
+int tslb_set_kernel(tslb_ctx *c, int kernel)
+{
+    if (!c) return TSLB_EINVAL;
+    if (kernel < TSLB_KERNEL_AUTO || kernel > TSLB_KERNEL_MARCH) return fail(c, TSLB_EINVAL, "unknown kernel id");
+    c->kernel_req = kernel;
+    return TSLB_OK;
+}
+
+int tslb_active_kernel(const tslb_ctx *c)
+{
+    if (!c) return -1;
+    const char *why = "";
+    return pick_kernel(c, &why);
+}
+
+int tslb_step(tslb_ctx *c, int n, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (n < 0) return fail(c, TSLB_EINVAL, "n < 0");
+    rc = check_boundary_set(c);
+    if (rc) return rc;
+    const char *why = "";
+    const int k = pick_kernel(c, &why);
+    if (k < 0) return fail(c, TSLB_EINVAL, "TSLB_KERNEL_MARCH does not cover this configuration: %s", why);
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int s = 0; s < n; ++s) {
+        cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);           // step 1: boundary nodes at time t
+        if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+        e = (k == TSLB_KERNEL_MARCH) ? tslb_launch_march(c, st) : tslb_launch_gather(c, st);  // steps 2-4
+        if (e != cudaSuccess) return cuda_fail(c, "sweep kernel", e);
+        c->cur = 1 - c->cur;                                               // step 5: AB flip-flop
+        c->t += 1;
+    }
+    return TSLB_OK;
+}
+
+int tslb_get_moments(tslb_ctx *c, void *dev_dst, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (!dev_dst) return fail(c, TSLB_EINVAL, "dev_dst == NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_export(c, c->buf[c->cur], dev_dst, st);
+    if (e != cudaSuccess) return cuda_fail(c, "export kernel", e);
+    return TSLB_OK;
+}
+
+int tslb_get_moments_host(tslb_ctx *c, void *host_dst, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (!host_dst) return fail(c, TSLB_EINVAL, "host_dst == NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    // the other buffer holds only the stale time t-1 state: use it as the staging area
+    e = tslb_launch_export(c, c->buf[c->cur], c->buf[1 - c->cur], st);
+    if (e != cudaSuccess) return cuda_fail(c, "export kernel", e);
+    e = cudaMemcpyAsync(host_dst, c->buf[1 - c->cur], TSLB_NF * tslb_sites(c) * tslb_elem(c), cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return cuda_fail(c, "D2H copy", e);
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, "cudaStreamSynchronize", e);
+    return TSLB_OK;
+}
+
+int tslb_diagnostics(tslb_ctx *c, double *dev_out5, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (!dev_out5) return fail(c, TSLB_EINVAL, "dev_out5 == NULL");
+    cudaError_t e = tslb_launch_diag(c, dev_out5, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "diagnostics kernels", e);
+    return TSLB_OK;
+}
+
+long long tslb_step_count(const tslb_ctx *c) { return c && c->have_state ? c->t : -1; }
+long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
+const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err : g_create_err; }
+const char *tslb_version(void) { return "tslb-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

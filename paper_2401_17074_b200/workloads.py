@@ -151,25 +151,28 @@ def jet(nx: int = 256, ny: int = 256, nz: int = 768, steps: int = 1000, dtype: s
                     M.astype(_NP_DTYPE[dtype]), faces=faces, inlet=inlet)
 
 
-def throughput(n: int = 512, dtype: str = "f32", steps: int = 200) -> Workload:
+def throughput(n: int = 512, dtype: str = "f32", steps: int = 200, edge: Optional[int] = None) -> Workload:
     """configs[4]: periodic cube, random-phase Taylor-Green U0 = 0.02 (3 phases ~ U(0, 2 pi), seed = n),
-    tau = 0.501."""
+    tau = 0.501.  With `edge` only the sub-cube [0, edge)^3 of the n^3 field is built (a bounded sample of
+    the same workload for the CPU baseline; it is then treated as a periodic edge^3 box)."""
     rng = np.random.Generator(np.random.PCG64(n))
     ph = rng.uniform(0.0, 2.0 * np.pi, size=3)
     # built in the run dtype plane by plane to keep the host footprint at one copy for 512^3 / 768^3
     npdt = _NP_DTYPE[dtype]
-    M = np.zeros((10, n, n, n), dtype=npdt)
+    e = n if edge is None else min(edge, n)
+    M = np.zeros((10, e, e, e), dtype=npdt)
     M[0] = 1.0
-    X = _phase(n)[None, :] + ph[0]
-    Y = _phase(n)[:, None] + ph[1]
-    Z = _phase(n) + ph[2]
+    X = _phase(n)[None, :e] + ph[0]
+    Y = _phase(n)[:e, None] + ph[1]
+    Z = _phase(n)[:e] + ph[2]
     a = 0.02 * np.sin(X) * np.cos(Y)
     b = -0.02 * np.cos(X) * np.sin(Y)
     cz = np.cos(Z)
-    for k in range(n):
+    for k in range(e):
         M[1, k] = (a * cz[k]).astype(npdt)
         M[2, k] = (b * cz[k]).astype(npdt)
-    return Workload("cfg4_tp%d_%s" % (n, dtype), n, n, n, dtype, 0.501, steps, M)
+    name = "cfg4_tp%d_%s" % (n, dtype) + ("" if e == n else "_sub%d" % e)
+    return Workload(name, e, e, e, dtype, 0.501, steps, M)
 
 
 def random_state(nx: int, ny: int, nz: int, seed: int = 7, dtype: str = "f64", tau: float = 0.7,

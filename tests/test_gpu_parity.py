@@ -1,0 +1,231 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on identical
+seeded inputs.  All tests need a B200: run with  pytest -m gpu  on the GPU box."""
+import numpy as np
+import pytest
+
+from paper_2401_17074_b200 import workloads as W
+from tests.parity_util import (TOL, assert_parity, errors, gpu_state, make_gpu, make_oracle, run_both, subbox)
+
+pytestmark = pytest.mark.gpu
+
+GATHER, MARCH = 1, 2
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2401_17074_b200 import binding, build
+    build.build_lib()
+    binding.load_library()
+    return binding
+
+
+def kernels_for(B, w):
+    """Every sweep kernel that covers this workload (the gather kernel covers everything)."""
+    sim = B.from_workload(w, B.KERNEL_AUTO)
+    ks = [GATHER] + ([MARCH] if sim.active_kernel() == MARCH else [])
+    sim.close()
+    return ks
+
+
+def with_faces(w, faces, g=(0.0, 0.0, 0.0), inlet_face=None, seed=5):
+    w.faces = dict(faces)
+    w.g = g
+    if inlet_face is not None:
+        n = {0: (w.nz, w.ny), 1: (w.nz, w.nx), 2: (w.ny, w.nx)}[inlet_face // 2]
+        up = np.random.default_rng(seed).uniform(-0.03, 0.03, (3,) + n).astype(w.np_dtype)
+        w.inlet = W.Inlet(inlet_face, up, 0.05, 9, 0b111)
+    return w
+
+
+# ---------------------------------------------------------------------------------------------
+# small cases: several tiles + ragged tails, every boundary kind, both dtypes, every kernel
+# ---------------------------------------------------------------------------------------------
+SHAPES = [(3, 3, 3), (4, 3, 5), (5, 7, 9), (33, 17, 6), (64, 12, 10), (130, 9, 7), (136, 36, 5), (260, 20, 4)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_periodic_random_state(B, oracle_mod, shape, dtype):
+    w = W.random_state(*shape, seed=31, dtype=dtype, tau=0.62)
+    w.g = (1e-4, -2e-4, 3e-4)
+    for k in kernels_for(B, w):
+        G, R, _ = run_both(oracle_mod, w, 3, k)
+        assert_parity(w, G, R, "kernel %d" % k)
+
+
+BC_SETS = {
+    "walls_y+force": dict(faces={W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, g=(2e-4, 0, 1e-4)),
+    "walls_z": dict(faces={W.FACE_ZLO: W.BC_BOUNCE_BACK, W.FACE_ZHI: W.BC_BOUNCE_BACK}),
+    "walls_x": dict(faces={W.FACE_XLO: W.BC_BOUNCE_BACK, W.FACE_XHI: W.BC_BOUNCE_BACK}, g=(0, 1e-4, 0)),
+    "walls_xyz": dict(faces={f: W.BC_BOUNCE_BACK for f in range(6)}, g=(1e-4, 1e-4, -1e-4)),
+    "jet_like": dict(faces={W.FACE_ZLO: W.BC_VELOCITY_INLET, **{f: W.BC_OUTLET_ZERO_GRADIENT for f in (0, 1, 2, 3, 5)}},
+                     inlet_face=W.FACE_ZLO),
+    "inlet_x_walls_y": dict(faces={W.FACE_XLO: W.BC_VELOCITY_INLET, W.FACE_XHI: W.BC_OUTLET_ZERO_GRADIENT,
+                                   W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, inlet_face=W.FACE_XLO,
+                            g=(1e-4, 0, 0)),
+    "outlet_y_walls_z": dict(faces={W.FACE_YLO: W.BC_OUTLET_ZERO_GRADIENT, W.FACE_YHI: W.BC_VELOCITY_INLET,
+                                    W.FACE_ZLO: W.BC_BOUNCE_BACK, W.FACE_ZHI: W.BC_BOUNCE_BACK}, inlet_face=W.FACE_YHI),
+    "mixed_wall_outlet_same_axis": dict(faces={W.FACE_ZLO: W.BC_BOUNCE_BACK, W.FACE_ZHI: W.BC_OUTLET_ZERO_GRADIENT}),
+}
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("bc", sorted(BC_SETS))
+@pytest.mark.parametrize("shape", [(4, 3, 5), (12, 10, 7), (136, 11, 6)])
+def test_boundary_sets(B, oracle_mod, shape, bc, dtype):
+    w = with_faces(W.random_state(*shape, seed=17, dtype=dtype, tau=0.58), **BC_SETS[bc])
+    for k in kernels_for(B, w):
+        G, R, _ = run_both(oracle_mod, w, 4, k)
+        assert_parity(w, G, R, "%s kernel %d" % (bc, k))
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs
+# ---------------------------------------------------------------------------------------------
+def test_config0_full(B, oracle_mod):
+    """configs[0]: 32^3 fp64 Taylor-Green, tau = 0.8, 100 steps, max |d| <= 1e-12."""
+    w = W.config0()
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 10])
+        e = assert_parity(w, G, R, "kernel %d" % k)
+        print("config0 kernel %d: err(rho,u,Pi) = %s, curve %s" % (k, e, curve))
+        assert abs(G[0].sum() - 32**3) < 1e-9                       # mass conserved
+
+
+def test_config1_reduced_full_steps(B, oracle_mod):
+    """configs[1] at 32^3: fp32, near-inviscid TG + noise, the full 1000 steps; parity curve logged."""
+    w = W.config1(n=32, steps=1000)
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 10, 100])
+        print("config1@32 kernel %d curve (rho,u,Pi): %s" % (k, curve))
+        assert_parity(w, G, R, "kernel %d" % k)
+        assert np.abs(G[1:4]).max() < 0.1 and 0.9 < G[0].min() and G[0].max() < 1.1   # boundedness
+        assert abs(G[0].astype(np.float64).sum() / 32**3 - 1) < 1e-6                   # mass
+
+
+def test_config1_full_size_100_steps(B, oracle_mod):
+    """configs[1] at its full 128^3: 100 steps element by element (the oracle needs ~minutes for 1000)."""
+    w = W.config1()
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, 100, k, checkpoints=[1, 10])
+        print("config1@128 kernel %d curve: %s" % (k, curve))
+        assert_parity(w, G, R, "kernel %d" % k)
+
+
+def test_config2_channel_reduced_full_steps(B, oracle_mod):
+    """configs[2] shape at 48x32x24 (h = 16): walls + body force, the full 2000 steps."""
+    w = W.channel(48, 32, 24, steps=2000)
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 10, 100, 1000])
+        print("channel@48x32x24 kernel %d curve: %s" % (k, curve))
+        assert_parity(w, G, R, "kernel %d" % k)
+
+
+def test_config3_jet_reduced_full_steps(B, oracle_mod):
+    """configs[3] shape at 32x32x96, D = 6: inlet with noise + outlets, the full 1000 steps."""
+    w = W.jet(32, 32, 96, steps=1000, D=6.0)
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 10, 100])
+        print("jet@32x32x96 kernel %d curve: %s" % (k, curve))
+        assert_parity(w, G, R, "kernel %d" % k)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config4_64cube_200_steps(B, oracle_mod, dtype):
+    w = W.throughput(64, dtype, 200)
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, 200, k, checkpoints=[1, 10])
+        print("throughput64 %s kernel %d curve: %s" % (dtype, k, curve))
+        assert_parity(w, G, R, "kernel %d" % k)
+
+
+# ---------------------------------------------------------------------------------------------
+# full sizes, in the launch configuration bench.py times: sampled sub-boxes + invariants
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,dtype", [(512, "f32"), (256, "f64")])
+def test_full_size_sampled_subboxes(B, oracle_mod, n, dtype):
+    """Bench workload at full size: 3 GPU steps on the whole cube; the oracle recomputes sub-boxes cut from the
+    SAME seeded initial state (never from GPU output) and the uncontaminated cores are compared."""
+    import torch
+    w = W.throughput(n, dtype, 3)
+    sim = B.from_workload(w, B.KERNEL_AUTO)
+    sim.set_moments(torch.from_numpy(w.moments).to("cuda"))
+    sim.step(3)
+    G = gpu_state(sim)
+    k = 3
+    for lo in [(0, 0, 0), (n - 9, n - 9, n - 9), (n // 2 - 3, 0, n - 5), (124, 250, 3)]:
+        lo = [v - 4 for v in lo]                      # boxes straddle the periodic wrap and tile edges
+        hi = [v + 16 for v in lo]
+        s = subbox(w, lo, hi)
+        o = make_oracle(oracle_mod, s); o.step(k)
+        R = o.get_moments()
+        ix = [np.arange(lo[a] + k, hi[a] - k) % n for a in range(3)]
+        Gs = G[:, ix[2]][:, :, ix[1]][:, :, :, ix[0]]
+        Rs = R[:, k:-k, k:-k, k:-k]
+        s.nx = s.ny = s.nz = 16 - 2 * k
+        assert_parity(s, Gs, Rs, "sub-box at %s" % (lo,))
+    m = G[0].sum(dtype=np.float64)
+    assert abs(m / n**3 - 1) < 1e-7
+    sim.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# library behaviour on the device
+# ---------------------------------------------------------------------------------------------
+def test_checkpoint_resume_bitwise(B):
+    """get_moments + set_moments is the checkpoint: 2n steps == n, get, set, n (bitwise)."""
+    import torch
+    w = W.config1(n=32, steps=20)
+    for k in kernels_for(B, w):
+        a = make_gpu(w, k); a.step(20); Ga = a.get_moments().clone()
+        b = make_gpu(w, k); b.step(10); mid = b.get_moments().clone()
+        c = make_gpu(w, k); c.set_moments(mid); c.step(10); Gc = c.get_moments()
+        torch.cuda.synchronize()
+        assert torch.equal(Ga, Gc)
+        a2 = make_gpu(w, k); a2.step(20)
+        assert torch.equal(Ga, a2.get_moments())       # rerun is bitwise reproducible
+
+
+def test_diagnostics_match_oracle(B, oracle_mod):
+    import torch
+    for w in (W.channel(24, 16, 12, steps=30, dtype="f64"), W.jet(16, 16, 24, steps=30, dtype="f32", D=5.0)):
+        o = make_oracle(oracle_mod, w); sim = make_gpu(w, B.KERNEL_AUTO)
+        o.step(30); sim.step(30)
+        d = sim.diagnostics(); torch.cuda.synchronize()
+        d = d.cpu().numpy(); r = o.diagnostics()
+        tol = 1e-12 if w.dtype == "f64" else 1e-5
+        assert abs(d[0] / r[0] - 1) < tol
+        np.testing.assert_allclose(d[1:], r[1:], rtol=tol * 10, atol=tol * abs(r[0]) * 1e-2)
+        d2 = sim.diagnostics().cpu().numpy()
+        np.testing.assert_array_equal(d, d2)           # fixed-order reduction
+
+
+def test_host_buffer_round_trip(B, oracle_mod):
+    """tslb_set_moments_host / tslb_get_moments_host (the e2e path of bench.py)."""
+    w = W.random_state(20, 9, 7, seed=2, dtype="f32")
+    sim = B.from_workload(w)
+    sim.set_moments_host(np.ascontiguousarray(w.moments))
+    out = np.empty_like(w.moments)
+    sim.get_moments_host(out)
+    np.testing.assert_array_equal(out, w.moments)
+    sim.step(2)
+    sim.get_moments_host(out)
+    o = make_oracle(oracle_mod, w); o.step(2)
+    assert_parity(w, out.astype(np.float64), o.get_moments())
+
+
+def test_step_errors_on_device(B):
+    w = W.random_state(8, 8, 8, dtype="f64")
+    sim = B.from_workload(w)
+    with pytest.raises(B.TSLBError) as e:
+        sim.step(1)
+    assert e.value.code == B.TSLB_ESTATE
+    sim = make_gpu(w, B.KERNEL_AUTO)
+    with pytest.raises(B.TSLBError):
+        sim.step(-1)
+    sim.set_boundary(B.FACE_XLO, B.BC_BOUNCE_BACK)      # periodic on XHI only -> inconsistent
+    with pytest.raises(B.TSLBError) as e:
+        sim.step(1)
+    assert e.value.code == B.TSLB_EINVAL
