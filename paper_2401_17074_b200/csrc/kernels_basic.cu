@@ -127,7 +127,8 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
 #pragma unroll
             for (int cx = -1; cx <= 1; ++cx) {
                 const bool bounced = bx[cx + 1] | by[cy + 1] | bz[cz + 1];
-                const T w = (T)((cx ? 1.0 / 6 : 2.0 / 3) * (cy ? 1.0 / 6 : 2.0 / 3) * (cz ? 1.0 / 6 : 2.0 / 3));
+                // 216 w_i = 64, 16, 4, 1: exact powers of two, so no rounded weight multiplies the data
+                const T w = (T)((cx ? 1 : 4) * (cy ? 1 : 4) * (cz ? 1 : 4));
                 T f;
                 if (cx == 0 && cy == 0 && cz == 0) {
                     f = fstar_shifted(own, 0, 0, 0, (T)1, w, p.beta, p.g);
@@ -148,19 +149,24 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                 if (cx && cz) Sxz += (T)(cx * cz) * f;
                 if (cy && cz) Syz += (T)(cy * cz) * f;
             }
-    // rho' = 1 + dR; u' = J / rho'; Pi' = S - rho'(I/3 + u'u') with S_aa = dS_aa + 1/3   (Eq. 12)
-    const T rho = (T)1 + dR;
-    const T inv = (T)1 / rho;
+    // All sums are 216-scaled.  rho' = 1 + dR; u' = J / rho'; Pi' = S - rho'(I/3 + u'u') with S_aa = dS_aa + 1/3
+    // (Eq. 12).  x/216 is formed as x*hi + x*lo (unbiased); a rounded 1/216 or rounded w_i would be a systematic
+    // per-step gain that compounds over thousands of steps.
+    const T hi = (T)(1.0 / 216.0);
+    const T lo = (T)(1.0 / 216.0 - (double)hi);
+    const T dr = fma(dR, lo, dR * hi);
+    const T rho = (T)1 + dr;
+    const T inv = (T)1 / ((T)216 + dR);
     const T ux = Jx * inv, uy = Jy * inv, uz = Jz * inv;
-    const T third = (T)(1.0 / 3.0);
-    B[ip] = dR;
+    const T iso = (T)(1.0 / 3.0) * dr;
+    B[ip] = dr;
     B[N + ip] = ux; B[2 * N + ip] = uy; B[3 * N + ip] = uz;
-    B[4 * N + ip] = Sxx - third * dR - rho * ux * ux;
-    B[5 * N + ip] = Syy - third * dR - rho * uy * uy;
-    B[6 * N + ip] = Szz - third * dR - rho * uz * uz;
-    B[7 * N + ip] = Sxy - rho * ux * uy;
-    B[8 * N + ip] = Sxz - rho * ux * uz;
-    B[9 * N + ip] = Syz - rho * uy * uz;
+    B[4 * N + ip] = fma(Sxx, lo, Sxx * hi) - iso - rho * ux * ux;
+    B[5 * N + ip] = fma(Syy, lo, Syy * hi) - iso - rho * uy * uy;
+    B[6 * N + ip] = fma(Szz, lo, Szz * hi) - iso - rho * uz * uz;
+    B[7 * N + ip] = fma(Sxy, lo, Sxy * hi) - rho * ux * uy;
+    B[8 * N + ip] = fma(Sxz, lo, Sxz * hi) - rho * ux * uz;
+    B[9 * N + ip] = fma(Syz, lo, Syz * hi) - rho * uy * uz;
 }
 
 // ---------------------------------------------------------------------------------------------
