@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- GLUPS of the fused TSLB sweep (BASELINE.json metric) on N B200s of one node.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 512] [--dtype f32] [--kernel auto|gather|march]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 512] [--dtype f32] [--kernel auto|gather|tile]
     python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
 
 A "step" is one lattice time step = one pass of the whole hot path (boundary
@@ -39,7 +39,7 @@ def parse_args(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=512, help="cube edge of the configs[4] workload")
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "march"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "tile"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
@@ -219,7 +219,7 @@ def run_ours(args):
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     BLD.build_lib()
-    kernel = {"auto": B.KERNEL_AUTO, "gather": B.KERNEL_GATHER, "march": B.KERNEL_MARCH}[args.kernel]
+    kernel = {"auto": B.KERNEL_AUTO, "gather": B.KERNEL_GATHER, "tile": B.KERNEL_TILE}[args.kernel]
 
     w = W.throughput(args.n, args.dtype, args.steps)
     sim = B.from_workload(w, kernel)

@@ -53,9 +53,9 @@ enum {
     TSLB_BC_OUTLET_ZERO_GRADIENT = 3, /* nodes ON the face: all 10 moments copied from x_F              */
     TSLB_BC_BODY_FORCE = 4            /* not a face kind: sets the body acceleration g (face ignored)   */
 };
-/* Which sweep kernel tslb_step uses. AUTO picks the register-marching kernel when the lattice and the
- * boundary set allow it and the per-direction gather kernel otherwise. */
-enum { TSLB_KERNEL_AUTO = 0, TSLB_KERNEL_GATHER = 1, TSLB_KERNEL_MARCH = 2 };
+/* Which sweep kernel tslb_step uses. AUTO picks the TMA-staged register-marching tile kernel when the
+ * boundary set allows it and the per-direction gather kernel otherwise. */
+enum { TSLB_KERNEL_AUTO = 0, TSLB_KERNEL_GATHER = 1, TSLB_KERNEL_TILE = 2 };
 
 /* Parameters of TSLB_BC_VELOCITY_INLET (PAPER.md:181 Eq. 22, :270; readings A13, A14).
  * dev_u_plane: imposed velocity on the face, [3][n_b][n_a] of the context dtype, a = lower in-plane
@@ -80,12 +80,12 @@ int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out);
 /* Free the context (host memory only; the workspace and inlet planes stay the caller's). NULL is a no-op. */
 void tslb_destroy(tslb_ctx *ctx);
 
-/* Bytes of device memory the context needs: two moment buffers of 10*nx*ny*nz elements plus scratch for
- * the diagnostics reduction and the host-copy staging area.  0 if ctx == NULL. */
+/* Bytes of device memory the context needs: two moment buffers in the internal layout (10 fields, each padded
+ * by one ghost layer per side and to 16-byte rows) plus scratch for the diagnostics reduction.  0 if ctx == NULL. */
 size_t tslb_workspace_bytes(const tslb_ctx *ctx);
 
 /* Give the context its device memory (256-byte aligned, >= tslb_workspace_bytes, caller-owned).  First
- * call that touches CUDA: queries the current device.  Rebinding discards the state (set_moments again).
+ * call that touches CUDA: queries the current device, zeroes the workspace, builds the TMA descriptors.  Rebinding discards the state (set_moments again).
  * TSLB_EINVAL: NULL / misaligned / too small.  TSLB_ECUDA: no usable device. */
 int tslb_bind_workspace(tslb_ctx *ctx, void *dev_ptr, size_t bytes);
 
@@ -105,14 +105,14 @@ int tslb_set_moments_host(tslb_ctx *ctx, const void *host_src, void *stream);
  * set (PERIODIC must be on both faces of an axis) is checked by tslb_step. */
 int tslb_set_boundary(tslb_ctx *ctx, int face, int kind, const void *params);
 
-/* Choose the sweep kernel (TSLB_KERNEL_*).  TSLB_EINVAL if MARCH is forced on a configuration it does not
+/* Choose the sweep kernel (TSLB_KERNEL_*).  TSLB_EINVAL if TILE is forced on a configuration it does not
  * cover (reported by tslb_step). */
 int tslb_set_kernel(tslb_ctx *ctx, int kernel);
-/* The kernel the next tslb_step would launch (TSLB_KERNEL_GATHER or TSLB_KERNEL_MARCH), or -1. */
+/* The kernel the next tslb_step would launch (TSLB_KERNEL_GATHER or TSLB_KERNEL_TILE), or -1. */
 int tslb_active_kernel(const tslb_ctx *ctx);
 
-/* Advance n time steps (n >= 0): n x { boundary-node fill at time t ; fused stream-collide sweep A -> B ;
- * swap }.  Asynchronous on `stream`; no host<->device traffic.  TSLB_ESTATE before bind/set_moments,
+/* Advance n time steps (n >= 0): n x { boundary-node fill + ghost-layer refresh at time t ; fused stream-collide
+ * sweep A -> B ; swap }.  Asynchronous on `stream`; no host<->device traffic.  TSLB_ESTATE before bind/set_moments,
  * TSLB_EINVAL for n < 0 or an inconsistent boundary set, TSLB_ECUDA on a launch error. */
 int tslb_step(tslb_ctx *ctx, int n, void *stream);
 

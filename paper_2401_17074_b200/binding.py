@@ -17,8 +17,8 @@ TSLB_F32, TSLB_F64 = 0, 1
 TSLB_OK, TSLB_EINVAL, TSLB_ENOMEM, TSLB_ECUDA, TSLB_ESTATE = range(5)
 FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
 BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE = range(5)
-KERNEL_AUTO, KERNEL_GATHER, KERNEL_MARCH = range(3)
-KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_MARCH: "march"}
+KERNEL_AUTO, KERNEL_GATHER, KERNEL_TILE = range(3)
+KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile"}
 
 # every symbol include/tslb.h declares (tests check that the library exports all of them)
 SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",

@@ -1,5 +1,5 @@
 // kernels_basic.cu -- the per-direction "gather" sweep (covers every boundary set and lattice shape),
-// the boundary-node fill, layout import/export and the diagnostics reduction.  sm_100a.
+// the boundary-node fill, the ghost-layer (halo) refresh, layout import/export and the diagnostics reduction.  sm_100a.
 //
 // Arithmetic follows PAPER.md:154 (Eq. 18) with the readings of DESIGN.md; contractions are reduced by
 // hand.  Internal storage is the SHIFTED form: field 0 holds drho = rho - 1
@@ -16,7 +16,7 @@ struct Site {
 };
 
 template <typename T>
-__device__ __forceinline__ Site<T> load_site(const T *__restrict__ A, size_t N, size_t i)
+__device__ __forceinline__ Site<T> load_site(const T *__restrict__ A, long long N, long long i)
 {
     Site<T> s;
     s.dr = __ldg(A + i);
@@ -32,18 +32,21 @@ __device__ __forceinline__ Site<T> load_site(const T *__restrict__ A, size_t N, 
     return s;
 }
 
-// f*_c(M) - w_c for direction (sgn*cx, sgn*cy, sgn*cz); cx,cy,cz are compile-time after unrolling.
+// f*_c(M) - w_c - (base of the linear momentum term) for direction (sgn*cx, sgn*cy, sgn*cz); cx,cy,cz are
+// compile-time after unrolling.
 //   f* = w [ rho (1 + 3 c.(u+g) + 4.5((c.u)^2 - |u|^2/3) + 4.5((c.u)^3 - (c.u)|u|^2))          Eq. 14
 //          + beta (4.5 (cPc - trP/3) + 4.5 (3 cPc c.u - trP c.u - 2 cPu)) ]                      Eq. 17
 // Terms odd in c change sign with sgn (bounce-back evaluates the opposite direction at the own node).
+// INCREMENT FORM: the linear term 3 w c.(rho (u+g)) of the source node is written as
+// 3 w c.u(x) + 3 w lin, with u(x) the velocity of the TARGET node; sum_i c_i (3 w_i c_i.u(x)) = 216 u(x) exactly, so
+// the base never passes through rounded arithmetic and only `lin` (a difference of neighbouring velocities plus
+// small terms) does.  The caller passes lin = c.(u_src - u_x) + c.(g + drho_src (u_src + g)).
 template <typename T>
-__device__ __forceinline__ T fstar_shifted(const Site<T> &m, int cx, int cy, int cz, T sgn, T w, T beta,
-                                           const T *g)
+__device__ __forceinline__ T fstar_incr(const Site<T> &m, int cx, int cy, int cz, T sgn, T w, T beta, T lin)
 {
     const T fx = (T)cx, fy = (T)cy, fz = (T)cz;
     const T rho = (T)1 + m.dr;
     const T cu = fx * m.ux + fy * m.uy + fz * m.uz;
-    const T cg = fx * g[0] + fy * g[1] + fz * g[2];
     const T uu = m.ux * m.ux + m.uy * m.uy + m.uz * m.uz;
     const T trP = m.pxx + m.pyy + m.pzz;
     const T cPx = fx * m.pxx + fy * m.pxy + fz * m.pxz;  // (c.P)_x
@@ -52,10 +55,10 @@ __device__ __forceinline__ T fstar_shifted(const Site<T> &m, int cx, int cy, int
     const T cPc = cPx * fx + cPy * fy + cPz * fz;
     const T cPu = cPx * m.ux + cPy * m.uy + cPz * m.uz;
     const T even_eq = (T)4.5 * cu * cu - (T)1.5 * uu;
-    const T odd_eq = (T)3 * (cu + cg) + (T)4.5 * cu * (cu * cu - uu);
+    const T odd_eq = (T)4.5 * cu * (cu * cu - uu);
     const T even_ne = (T)4.5 * cPc - (T)1.5 * trP;
     const T odd_ne = (T)4.5 * ((T)3 * cPc * cu - trP * cu - (T)2 * cPu);
-    return w * (m.dr + rho * (even_eq + sgn * odd_eq) + beta * (even_ne + sgn * odd_ne));
+    return w * (m.dr + (T)3 * lin + rho * (even_eq + sgn * odd_eq) + beta * (even_ne + sgn * odd_ne));
 }
 
 __device__ __forceinline__ bool is_open_kind(int k)
@@ -66,14 +69,15 @@ __device__ __forceinline__ bool is_open_kind(int k)
 template <typename P>
 __device__ __forceinline__ bool on_open_face(const P &p, int x, int y, int z)
 {
-    return (x == 0 && is_open_kind(p.kind[0])) || (x == p.nx - 1 && is_open_kind(p.kind[1])) ||
-           (y == 0 && is_open_kind(p.kind[2])) || (y == p.ny - 1 && is_open_kind(p.kind[3])) ||
-           (z == 0 && is_open_kind(p.kind[4])) || (z == p.nz - 1 && is_open_kind(p.kind[5]));
+    return (x == 0 && is_open_kind(p.kind[0])) || (x == p.L.nx - 1 && is_open_kind(p.kind[1])) ||
+           (y == 0 && is_open_kind(p.kind[2])) || (y == p.L.ny - 1 && is_open_kind(p.kind[3])) ||
+           (z == 0 && is_open_kind(p.kind[4])) || (z == p.L.nz - 1 && is_open_kind(p.kind[5]));
 }
 
 // ---------------------------------------------------------------------------------------------
 // Gather sweep: one thread per node, 27 upstream nodes read straight from global memory (L1/L2
-// provide the reuse).  SURVEY.md 8(a) rows a1-a8 in one kernel.
+// provide the reuse).  SURVEY.md 8(a) rows a1-a8 in one kernel.  Does its own periodic wrap (never
+// reads the ghost layers), so it needs no halo refresh.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__ A, T *__restrict__ B,
@@ -82,9 +86,9 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
-    if (x >= p.nx || y >= p.ny) return;
-    const size_t N = (size_t)p.nx * p.ny * p.nz;
-    const size_t ip = ((size_t)z * p.ny + y) * p.nx + x;
+    if (x >= p.L.nx || y >= p.L.ny) return;
+    const long long N = p.L.field;
+    const long long ip = lay_idx(p.L, x, y, z);
     const Site<T> own = load_site(A, N, ip);
 
     if (on_open_face(p, x, y, z)) {  // boundary nodes are not advanced: M_{t+1}(x_B) := M_t(x_B)
@@ -99,7 +103,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
     int sx[3], sy[3], sz[3];
     bool bx[3], by[3], bz[3];
     {
-        const int n[3] = {p.nx, p.ny, p.nz};
+        const int n[3] = {p.L.nx, p.L.ny, p.L.nz};
         const int q[3] = {x, y, z};
         int *s[3] = {sx, sy, sz};
         bool *b[3] = {bx, by, bz};
@@ -131,12 +135,21 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                 const T w = (T)((cx ? 1 : 4) * (cy ? 1 : 4) * (cz ? 1 : 4));
                 T f;
                 if (cx == 0 && cy == 0 && cz == 0) {
-                    f = fstar_shifted(own, 0, 0, 0, (T)1, w, p.beta, p.g);
+                    f = fstar_incr(own, 0, 0, 0, (T)1, w, p.beta, (T)0);
                 } else {
                     // halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) from the node's own moments
-                    const size_t is = bounced ? ip : ((size_t)sz[cz + 1] * p.ny + sy[cy + 1]) * p.nx + sx[cx + 1];
+                    const long long is = bounced ? ip : lay_idx(p.L, sx[cx + 1], sy[cy + 1], sz[cz + 1]);
                     const Site<T> m = load_site(A, N, is);
-                    f = fstar_shifted(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, p.g);
+                    // small part of rho (u + g): g + drho (u + g), per component
+                    const T smx = fma(m.dr, m.ux + p.g[0], p.g[0]);
+                    const T smy = fma(m.dr, m.uy + p.g[1], p.g[1]);
+                    const T smz = fma(m.dr, m.uz + p.g[2], p.g[2]);
+                    T lin;
+                    if (bounced)   // reversed direction at the own node: -c.psi(x) = c.u(x) + [-(2 c.u(x) + c.small(x))]
+                        lin = -((T)cx * ((T)2 * own.ux + smx) + (T)cy * ((T)2 * own.uy + smy) + (T)cz * ((T)2 * own.uz + smz));
+                    else
+                        lin = (T)cx * ((m.ux - own.ux) + smx) + (T)cy * ((m.uy - own.uy) + smy) + (T)cz * ((m.uz - own.uz) + smz);
+                    f = fstar_incr(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, lin);
                 }
                 dR += f;                                  // arrival direction c_i in every sum
                 if (cx) Jx += (T)cx * f;
@@ -149,15 +162,18 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                 if (cx && cz) Sxz += (T)(cx * cz) * f;
                 if (cy && cz) Syz += (T)(cy * cz) * f;
             }
-    // All sums are 216-scaled.  rho' = 1 + dR; u' = J / rho'; Pi' = S - rho'(I/3 + u'u') with S_aa = dS_aa + 1/3
-    // (Eq. 12).  x/216 is formed as x*hi + x*lo (unbiased); a rounded 1/216 or rounded w_i would be a systematic
-    // per-step gain that compounds over thousands of steps.
+    // All sums are 216-scaled and J lacks its base 216 u(x).  rho' = 1 + dR/216; u' = (216 u + J) / (216 rho')
+    // = u + (J - u dR) / (216 + dR); Pi' = S - rho'(I/3 + u'u') with S_aa = dS_aa + 1/3 (Eq. 12).  x/216 is formed as
+    // x*hi + x*lo (unbiased); a rounded 1/216 or rounded w_i would be a systematic per-step gain that compounds over
+    // thousands of steps.
     const T hi = (T)(1.0 / 216.0);
     const T lo = (T)(1.0 / 216.0 - (double)hi);
     const T dr = fma(dR, lo, dR * hi);
     const T rho = (T)1 + dr;
     const T inv = (T)1 / ((T)216 + dR);
-    const T ux = Jx * inv, uy = Jy * inv, uz = Jz * inv;
+    const T ux = fma(fma(-own.ux, dR, Jx), inv, own.ux);
+    const T uy = fma(fma(-own.uy, dR, Jy), inv, own.uy);
+    const T uz = fma(fma(-own.uz, dR, Jz), inv, own.uz);
     const T iso = (T)(1.0 / 3.0) * dr;
     B[ip] = dr;
     B[N + ip] = ux; B[2 * N + ip] = uy; B[3 * N + ip] = uz;
@@ -184,12 +200,12 @@ __device__ __forceinline__ uint64_t mix64(uint64_t z)  // SplitMix64 finaliser (
 }
 
 template <typename T>
-__global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p, int plane_max)
+__global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
 {
     const int f = blockIdx.y;
     if (!is_open_kind(p.kind[f])) return;
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    const int n[3] = {p.nx, p.ny, p.nz};
+    const int n[3] = {p.L.nx, p.L.ny, p.L.nz};
     const int ax = f >> 1;
     const int a = (ax == 0) ? 1 : 0;
     const int b = (ax == 2) ? 1 : 2;
@@ -209,9 +225,9 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p, int plane_
         if (r[d] == 0 && is_open_kind(p.kind[2 * d])) r[d] = 1;
         if (r[d] == n[d] - 1 && is_open_kind(p.kind[2 * d + 1])) r[d] = n[d] - 2;
     }
-    const size_t N = (size_t)p.nx * p.ny * p.nz;
-    const size_t ib = ((size_t)q[2] * p.ny + q[1]) * p.nx + q[0];
-    const size_t iF = ((size_t)r[2] * p.ny + r[1]) * p.nx + r[0];
+    const long long N = p.L.field;
+    const long long ib = lay_idx(p.L, q[0], q[1], q[2]);
+    const long long iF = lay_idx(p.L, r[0], r[1], r[2]);
 #pragma unroll
     for (int k = 0; k < TSLB_NF; ++k) M[k * N + ib] = M[k * N + iF];
     for (int f2 = 0; f2 < 6; ++f2) {
@@ -221,8 +237,9 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p, int plane_
         const int a2 = (ax2 == 0) ? 1 : 0, b2 = (ax2 == 2) ? 1 : 2;
         const size_t pl = (size_t)n[a2] * n[b2];
         const size_t jj = (size_t)q[b2] * n[a2] + q[a2];
+        const uint64_t lin = ((uint64_t)q[2] * p.L.ny + q[1]) * p.L.nx + q[0];   // API linear index of the node
         uint64_t k64 = mix64(p.inlet[f2].seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(p.t + 1)));
-        k64 = mix64(k64 + (uint64_t)ib);
+        k64 = mix64(k64 + lin);
         const double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
         const T *up = (const T *)p.inlet[f2].u_plane;
 #pragma unroll
@@ -236,16 +253,68 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p, int plane_
 }
 
 // ---------------------------------------------------------------------------------------------
-// API layout <-> internal layout (field 0: rho <-> rho - 1; exact for 0.5 <= rho <= 2)
+// Ghost-layer refresh: every ghost cell (a coordinate equal to -1 or n) takes the
+// 10 moments of the interior node obtained by wrapping its coordinates on periodic axes and clamping
+// them on the others.  The TMA-staged sweep reads neighbours through these layers, so it carries no
+// wrap logic; ghost cells behind a wall or an open face are never used by a node that is advanced
+// (they only keep the staged tiles finite).  Launched after the boundary-node fill.
+// One thread per ghost cell of one of the three slab pairs: x slabs (full y,z extent incl. ghosts),
+// y slabs (x interior only), z slabs (x,y interior only) -- together every ghost cell exactly once.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void halo_kernel(T *__restrict__ M, FillParams p)
+{
+    const Layout &L = p.L;
+    const long long nXs = 2LL * (L.ny + 2) * (L.nz + 2);   // x = -1 / nx, all y,z incl. ghosts
+    const long long nYs = 2LL * L.nx * (L.nz + 2);          // y = -1 / ny, x interior, all z incl. ghosts
+    const long long nZs = 2LL * L.nx * L.ny;                // z = -1 / nz, x,y interior
+    const long long tot = nXs + nYs + nZs;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += stride) {
+        int x, y, z;
+        if (i < nZs) {                       // z slabs first: rows are contiguous in x
+            const long long j = i >> 1;
+            z = (i & 1) ? L.nz : -1;
+            x = (int)(j % L.nx); y = (int)(j / L.nx);
+        } else if (i < nZs + nYs) {
+            const long long j = (i - nZs) >> 1;
+            y = ((i - nZs) & 1) ? L.ny : -1;
+            x = (int)(j % L.nx); z = (int)(j / L.nx) - 1;
+        } else {
+            const long long j = (i - nZs - nYs) >> 1;
+            x = ((i - nZs - nYs) & 1) ? L.nx : -1;
+            y = (int)(j % (L.ny + 2)) - 1; z = (int)(j / (L.ny + 2)) - 1;
+        }
+        const int n[3] = {L.nx, L.ny, L.nz};
+        int q[3] = {x, y, z};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (q[a] < 0) q[a] = (p.kind[2 * a] == TSLB_BC_PERIODIC) ? n[a] - 1 : 0;
+            else if (q[a] >= n[a]) q[a] = (p.kind[2 * a + 1] == TSLB_BC_PERIODIC) ? 0 : n[a] - 1;
+        }
+        const long long ig = lay_idx(L, x, y, z), is = lay_idx(L, q[0], q[1], q[2]);
+#pragma unroll
+        for (int k = 0; k < TSLB_NF; ++k) M[k * L.field + ig] = M[k * L.field + is];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// API layout [10][nz][ny][nx] <-> internal padded layout (field 0: rho <-> rho - 1; exact for 0.5 <= rho <= 2)
 // ---------------------------------------------------------------------------------------------
 template <typename T, int DIR>
-__global__ void convert_kernel(const T *__restrict__ src, T *__restrict__ dst, size_t N)
+__global__ void convert_kernel(const T *__restrict__ src, T *__restrict__ dst, Layout L)
 {
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < TSLB_NF * N; i += stride) {
-        T v = src[i];
-        if (i < N) v = DIR > 0 ? v - (T)1 : v + (T)1;
-        dst[i] = v;
+    const long long N = (long long)L.nx * L.ny * L.nz;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < TSLB_NF * N; i += stride) {
+        const int k = (int)(i / N);
+        const long long s = i - k * N;
+        const int x = (int)(s % L.nx);
+        const long long r = s / L.nx;
+        const int y = (int)(r % L.ny), z = (int)(r / L.ny);
+        const long long j = k * L.field + lay_idx(L, x, y, z);
+        if (DIR > 0) { T v = src[i]; if (k == 0) v -= (T)1; dst[j] = v; }
+        else { T v = src[j]; if (k == 0) v += (T)1; dst[i] = v; }
     }
 }
 
@@ -263,14 +332,16 @@ template <typename T>
 __global__ void __launch_bounds__(TSLB_DIAG_THREADS) diag_partial_kernel(const T *__restrict__ A, FillParams p,
                                                                           double *__restrict__ partial)
 {
-    const size_t N = (size_t)p.nx * p.ny * p.nz;
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const long long Ns = (long long)p.L.nx * p.L.ny * p.L.nz;
+    const long long N = p.L.field;
+    const long long stride = (long long)gridDim.x * blockDim.x;
     double acc[5] = {0, 0, 0, 0, 0};
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += stride) {
-        const int x = (int)(i % p.nx);
-        const size_t r = i / p.nx;
-        const int y = (int)(r % p.ny), z = (int)(r / p.ny);
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < Ns; s += stride) {
+        const int x = (int)(s % p.L.nx);
+        const long long r = s / p.L.nx;
+        const int y = (int)(r % p.L.ny), z = (int)(r / p.L.ny);
         if (on_open_face(p, x, y, z)) continue;
+        const long long i = lay_idx(p.L, x, y, z);
         const double rho = 1.0 + (double)A[i];
         const double ux = A[N + i], uy = A[2 * N + i], uz = A[3 * N + i];
         acc[0] += rho; acc[1] += rho * ux; acc[2] += rho * uy; acc[3] += rho * uz;
@@ -305,7 +376,7 @@ template <typename T>
 SweepParams<T> make_params(const tslb_ctx *c)
 {
     SweepParams<T> p;
-    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    p.L = c->L;
     for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
     p.beta = (T)(1.0 - c->omega);
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
@@ -315,7 +386,7 @@ SweepParams<T> make_params(const tslb_ctx *c)
 FillParams make_fill(const tslb_ctx *c)
 {
     FillParams p;
-    p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+    p.L = c->L;
     for (int f = 0; f < 6; ++f) { p.kind[f] = c->kind[f]; p.inlet[f] = c->inlet[f]; }
     p.t = c->t;
     return p;
@@ -337,17 +408,33 @@ cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st)
     return cudaGetLastError();
 }
 
+static bool any_open(const tslb_ctx *c)
+{
+    for (int f = 0; f < 6; ++f)
+        if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT) return true;
+    return false;
+}
+
 cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st)
 {
-    bool any = false;
-    for (int f = 0; f < 6; ++f) any |= (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT);
-    if (!any) return cudaSuccess;
+    if (!any_open(c)) return cudaSuccess;
     int pm = c->nx * c->ny;
     if (c->nx * c->nz > pm) pm = c->nx * c->nz;
     if (c->ny * c->nz > pm) pm = c->ny * c->nz;
     dim3 block(128), grid((pm + 127) / 128, 6);
-    if (c->dtype == TSLB_F32) fill_boundary_kernel<float><<<grid, block, 0, st>>>((float *)buf, make_fill(c), pm);
-    else fill_boundary_kernel<double><<<grid, block, 0, st>>>((double *)buf, make_fill(c), pm);
+    if (c->dtype == TSLB_F32) fill_boundary_kernel<float><<<grid, block, 0, st>>>((float *)buf, make_fill(c));
+    else fill_boundary_kernel<double><<<grid, block, 0, st>>>((double *)buf, make_fill(c));
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st)
+{
+    const long long tot = 2LL * (c->ny + 2) * (c->nz + 2) + 2LL * c->nx * (c->nz + 2) + 2LL * c->nx * c->ny;
+    long long blocks = (tot + 255) / 256;
+    if (blocks > (long long)c->sm_count * 16) blocks = (long long)c->sm_count * 16;
+    if (c->dtype == TSLB_F32) halo_kernel<float><<<(unsigned)blocks, 256, 0, st>>>((float *)buf, make_fill(c));
+    else halo_kernel<double><<<(unsigned)blocks, 256, 0, st>>>((double *)buf, make_fill(c));
     c->launches++;
     return cudaGetLastError();
 }
@@ -358,8 +445,8 @@ static cudaError_t launch_convert(tslb_ctx *c, const void *src, void *dst, cudaS
     const size_t N = tslb_sites(c);
     size_t blocks = (TSLB_NF * N + 255) / 256;
     if (blocks > (size_t)c->sm_count * 16) blocks = (size_t)c->sm_count * 16;
-    if (c->dtype == TSLB_F32) convert_kernel<float, DIR><<<(unsigned)blocks, 256, 0, st>>>((const float *)src, (float *)dst, N);
-    else convert_kernel<double, DIR><<<(unsigned)blocks, 256, 0, st>>>((const double *)src, (double *)dst, N);
+    if (c->dtype == TSLB_F32) convert_kernel<float, DIR><<<(unsigned)blocks, 256, 0, st>>>((const float *)src, (float *)dst, c->L);
+    else convert_kernel<double, DIR><<<(unsigned)blocks, 256, 0, st>>>((const double *)src, (double *)dst, c->L);
     c->launches++;
     return cudaGetLastError();
 }

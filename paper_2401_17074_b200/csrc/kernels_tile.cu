@@ -1,0 +1,590 @@
+// kernels_tile.cu -- the TMA-staged, register-marching SEPARABLE sweep (the fast path of tslb_step) for sm_100a.
+//
+// Same update as the gather kernel (Eq. 18 + Eq. 12), evaluated in the form derived in
+// the post-collision population of a source node is linear in 17 Hermite
+// coefficients A_k of that node (k = (kx,ky,kz), k_a <= 2, |k| <= 3; Eq. 13, 16, 17), and because D3Q27 and its
+// Hermite basis are tensor products the 27-direction pull + moment sums factor into three 1-D 3-tap passes
+//       M'_p(x) = sum_k  T^x_{px,kx} T^y_{py,ky} T^z_{pz,kz}  A_k ,      T_{p,q} phi (x) = sum_c w(c) c^p h_q(c) phi(x - c).
+// With every field scaled by 216 (and the q = 2 fields by a further 2/3) all taps are the small integers
+// 1, 4, -2, so no rounded lattice weight ever multiplies the data.
+//
+// Data path: a CTA owns a 30 x 8 column of nodes and marches along z.  One elected
+// thread streams the z-planes of the 10 moment fields, 32 x 10 nodes each (the tile plus a 1-node halo), from the
+// padded SoA buffer into a 4-deep shared-memory ring with TMA (cp.async.bulk.tensor.4d, mbarrier complete_tx);
+// ghost layers in the buffer stand for the periodic images, so the kernel has no wrap logic.  Every warp owns
+// 2 rows (packed in a 2-wide register pair so fp32 issues as FFMA2/FADD2) x 32 columns (30 outputs + 2 halo lanes):
+//   y pass: in registers, from the A_k of rows r0-1 .. r0+2 read from shared memory,
+//   x pass: neighbours' values by warp shuffles,
+//   z pass: by marching -- 3 running values per (px,py) group, no plane is staged twice.
+// Each node's moments leave HBM once per tile (halo re-reads hit L2) and the 10 new moments are written once:
+// 80 B (fp32) / 160 B (fp64) of compulsory traffic per node update.
+//
+// INCREMENT FORM: the base 3 u_a of the first-order coefficients never enters the
+// passes.  A pass with taps (t-, t0, t+) applied to B*u gives (t- + t0 + t+) B u(x) + B [t- (u(x-1) - u(x)) + t+ (u(x+1) - u(x))];
+// only the bracket (exact differences of stored velocities) is added at each stage, and the product of the tap sums,
+// 216 u_a(x), is re-attached in closed form at the end:  u' = u + (J_small - u dR) / (216 + dR).
+#include "tslb_internal.h"
+
+namespace {
+
+// ---- 2-wide packs --------------------------------------------------------------------------------------
+struct D2 { double x, y; };
+template <typename T> struct PackOf;
+template <> struct PackOf<float> { typedef float2 type; };
+template <> struct PackOf<double> { typedef D2 type; };
+
+__device__ __forceinline__ float2 pk(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ D2 pk(double a, double b) { D2 r; r.x = a; r.y = b; return r; }
+#ifndef TSLB_SCALAR_F32
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 psub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
+#else
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return make_float2(a.x * b.x, a.y * b.y); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
+__device__ __forceinline__ float2 psub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#endif
+__device__ __forceinline__ D2 padd(D2 a, D2 b) { return pk(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ D2 pmul(D2 a, D2 b) { return pk(a.x * b.x, a.y * b.y); }
+__device__ __forceinline__ D2 pfma(D2 a, D2 b, D2 c) { return pk(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
+__device__ __forceinline__ D2 psub(D2 a, D2 b) { return pk(a.x - b.x, a.y - b.y); }
+template <typename P, typename T> __device__ __forceinline__ P pbc(T s) { return pk(s, s); }
+// a*s + c and a*s with a scalar s
+template <typename P, typename T> __device__ __forceinline__ P pfmas(P a, T s, P c) { return pfma(a, pbc<P, T>(s), c); }
+template <typename P, typename T> __device__ __forceinline__ P pmuls(P a, T s) { return pmul(a, pbc<P, T>(s)); }
+
+template <typename P> __device__ __forceinline__ P shfl_up1(P v)
+{
+    return pk(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1));
+}
+template <typename P> __device__ __forceinline__ P shfl_dn1(P v)
+{
+    return pk(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1));
+}
+
+// ---- TMA / mbarrier (PTX; SASS: UTMALDG, SYNCS) ----------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
+template <typename T>
+struct TileParams {
+    Layout L;
+    int kind[6];
+    T beta, g[3];
+    int zchunk;  // planes per z chunk
+};
+
+// valid Hermite index: each <= 2, sum <= 3 (H3_aaa == 0 on this lattice)
+__host__ __device__ constexpr bool kvalid(int kx, int ky, int kz) { return kx <= 2 && ky <= 2 && kz <= 2 && kx + ky + kz <= 3; }
+
+// ---- Hermite coefficients of one pack of two nodes, round kz (216-scaled, integer prefactors) -----------
+//   A000 = drho                       A100 = 3 [rho (ux+gx) - ux]  (increment form: base 3 ux handled apart)
+//   A200 = 3 (rho ux ux + beta Pxx)   A110 = 9 (rho ux uy + beta Pxy)   (Eq. 13 + Eq. 7/17, n = 2)
+//   A210 = 9 a3_xxy, A111 = 27 a3_xyz,  a3_abg = rho ua ub ug + beta (Pab ug + ua Pbg + ub Pag)   (Eq. 16-17)
+// raw[]: drho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz.  Out: A[kx][ky] for this kz.
+template <int KZ, typename P, typename T>
+__device__ __forceinline__ void hermite_round(const P (&raw)[TSLB_NF], T beta, const T (&g)[3], P (&A)[3][3])
+{
+    const P one = pbc<P, T>((T)1);
+    const P rho = padd(one, raw[0]);
+    const P r3 = pmuls(rho, (T)3);
+    const P d3 = pmuls(raw[0], (T)3);
+    const P ux = raw[1], uy = raw[2], uz = raw[3];
+    const T b3 = (T)3 * beta, b9 = (T)9 * beta;
+    if (KZ == 0) {
+        const P m3x = pmul(r3, ux), m3y = pmul(r3, uy);
+        const P q9xy = pmuls(raw[7], b9);
+        const P a20 = pfma(m3x, ux, pmuls(raw[4], b3));
+        const P a02 = pfma(m3y, uy, pmuls(raw[5], b3));
+        A[0][0] = raw[0];
+        A[1][0] = pfma(d3, padd(ux, pbc<P, T>(g[0])), pbc<P, T>((T)3 * g[0]));   // 3 [g + drho (u + g)]
+        A[0][1] = pfma(d3, padd(uy, pbc<P, T>(g[1])), pbc<P, T>((T)3 * g[1]));
+        A[2][0] = a20;
+        A[0][2] = a02;
+        A[1][1] = pfma(pmuls(m3x, (T)3), uy, q9xy);
+        A[2][1] = pfma(padd(ux, ux), q9xy, pmul(a20, pmuls(uy, (T)3)));
+        A[1][2] = pfma(padd(uy, uy), q9xy, pmul(a02, pmuls(ux, (T)3)));
+    } else if (KZ == 1) {
+        const P m3x = pmul(r3, ux), m3y = pmul(r3, uy);
+        const P m9x = pmuls(m3x, (T)3), m9y = pmuls(m3y, (T)3);
+        const P q9xy = pmuls(raw[7], b9), q9xz = pmuls(raw[8], b9), q9yz = pmuls(raw[9], b9);
+        const P a200 = pfma(m3x, ux, pmuls(raw[4], b3));
+        const P a020 = pfma(m3y, uy, pmuls(raw[5], b3));
+        const P a110 = pfma(m9x, uy, q9xy);
+        const P u3x = pmuls(ux, (T)3), u3y = pmuls(uy, (T)3), u3z = pmuls(uz, (T)3);
+        A[0][0] = pfma(d3, padd(uz, pbc<P, T>(g[2])), pbc<P, T>((T)3 * g[2]));
+        A[1][0] = pfma(m9x, uz, q9xz);
+        A[0][1] = pfma(m9y, uz, q9yz);
+        A[2][0] = pfma(padd(ux, ux), q9xz, pmul(a200, u3z));
+        A[0][2] = pfma(padd(uy, uy), q9yz, pmul(a020, u3z));
+        A[1][1] = pfma(u3x, q9yz, pfma(u3y, q9xz, pmul(u3z, a110)));
+    } else {
+        const P m3z = pmul(r3, uz);
+        const P q9xz = pmuls(raw[8], b9), q9yz = pmuls(raw[9], b9);
+        const P a002 = pfma(m3z, uz, pmuls(raw[6], b3));
+        const P uz2 = padd(uz, uz);
+        A[0][0] = a002;
+        A[1][0] = pfma(uz2, q9xz, pmul(a002, pmuls(ux, (T)3)));
+        A[0][1] = pfma(uz2, q9yz, pmul(a002, pmuls(uy, (T)3)));
+    }
+}
+
+// ---- one 1-D pass on a group of up to three fields q = 0,1,2 given S_q = phi(-1)+phi(+1), D_q = phi(-1)-phi(+1)
+//      and the centre values c0, c2:      out0 = E + 4 c0 - 2 c2,  out1 = D0 + S1 + D2,  out2 = E = S0 + D1 + S2
+template <int NQ, typename P, typename T>
+__device__ __forceinline__ void pass_group(const P (&S)[3], const P (&D)[3], P c0, P c2, P &o0, P &o1, P &o2)
+{
+    P E = S[0];
+    P O = D[0];
+    if (NQ >= 2) { E = padd(E, D[1]); O = padd(O, S[1]); }
+    if (NQ >= 3) { E = padd(E, S[2]); O = padd(O, D[2]); }
+    o2 = E;
+    o1 = O;
+    o0 = pfmas(c0, (T)4, E);
+    if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
+}
+
+// Contribution of the bounced directions at a node next to a halfway bounce-back wall on a y face
+// (DESIGN.md "Walls in the separable form"): f_i(x,t+1) = f*_ibar(x,t) for the 9 directions with c_y = sgn_in,
+// evaluated from the node's own 216-scaled Hermite coefficients (FULL first-order coefficients here: the increment
+// form treats the missing ghost row as u = 0, so the whole bounced population is a correction).  Adds to out[10]
+// (216-scaled raw moments in the order 000,100,010,001,200,020,002,110,101,011).  lo_wall: wall below (arrival
+// c_y = +1), else above.
+template <typename T>
+__device__ __noinline__ void bounce_y_correction(const T *__restrict__ Abuf, long long N, long long idx, T beta, const T (&g)[3],
+                                                 bool lo_wall, T (&out)[TSLB_NF])
+{
+    T raw[TSLB_NF];
+#pragma unroll
+    for (int f = 0; f < TSLB_NF; ++f) raw[f] = __ldg(Abuf + f * N + idx);
+    const T rho = (T)1 + raw[0], ux = raw[1], uy = raw[2], uz = raw[3];
+    const T u[3] = {ux, uy, uz};
+    const T Pm[3][3] = {{raw[4], raw[7], raw[8]}, {raw[7], raw[5], raw[9]}, {raw[8], raw[9], raw[6]}};
+    T a2[3][3];
+    for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) a2[a][b] = rho * u[a] * u[b] + beta * Pm[a][b];
+    // A(kx,ky,kz), scaled as in hermite_round
+    T A[3][3][3];
+    for (int i = 0; i < 27; ++i) (&A[0][0][0])[i] = (T)0;
+    A[0][0][0] = raw[0];
+    A[1][0][0] = (T)3 * rho * (ux + g[0]); A[0][1][0] = (T)3 * rho * (uy + g[1]); A[0][0][1] = (T)3 * rho * (uz + g[2]);
+    A[2][0][0] = (T)3 * a2[0][0]; A[0][2][0] = (T)3 * a2[1][1]; A[0][0][2] = (T)3 * a2[2][2];
+    A[1][1][0] = (T)9 * a2[0][1]; A[1][0][1] = (T)9 * a2[0][2]; A[0][1][1] = (T)9 * a2[1][2];
+    // a3_aab = a2_aa u_b + 2 u_a beta P_ab
+    A[2][1][0] = (T)9 * (a2[0][0] * uy + (T)2 * ux * beta * Pm[0][1]);
+    A[2][0][1] = (T)9 * (a2[0][0] * uz + (T)2 * ux * beta * Pm[0][2]);
+    A[1][2][0] = (T)9 * (a2[1][1] * ux + (T)2 * uy * beta * Pm[0][1]);
+    A[0][2][1] = (T)9 * (a2[1][1] * uz + (T)2 * uy * beta * Pm[1][2]);
+    A[1][0][2] = (T)9 * (a2[2][2] * ux + (T)2 * uz * beta * Pm[0][2]);
+    A[0][1][2] = (T)9 * (a2[2][2] * uy + (T)2 * uz * beta * Pm[1][2]);
+    A[1][1][1] = (T)27 * (a2[0][1] * uz + beta * (Pm[0][2] * uy + Pm[1][2] * ux));
+    // B(kx,kz) = sum_ky s^ky A(kx,ky,kz), s = t_ky(-c_y): wall below -> t(-1) = (1,-1,1); above -> t(+1) = (1,1,1)
+    const T s1 = lo_wall ? (T)-1 : (T)1;
+    T Bm[3][3];
+    for (int kx = 0; kx < 3; ++kx)
+        for (int kz = 0; kz < 3; ++kz) Bm[kx][kz] = A[kx][0][kz] + s1 * A[kx][1][kz] + A[kx][2][kz];
+    const T sg = lo_wall ? (T)1 : (T)-1;  // c_y^py of the arrival direction
+    // local sums L(p,q) = sum_c c^p t_q(-c): L(0,0)=6, L(1,1)=-2, L(2,0)=2, L(2,2)=2, others 0
+    out[0] += (T)36 * Bm[0][0];
+    out[1] += (T)-12 * Bm[1][0];
+    out[2] += sg * (T)36 * Bm[0][0];
+    out[3] += (T)-12 * Bm[0][1];
+    out[4] += (T)12 * (Bm[0][0] + Bm[2][0]);
+    out[5] += (T)36 * Bm[0][0];
+    out[6] += (T)12 * (Bm[0][0] + Bm[0][2]);
+    out[7] += sg * (T)-12 * Bm[1][0];
+    out[8] += (T)4 * Bm[1][1];
+    out[9] += sg * (T)-12 * Bm[0][1];
+}
+
+// finalise one node from its 216-scaled raw moments (m[1..3] lack their base 216 u) and store (Eq. 12)
+template <typename T>
+__device__ __forceinline__ void finalize_store(const T (&m)[TSLB_NF], const T (&uo)[3], T *__restrict__ Bbuf, long long N, long long idx)
+{
+    // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
+    const T hi = (T)(1.0 / 216.0);
+    const T lo = (T)(1.0 / 216.0 - (double)hi);
+    const T dR = fma(m[0], lo, m[0] * hi);
+    const T rho = (T)1 + dR;
+    const T inv = (T)1 / ((T)216 + m[0]);
+    // u' = (216 u + J) / (216 + dR216) = u + (J - u dR216) / (216 + dR216)
+    const T ux = fma(fma(-uo[0], m[0], m[1]), inv, uo[0]);
+    const T uy = fma(fma(-uo[1], m[0], m[2]), inv, uo[1]);
+    const T uz = fma(fma(-uo[2], m[0], m[3]), inv, uo[2]);
+    const T third = (T)(1.0 / 3.0);
+    const T iso = third * dR;
+    Bbuf[idx] = dR;
+    Bbuf[N + idx] = ux;
+    Bbuf[2 * N + idx] = uy;
+    Bbuf[3 * N + idx] = uz;
+    Bbuf[4 * N + idx] = fma(m[4], lo, m[4] * hi) - iso - rho * ux * ux;
+    Bbuf[5 * N + idx] = fma(m[5], lo, m[5] * hi) - iso - rho * uy * uy;
+    Bbuf[6 * N + idx] = fma(m[6], lo, m[6] * hi) - iso - rho * uz * uz;
+    Bbuf[7 * N + idx] = fma(m[7], lo, m[7] * hi) - rho * ux * uy;
+    Bbuf[8 * N + idx] = fma(m[8], lo, m[8] * hi) - rho * ux * uz;
+    Bbuf[9 * N + idx] = fma(m[9], lo, m[9] * hi) - rho * uy * uz;
+}
+
+// index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
+__host__ __device__ constexpr int gidx(int px, int py) { return py == 0 ? px : (py == 1 ? 3 + px : 5); }
+
+// TMA needs the byte offset of the box origin along x to be a multiple of 16 (measured on B200: an origin at a
+// multiple of 2 floats raises "illegal instruction").  The CTA's first column sits at element 30*seg, so the fp32 box
+// starts at that index rounded down to a multiple of 4 and is 36 wide; lanes read at an offset of 0 or 2.
+template <typename T> struct TileGeom;
+template <> struct TileGeom<float> { static constexpr int BXW = 36, ALIGN = 4; };
+template <> struct TileGeom<double> { static constexpr int BXW = 32, ALIGN = 2; };
+template <typename T> __host__ __device__ constexpr int box_elems() { return TSLB_NF * TILE_BY * TileGeom<T>::BXW; }
+// ring stride per stage in elements: box bytes rounded up to 128 (TMA destination alignment)
+template <typename T> __host__ __device__ constexpr int stage_elems() { return (int)(((box_elems<T>() * sizeof(T) + 127) / 128 * 128) / sizeof(T)); }
+
+template <typename T, bool WALLY>
+__global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
+                                                                   T *__restrict__ Bbuf, TileParams<T> p)
+{
+    typedef typename PackOf<T>::type P;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    T *ring = reinterpret_cast<T *>(smem_raw);          // TILE_NS stages of [10][TILE_BY][BXW]
+    constexpr int BXW = TileGeom<T>::BXW;
+    constexpr int STAGE_ELEMS = stage_elems<T>();
+    __shared__ uint64_t full_bar[TILE_NS];
+
+    const int lane = threadIdx.x & 31;
+    const int wid = threadIdx.x >> 5;
+    const Layout &L = p.L;
+    const long long N = L.field;
+
+    // ---- columns: the CTA outputs [xs, xs+30); lane l holds column xs - 1 + l -------------------------------
+    const int xs = blockIdx.x * TILE_COLS;
+    const int col = xs - 1 + lane;
+    const int xb = xs & ~(TileGeom<T>::ALIGN - 1);       // box origin (element index in the padded row), 16-byte aligned
+    const bool col_out = lane >= 1 && lane <= TILE_COLS && col < L.nx;  // this lane produces output
+    // ---- rows: pack .x = row r0, .y = row r0+1; halo rows r0-1, r0+2 ------------------------------------------
+    const int row0 = blockIdx.y * (2 * TILE_WY);
+    const int r0 = row0 + 2 * wid;
+    const bool warp_active = r0 < L.ny;
+    const bool row1_valid = r0 + 1 < L.ny;
+    // rows beyond a bounce-back wall contribute nothing (their part is added by bounce_y_correction)
+    const bool ghost_lo = WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && r0 == 0;                 // row r0-1
+    const bool ghost_mid = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 1 == L.ny;         // rows r0+1, r0+2
+    const bool ghost_hi = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 2 == L.ny;          // row r0+2
+    const bool any_ghost = ghost_lo || ghost_mid || ghost_hi;
+
+    const int z0 = blockIdx.z * p.zchunk;
+    const int z1 = min(z0 + p.zchunk, L.nz);
+    const int nplanes = z1 - z0 + 2;                     // source planes z0-1 .. z1
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < TILE_NS; ++s) mbar_init(&full_bar[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    // plane i of this CTA = source plane z0-1+i: box origin (element xs, padded row row0, padded plane z0+i, field 0)
+    auto issue = [&](int i) {
+        const int s = i % TILE_NS;
+        mbar_expect_tx(&full_bar[s], (uint32_t)(box_elems<T>() * sizeof(T)));
+        tma_load_4d(ring + s * STAGE_ELEMS, &tmA, &full_bar[s], xb, row0, z0 + i, 0);
+    };
+    if (threadIdx.x == 0)
+        for (int i = 0; i < TILE_NS && i < nplanes; ++i) issue(i);
+
+    // z-march state per (px,py) group: Vp of plane zs-2, centre term of plane zs-1, Vp of plane zs-1
+    P vp2[6], cc1[6], vp1[6];
+    // increment form along z: velocity of the previous plane and its backward difference, rows r0, r0+1
+    P uprev[3], dprev[3];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); cc1[i] = vp2[i]; vp1[i] = vp2[i]; }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
+
+    for (int i = 0; i < nplanes; ++i) {
+        const int stg = i % TILE_NS;
+        mbar_wait(&full_bar[stg], (uint32_t)((i / TILE_NS) & 1));
+        if (warp_active) {
+            const int zs = z0 - 1 + i;
+            const T *S = ring + stg * STAGE_ELEMS + (2 * wid) * BXW + (xs - xb) + lane;
+
+            // ---- a1: moments of rows r0-1 .. r0+2 at this column, packed (r0-1,r0) and (r0+1,r0+2) -------------
+            P rlo[TSLB_NF], rhi[TSLB_NF];
+#pragma unroll
+            for (int f = 0; f < TSLB_NF; ++f) {
+                const T *s = S + f * (TILE_BY * BXW);
+                rlo[f] = pk(s[0], s[BXW]);
+                rhi[f] = pk(s[2 * BXW], s[3 * BXW]);
+            }
+            // ---- increment form: centre velocities and their exact differences along y, x, z --------------------
+            P uc[3], Ly[3], Dy[3], Lx[3], Dx[3], Lz[3], Dz[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                P up = rlo[1 + a], dn = rhi[1 + a];
+                uc[a] = pk(up.y, dn.x);
+                if (any_ghost) {   // a node beyond a wall enters the differences as u = 0
+                    if (ghost_lo) up.x = (T)0;
+                    if (ghost_hi) dn.y = (T)0;
+                    if (ghost_mid) { dn.x = (T)0; dn.y = (T)0; }
+                }
+                const P dm = psub(up, uc[a]), dp = psub(dn, uc[a]);
+                Ly[a] = padd(dm, dp);
+                Dy[a] = psub(dm, dp);
+                const T *s = S + (1 + a) * (TILE_BY * BXW);
+                const P xl = pk(s[BXW - 1], s[2 * BXW - 1]), xr = pk(s[BXW + 1], s[2 * BXW + 1]);
+                const P em = psub(xl, uc[a]), ep = psub(xr, uc[a]);
+                Lx[a] = padd(em, ep);
+                Dx[a] = psub(em, ep);
+                const P dcur = psub(uc[a], uprev[a]);        // u(zs) - u(zs-1)
+                Lz[a] = psub(dcur, dprev[a]);               // at the target plane zs-1
+                Dz[a] = psub(pmuls(dprev[a], (T)-1), dcur); // u(zs-2) - u(zs)
+                dprev[a] = dcur;
+            }
+
+            P vp0[6], vm0[6], cc0[6];  // this plane's Vp, Vm, centre term per group
+#pragma unroll
+            for (int kz = 0; kz < 3; ++kz) {
+                // ---- a2: Hermite coefficients of the four rows for this kz --------------------------------------
+                P Alo[3][3], Ahi[3][3];
+                if (kz == 0) { hermite_round<0, P, T>(rlo, p.beta, p.g, Alo); hermite_round<0, P, T>(rhi, p.beta, p.g, Ahi); }
+                if (kz == 1) { hermite_round<1, P, T>(rlo, p.beta, p.g, Alo); hermite_round<1, P, T>(rhi, p.beta, p.g, Ahi); }
+                if (kz == 2) { hermite_round<2, P, T>(rlo, p.beta, p.g, Alo); hermite_round<2, P, T>(rhi, p.beta, p.g, Ahi); }
+                if (any_ghost) {
+#pragma unroll
+                    for (int kx = 0; kx < 3; ++kx)
+#pragma unroll
+                        for (int ky = 0; ky < 3; ++ky)
+                            if (kvalid(kx, ky, kz)) {
+                                if (ghost_lo) Alo[kx][ky].x = (T)0;
+                                if (ghost_hi) Ahi[kx][ky].y = (T)0;
+                                if (ghost_mid) { Ahi[kx][ky].x = (T)0; Ahi[kx][ky].y = (T)0; }
+                            }
+                }
+                // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 -------------------------
+                P G1[3][3];
+#pragma unroll
+                for (int kx = 0; kx < 3; ++kx) {
+                    if (!kvalid(kx, 0, kz)) continue;
+                    P Sq[3], Dq[3];
+#pragma unroll
+                    for (int ky = 0; ky < 3; ++ky)
+                        if (kvalid(kx, ky, kz)) { Sq[ky] = padd(Alo[kx][ky], Ahi[kx][ky]); Dq[ky] = psub(Alo[kx][ky], Ahi[kx][ky]); }
+                    const P c0 = pk(Alo[kx][0].y, Ahi[kx][0].x);
+                    if (kvalid(kx, 2, kz)) {
+                        const P c2 = pk(Alo[kx][2].y, Ahi[kx][2].x);
+                        pass_group<3, P, T>(Sq, Dq, c0, c2, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    } else if (kvalid(kx, 1, kz)) {
+                        pass_group<2, P, T>(Sq, Dq, c0, c0, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    } else {
+                        pass_group<1, P, T>(Sq, Dq, c0, c0, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    }
+                }
+                // y-stage increments of the bases 3 u_a (tap sums along y: 6, 0, 2 for py = 0, 1, 2 when ky = 0; 0, 2, 0 when ky = 1)
+                if (kz == 0) {
+                    G1[0][1] = pfmas(Ly[0], (T)3, G1[0][1]); G1[1][1] = pfmas(Dy[0], (T)3, G1[1][1]); G1[2][1] = pfmas(Ly[0], (T)3, G1[2][1]);
+                    G1[0][0] = pfmas(Dy[1], (T)3, G1[0][0]); G1[1][0] = pfmas(Ly[1], (T)3, G1[1][0]); G1[2][0] = pfmas(Dy[1], (T)3, G1[2][0]);
+                }
+                if (kz == 1) {
+                    G1[0][0] = pfmas(Ly[2], (T)3, G1[0][0]); G1[1][0] = pfmas(Dy[2], (T)3, G1[1][0]); G1[2][0] = pfmas(Ly[2], (T)3, G1[2][0]);
+                }
+                // ---- x pass (warp shuffles): G2[px][py] = sum_kx T^x_{px,kx} G1[py][kx]; then the z bookkeeping ----
+#pragma unroll
+                for (int py = 0; py < 3; ++py) {
+                    P Sq[3], Dq[3];
+#pragma unroll
+                    for (int kx = 0; kx < 3; ++kx)
+                        if (kvalid(kx, 0, kz)) {
+                            const P up = shfl_up1(G1[py][kx]);  // value at column-1  (c_x = +1 pulls from x-1)
+                            const P dn = shfl_dn1(G1[py][kx]);  // value at column+1
+                            Sq[kx] = padd(up, dn);
+                            Dq[kx] = psub(up, dn);
+                        }
+                    P o[3];
+                    if (kvalid(2, 0, kz)) pass_group<3, P, T>(Sq, Dq, G1[py][0], G1[py][2], o[0], o[1], o[2]);
+                    else pass_group<2, P, T>(Sq, Dq, G1[py][0], G1[py][0], o[0], o[1], o[2]);
+                    // x-stage increments: base multipliers after the y stage are 18 (py=0) and 6 (py=2) for ux (kx=1) and uz
+                    // (kx=0, kz=1), 6 (py=1) for uy (kx=0)
+                    if (kz == 0 && py == 0) { o[0] = pfmas(Dx[0], (T)18, o[0]); o[1] = pfmas(Lx[0], (T)18, o[1]); o[2] = pfmas(Dx[0], (T)18, o[2]); }
+                    if (kz == 0 && py == 2) { o[0] = pfmas(Dx[0], (T)6, o[0]); }
+                    if (kz == 0 && py == 1) { o[0] = pfmas(Lx[1], (T)6, o[0]); o[1] = pfmas(Dx[1], (T)6, o[1]); }
+                    if (kz == 1 && py == 0) { o[0] = pfmas(Lx[2], (T)18, o[0]); o[1] = pfmas(Dx[2], (T)18, o[1]); o[2] = pfmas(Lx[2], (T)18, o[2]); }
+                    if (kz == 1 && py == 2) { o[0] = pfmas(Lx[2], (T)6, o[0]); }
+#pragma unroll
+                    for (int px = 0; px + py <= 2; ++px) {
+                        const int gi = gidx(px, py);
+                        const P v = o[px];
+                        // Vp = phi0 + phi1 + phi2, Vm = phi0 - phi1 + phi2, centre = 4 phi0 - 2 phi2   (over kz)
+                        if (kz == 0) { vp0[gi] = v; vm0[gi] = v; cc0[gi] = pmuls(v, (T)4); }
+                        if (kz == 1) { vp0[gi] = padd(vp0[gi], v); vm0[gi] = psub(vm0[gi], v); }
+                        if (kz == 2) { vp0[gi] = padd(vp0[gi], v); vm0[gi] = padd(vm0[gi], v); cc0[gi] = pfmas(v, (T)-2, cc0[gi]); }
+                    }
+                }
+            }
+
+            // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
+            //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
+            const int zt = zs - 1;
+            if (zt >= z0 && col_out) {
+                P m[TSLB_NF];
+                {
+                    const P e00 = padd(vp2[0], vm0[0]);
+                    m[0] = pfmas(Dz[2], (T)108, padd(e00, cc1[0]));            // 000
+                    m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));         // 001
+                    m[6] = pfmas(Dz[2], (T)108, e00);                          // 002
+                    const P e10 = padd(vp2[1], vm0[1]);
+                    m[1] = pfmas(Lz[0], (T)36, padd(e10, cc1[1]));             // 100
+                    m[8] = pfmas(Dz[0], (T)36, psub(vp2[1], vm0[1]));          // 101
+                    const P e01 = padd(vp2[3], vm0[3]);
+                    m[2] = pfmas(Lz[1], (T)36, padd(e01, cc1[3]));             // 010
+                    m[9] = pfmas(Dz[1], (T)36, psub(vp2[3], vm0[3]));          // 011
+                    m[4] = pfmas(Dz[2], (T)36, padd(padd(vp2[2], vm0[2]), cc1[2]));   // 200
+                    m[7] = padd(padd(vp2[4], vm0[4]), cc1[4]);                 // 110
+                    m[5] = pfmas(Dz[2], (T)36, padd(padd(vp2[5], vm0[5]), cc1[5]));   // 020
+                }
+                const long long i0 = lay_idx(L, col, r0, zt);
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    const int r = r0 + s;
+                    if (s == 1 && !row1_valid) break;
+                    const long long idx = i0 + (long long)s * L.px;
+                    T ms[TSLB_NF], uo[3];
+#pragma unroll
+                    for (int f = 0; f < TSLB_NF; ++f) ms[f] = s == 0 ? m[f].x : m[f].y;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) uo[a] = s == 0 ? uprev[a].x : uprev[a].y;
+                    if (WALLY) {
+                        if (r == 0 && p.kind[2] == TSLB_BC_BOUNCE_BACK) bounce_y_correction<T>(Abuf, N, idx, p.beta, p.g, true, ms);
+                        if (r == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK) bounce_y_correction<T>(Abuf, N, idx, p.beta, p.g, false, ms);
+                    }
+                    finalize_store<T>(ms, uo, Bbuf, N, idx);
+                }
+            }
+            // ---- shift the march state ---------------------------------------------------------------------------------
+#pragma unroll
+            for (int g = 0; g < 6; ++g) { vp2[g] = vp1[g]; vp1[g] = vp0[g]; cc1[g] = cc0[g]; }
+#pragma unroll
+            for (int a = 0; a < 3; ++a) uprev[a] = uc[a];
+        }
+        __syncthreads();                                  // every warp is done with stage `stg`: refill it
+        if (threadIdx.x == 0 && i + TILE_NS < nplanes) issue(i + TILE_NS);
+    }
+}
+
+template <typename T>
+TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
+{
+    TileParams<T> p;
+    p.L = c->L;
+    for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
+    p.beta = (T)(1.0 - c->omega);
+    for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
+    const int gx = (c->nx + TILE_COLS - 1) / TILE_COLS;
+    const int gy = (c->ny + 2 * TILE_WY - 1) / (2 * TILE_WY);
+    // z chunks: enough CTAs to fill the SMs a few times over, chunks long enough to amortise the 2 halo planes
+    const long long cols = (long long)gx * gy;
+    int chunks = (int)((8LL * c->sm_count + cols - 1) / cols);
+    if (chunks < 1) chunks = 1;
+    int zc = (c->nz + chunks - 1) / chunks;
+    if (zc < 16) zc = c->nz < 16 ? c->nz : 16;
+    p.zchunk = zc;
+    *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
+    return p;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+bool tslb_tile_supported(const tslb_ctx *c, const char **why)
+{
+    // bounce-back walls are handled on the y faces only (x or z walls: gather kernel)
+    for (int f = 0; f < 6; ++f)
+        if (c->kind[f] == TSLB_BC_BOUNCE_BACK && (f >> 1) != 1) {
+            if (why) *why = "bounce-back walls on x or z faces";
+            return false;
+        }
+    if (c->ws && !c->tmap_ok) {
+        if (why) *why = "TMA descriptors unavailable";
+        return false;
+    }
+    if (why) *why = "";
+    return true;
+}
+
+// TMA descriptors of the two moment buffers: 4-D tensor (x, y, z, field) of the padded SoA layout, box 36|32 x 10 x 1 x 10.
+// cuTensorMapEncodeTiled is fetched through the runtime so that the library links against cudart only.
+cudaError_t tslb_tile_prepare(tslb_ctx *c)
+{
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    const Layout &L = c->L;
+    const size_t es = tslb_elem(c);
+    const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)L.pz, TSLB_NF};
+    const cuuint64_t strides[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
+    const cuuint32_t box[4] = {(cuuint32_t)(c->dtype == TSLB_F64 ? TileGeom<double>::BXW : TileGeom<float>::BXW), TILE_BY, 1, TSLB_NF};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    for (int b = 0; b < 2; ++b) {
+        CUresult r = ((EncodeTiledFn)fn)(&c->tmap[b], c->dtype == TSLB_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                                         4, c->buf[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    const int smem32 = TILE_NS * stage_elems<float>() * 4, smem64 = TILE_NS * stage_elems<double>() * 8;
+    e = cudaFuncSetAttribute(sweep_tile_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem64);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem64);
+    if (e != cudaSuccess) return e;
+    c->tmap_ok = 1;
+    return cudaSuccess;
+}
+
+cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
+{
+    const bool wally = c->kind[2] == TSLB_BC_BOUNCE_BACK || c->kind[3] == TSLB_BC_BOUNCE_BACK;
+    dim3 grid;
+    if (c->dtype == TSLB_F32) {
+        TileParams<float> p = make_tile<float>(c, &grid);
+        const size_t smem = (size_t)TILE_NS * stage_elems<float>() * sizeof(float);
+        if (wally) sweep_tile_kernel<float, true><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<float, false><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
+    } else {
+        TileParams<double> p = make_tile<double>(c, &grid);
+        const size_t smem = (size_t)TILE_NS * stage_elems<double>() * sizeof(double);
+        if (wally) sweep_tile_kernel<double, true><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<double, false><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
+    }
+    c->launches++;
+    return cudaGetLastError();
+}

@@ -25,7 +25,21 @@ int cuda_fail(tslb_ctx *c, const char *what, cudaError_t e)
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
-size_t buffer_bytes(const tslb_ctx *c) { return align256(TSLB_NF * tslb_sites(c) * tslb_elem(c)); }
+size_t buffer_bytes(const tslb_ctx *c) { return align256((size_t)TSLB_NF * (size_t)c->L.field * tslb_elem(c)); }
+
+// padded internal layout (tslb_internal.h): one ghost layer on every side, 16-byte rows, never smaller than a TMA box
+Layout make_layout(int nx, int ny, int nz)
+{
+    Layout L;
+    L.nx = nx; L.ny = ny; L.nz = nz;
+    L.px = (nx + 2 + 3) & ~3;
+    if (L.px < 64) L.px = 64;
+    L.py = ny + 2 < TILE_BY ? TILE_BY : ny + 2;
+    L.pz = nz + 2;
+    L.plane = (long long)L.px * L.py;
+    L.field = L.plane * L.pz;
+    return L;
+}
 
 int check_ready(tslb_ctx *c, bool need_state)
 {
@@ -43,12 +57,29 @@ int check_boundary_set(tslb_ctx *c)
     return TSLB_OK;
 }
 
+// Boundary nodes of the open faces filled at time t (oracle step 1) and, for the tile kernel, the ghost layers
+// refreshed from the filled state.  Idempotent for a given (buffer, t): skipped when already done.
+cudaError_t refresh_boundary(tslb_ctx *c, bool need_halo, cudaStream_t st)
+{
+    if (c->halo_valid >= (need_halo ? 2 : 1)) return cudaSuccess;
+    cudaError_t e = cudaSuccess;
+    if (c->halo_valid < 1) e = tslb_launch_fill(c, c->buf[c->cur], st);
+    if (e != cudaSuccess) return e;
+    c->halo_valid = 1;
+    if (need_halo) {
+        e = tslb_launch_halo(c, c->buf[c->cur], st);
+        if (e != cudaSuccess) return e;
+        c->halo_valid = 2;
+    }
+    return cudaSuccess;
+}
+
 int pick_kernel(const tslb_ctx *c, const char **why)
 {
-    const bool ok = tslb_march_supported(c, why);
+    const bool ok = tslb_tile_supported(c, why);
     if (c->kernel_req == TSLB_KERNEL_GATHER) return TSLB_KERNEL_GATHER;
-    if (c->kernel_req == TSLB_KERNEL_MARCH) return ok ? TSLB_KERNEL_MARCH : -1;
-    return ok ? TSLB_KERNEL_MARCH : TSLB_KERNEL_GATHER;
+    if (c->kernel_req == TSLB_KERNEL_TILE) return ok ? TSLB_KERNEL_TILE : -1;
+    return ok ? TSLB_KERNEL_TILE : TSLB_KERNEL_GATHER;
 }
 
 }  // namespace
@@ -68,6 +99,7 @@ int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out)
     c->tau = tau; c->omega = 1.0 / tau;
     c->kernel_req = TSLB_KERNEL_AUTO;
     c->sm_count = 148;
+    c->L = make_layout(nx, ny, nz);
     *out = c;
     return TSLB_OK;
 }
@@ -97,7 +129,13 @@ int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
     c->buf[0] = dev_ptr;
     c->buf[1] = (char *)dev_ptr + buffer_bytes(c);
     c->scratch = (double *)((char *)dev_ptr + 2 * buffer_bytes(c));
-    c->cur = 0; c->t = 0; c->have_state = 0;
+    c->cur = 0; c->t = 0; c->have_state = 0; c->halo_valid = 0;
+    // padding cells are never written by the kernels: give them a defined (zero) value once
+    e = cudaMemset(dev_ptr, 0, 2 * buffer_bytes(c));
+    if (e != cudaSuccess) return cuda_fail(c, "cudaMemset(workspace)", e);
+    c->tmap_ok = 0;
+    e = tslb_tile_prepare(c);            // TMA descriptors of the two buffers (no-op failure => gather kernel only)
+    if (e != cudaSuccess) return cuda_fail(c, "TMA descriptor setup", e);
     return TSLB_OK;
 }
 
@@ -108,7 +146,7 @@ int tslb_set_moments(tslb_ctx *c, const void *dev_src, void *stream)
     if (!dev_src) return fail(c, TSLB_EINVAL, "dev_src == NULL");
     cudaError_t e = tslb_launch_import(c, dev_src, c->buf[0], (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
-    c->cur = 0; c->t = 0; c->have_state = 1;
+    c->cur = 0; c->t = 0; c->have_state = 1; c->halo_valid = 0;
     return TSLB_OK;
 }
 
@@ -125,7 +163,7 @@ int tslb_set_moments_host(tslb_ctx *c, const void *host_src, void *stream)
     if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(c, "cudaStreamSynchronize", e);
-    c->cur = 0; c->t = 0; c->have_state = 1;
+    c->cur = 0; c->t = 0; c->have_state = 1; c->halo_valid = 0;
     return TSLB_OK;
 }
 
@@ -155,13 +193,14 @@ int tslb_set_boundary(tslb_ctx *c, int face, int kind, const void *params)
         memset(&c->inlet[face], 0, sizeof c->inlet[face]);
     }
     c->kind[face] = kind;
+    c->halo_valid = 0;
     return TSLB_OK;
 }
 
 int tslb_set_kernel(tslb_ctx *c, int kernel)
 {
     if (!c) return TSLB_EINVAL;
-    if (kernel < TSLB_KERNEL_AUTO || kernel > TSLB_KERNEL_MARCH) return fail(c, TSLB_EINVAL, "unknown kernel id");
+    if (kernel < TSLB_KERNEL_AUTO || kernel > TSLB_KERNEL_TILE) return fail(c, TSLB_EINVAL, "unknown kernel id");
     c->kernel_req = kernel;
     return TSLB_OK;
 }
@@ -182,15 +221,16 @@ int tslb_step(tslb_ctx *c, int n, void *stream)
     if (rc) return rc;
     const char *why = "";
     const int k = pick_kernel(c, &why);
-    if (k < 0) return fail(c, TSLB_EINVAL, "TSLB_KERNEL_MARCH does not cover this configuration: %s", why);
+    if (k < 0) return fail(c, TSLB_EINVAL, "TSLB_KERNEL_TILE does not cover this configuration: %s", why);
     cudaStream_t st = (cudaStream_t)stream;
     for (int s = 0; s < n; ++s) {
-        cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);           // step 1: boundary nodes at time t
-        if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
-        e = (k == TSLB_KERNEL_MARCH) ? tslb_launch_march(c, st) : tslb_launch_gather(c, st);  // steps 2-4
+        cudaError_t e = refresh_boundary(c, k == TSLB_KERNEL_TILE, st);    // step 1: boundary nodes (+ ghost layers) at time t
+        if (e != cudaSuccess) return cuda_fail(c, "fill/halo kernel", e);
+        e = (k == TSLB_KERNEL_TILE) ? tslb_launch_tile(c, st) : tslb_launch_gather(c, st);  // steps 2-4
         if (e != cudaSuccess) return cuda_fail(c, "sweep kernel", e);
         c->cur = 1 - c->cur;                                               // step 5: AB flip-flop
         c->t += 1;
+        c->halo_valid = 0;
     }
     return TSLB_OK;
 }
@@ -201,7 +241,7 @@ int tslb_get_moments(tslb_ctx *c, void *dev_dst, void *stream)
     if (rc) return rc;
     if (!dev_dst) return fail(c, TSLB_EINVAL, "dev_dst == NULL");
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);
+    cudaError_t e = refresh_boundary(c, false, st);
     if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
     e = tslb_launch_export(c, c->buf[c->cur], dev_dst, st);
     if (e != cudaSuccess) return cuda_fail(c, "export kernel", e);
@@ -214,7 +254,7 @@ int tslb_get_moments_host(tslb_ctx *c, void *host_dst, void *stream)
     if (rc) return rc;
     if (!host_dst) return fail(c, TSLB_EINVAL, "host_dst == NULL");
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = tslb_launch_fill(c, c->buf[c->cur], st);
+    cudaError_t e = refresh_boundary(c, false, st);
     if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
     // the other buffer holds only the stale time t-1 state: use it as the staging area
     e = tslb_launch_export(c, c->buf[c->cur], c->buf[1 - c->cur], st);
@@ -239,6 +279,6 @@ int tslb_diagnostics(tslb_ctx *c, double *dev_out5, void *stream)
 long long tslb_step_count(const tslb_ctx *c) { return c && c->have_state ? c->t : -1; }
 long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
 const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err : g_create_err; }
-const char *tslb_version(void) { return "tslb-b200 0.1 (sm_100a)"; }
+const char *tslb_version(void) { return "tslb-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

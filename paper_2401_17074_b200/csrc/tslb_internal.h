@@ -1,17 +1,34 @@
-// tslb_internal.h -- host-side context and the parameter block handed to every kernel.
+// tslb_internal.h -- host-side context, the device-visible layout/parameter blocks and the launcher prototypes.
 // Product code (CUDA path).  Shares nothing with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
 #include "../../include/tslb.h"
 
-#define TSLB_NF 10  // rho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz
+#define TSLB_NF 10  // dr = rho - 1, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz
+
+// ---- internal moment-buffer layout -------------------------------------------------
+// SoA, one padded box per field: [pz = nz+2][py][px] elements, x fastest.  Node (x,y,z), -1 <= x <= nx etc.
+// (index -1 and n are the ghost layers), lives at element  (z+1)*plane + (y+1)*px + (x+1)  of its field.
+// px is a multiple of 4 (16-byte rows for TMA) and px >= 64, py >= ny+2 and py >= the TMA box height.
+struct Layout {
+    int nx, ny, nz;
+    int px, py, pz;
+    long long plane;  // px*py
+    long long field;  // px*py*pz
+};
+
+__host__ __device__ inline long long lay_idx(const Layout &L, int x, int y, int z)
+{
+    return (long long)(z + 1) * L.plane + (long long)(y + 1) * L.px + (x + 1);
+}
 
 // Device-visible description of one lattice + its boundary set (passed by value).
 template <typename T>
 struct SweepParams {
-    int nx, ny, nz;
+    Layout L;
     int kind[6];   // TSLB_BC_* per face
     T beta;        // 1 - omega = 1 - 1/tau, formed in double and rounded once (Eq. 5)
     T g[3];        // body acceleration
@@ -25,11 +42,18 @@ struct InletDev {
 };
 
 struct FillParams {
-    int nx, ny, nz;
+    Layout L;
     int kind[6];
     InletDev inlet[6];
     long long t;  // step index the fill belongs to (noise counter)
 };
+
+// geometry of the TMA-staged tile kernel (kernels_tile.cu)
+#define TILE_WY 4                       // warps per CTA, stacked along y; each warp owns 2 rows x 30 columns
+#define TILE_BX 32                      // lanes per warp row: 30 output columns + 1 halo column on each side
+#define TILE_BY (2 * TILE_WY + 2)       // TMA box height (8 output rows + 1 halo row on each side)
+#define TILE_NS 4                       // planes in the shared-memory ring
+#define TILE_COLS 30
 
 struct tslb_ctx {
     int nx, ny, nz, dtype;
@@ -37,14 +61,19 @@ struct tslb_ctx {
     double g[3];
     int kind[6];
     InletDev inlet[6];
+    Layout L;
     // device memory (caller-owned workspace)
     void *ws;
     size_t ws_bytes;
-    void *buf[2];     // moment buffers, internal form: field 0 holds rho - 1
+    void *buf[2];     // moment buffers, internal form (padded SoA, field 0 holds rho - 1)
     double *scratch;  // diagnostics partials
+    void *stage;      // staging area for the *_host calls (API layout)
+    CUtensorMap tmap[2];  // TMA descriptors of buf[0], buf[1]
+    int tmap_ok;
     int cur;          // buf[cur] holds time t
     long long t;
     int have_state;
+    int halo_valid;   // ghost layers + open-face boundary nodes of buf[cur] are up to date for time t
     int kernel_req;   // TSLB_KERNEL_*
     int sm_count;
     long long launches;
@@ -59,9 +88,11 @@ static inline size_t tslb_sites(const tslb_ctx *c) { return (size_t)c->nx * c->n
 
 // launchers (defined in the .cu files; all asynchronous on `st`, return cudaGetLastError())
 cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st);
-cudaError_t tslb_launch_march(tslb_ctx *c, cudaStream_t st);
-bool tslb_march_supported(const tslb_ctx *c, const char **why);
-cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st);
+cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st);
+bool tslb_tile_supported(const tslb_ctx *c, const char **why);
+cudaError_t tslb_tile_prepare(tslb_ctx *c);                                               // TMA descriptors, smem opt-in
+cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st);                    // open-face boundary nodes at time t
+cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st);                    // ghost layers
 cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // API -> internal
 cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // internal -> API
 cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st);
