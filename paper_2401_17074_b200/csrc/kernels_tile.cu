@@ -13,7 +13,7 @@
 // padded SoA buffer into a 4-deep shared-memory ring with TMA (cp.async.bulk.tensor.4d, mbarrier complete_tx);
 // ghost layers in the buffer stand for the periodic images, so the kernel has no wrap logic.  Every warp owns
 // 2 rows (packed in a 2-wide register pair so fp32 issues as FFMA2/FADD2) x 32 columns (30 outputs + 2 halo lanes):
-//   y pass: in registers, from the A_k of rows r0-1 .. r0+2 read from shared memory,
+//   y pass: in registers, from the A_k of rows r0-1 .. r0+2 read from shared memory (packs (r0,r0+1) and (r0-1,r0+2)),
 //   x pass: neighbours' values by warp shuffles,
 //   z pass: by marching -- 3 running values per (px,py) group, no plane is staged twice.
 // Each node's moments leave HBM once per tile (halo re-reads hit L2) and the 10 new moments are written once:
@@ -171,6 +171,20 @@ __device__ __forceinline__ void pass_group(const P (&S)[3], const P (&D)[3], P c
     if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
 }
 
+// The same pass for the y stage, where the rows are packed (centre, halo): W_q = D_q * sgn with sgn = (1,-1).
+template <int NQ, typename P, typename T>
+__device__ __forceinline__ void pass_group_y(const P (&S)[3], const P (&W)[3], P c0, P c2, P sgn, P &o0, P &o1, P &o2)
+{
+    P E, O;
+    if (NQ == 1) { E = S[0]; O = pmul(W[0], sgn); }
+    if (NQ == 2) { E = pfma(W[1], sgn, S[0]); O = pfma(W[0], sgn, S[1]); }
+    if (NQ == 3) { E = pfma(W[1], sgn, padd(S[0], S[2])); O = pfma(padd(W[0], W[2]), sgn, S[1]); }
+    o2 = E;
+    o1 = O;
+    o0 = pfmas(c0, (T)4, E);
+    if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
+}
+
 // Contribution of the bounced directions at a node next to a halfway bounce-back wall on a y face
 // (DESIGN.md "Walls in the separable form"): f_i(x,t+1) = f*_ibar(x,t) for the 9 directions with c_y = sgn_in,
 // evaluated from the node's own 216-scaled Hermite coefficients (FULL first-order coefficients here: the increment
@@ -224,32 +238,39 @@ __device__ __noinline__ void bounce_y_correction(const T *__restrict__ Abuf, lon
     out[9] += sg * (T)-12 * Bm[0][1];
 }
 
-// finalise one node from its 216-scaled raw moments (m[1..3] lack their base 216 u) and store (Eq. 12)
-template <typename T>
-__device__ __forceinline__ void finalize_store(const T (&m)[TSLB_NF], const T (&uo)[3], T *__restrict__ Bbuf, long long N, long long idx)
+// finalise the two rows of a pack from their 216-scaled raw moments (m[1..3] lack their base 216 u) and store (Eq. 12)
+template <typename P, typename T>
+__device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&uo)[3], T *__restrict__ Bbuf, long long N, long long i0,
+                                               long long i1, bool row1)
 {
     // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
     const T hi = (T)(1.0 / 216.0);
     const T lo = (T)(1.0 / 216.0 - (double)hi);
-    const T dR = fma(m[0], lo, m[0] * hi);
-    const T rho = (T)1 + dR;
-    const T inv = (T)1 / ((T)216 + m[0]);
+    const P dR = pfmas(m[0], lo, pmuls(m[0], hi));
+    const P rho = padd(pbc<P, T>((T)1), dR);
+    const P den = padd(pbc<P, T>((T)216), m[0]);
+    const P inv = pk((T)1 / den.x, (T)1 / den.y);
+    const P nm0 = pmuls(m[0], (T)-1);
     // u' = (216 u + J) / (216 + dR216) = u + (J - u dR216) / (216 + dR216)
-    const T ux = fma(fma(-uo[0], m[0], m[1]), inv, uo[0]);
-    const T uy = fma(fma(-uo[1], m[0], m[2]), inv, uo[1]);
-    const T uz = fma(fma(-uo[2], m[0], m[3]), inv, uo[2]);
-    const T third = (T)(1.0 / 3.0);
-    const T iso = third * dR;
-    Bbuf[idx] = dR;
-    Bbuf[N + idx] = ux;
-    Bbuf[2 * N + idx] = uy;
-    Bbuf[3 * N + idx] = uz;
-    Bbuf[4 * N + idx] = fma(m[4], lo, m[4] * hi) - iso - rho * ux * ux;
-    Bbuf[5 * N + idx] = fma(m[5], lo, m[5] * hi) - iso - rho * uy * uy;
-    Bbuf[6 * N + idx] = fma(m[6], lo, m[6] * hi) - iso - rho * uz * uz;
-    Bbuf[7 * N + idx] = fma(m[7], lo, m[7] * hi) - rho * ux * uy;
-    Bbuf[8 * N + idx] = fma(m[8], lo, m[8] * hi) - rho * ux * uz;
-    Bbuf[9 * N + idx] = fma(m[9], lo, m[9] * hi) - rho * uy * uz;
+    P o[TSLB_NF];
+    o[0] = dR;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) o[1 + a] = pfma(pfma(uo[a], nm0, m[1 + a]), inv, uo[a]);
+    const P niso = pmuls(dR, (T)(-1.0 / 3.0));
+    const P nrho = pmuls(rho, (T)-1);
+    const P rx = pmul(nrho, o[1]), ry = pmul(nrho, o[2]), rz = pmul(nrho, o[3]);
+    o[4] = pfma(rx, o[1], padd(pfmas(m[4], lo, pmuls(m[4], hi)), niso));
+    o[5] = pfma(ry, o[2], padd(pfmas(m[5], lo, pmuls(m[5], hi)), niso));
+    o[6] = pfma(rz, o[3], padd(pfmas(m[6], lo, pmuls(m[6], hi)), niso));
+    o[7] = pfma(rx, o[2], pfmas(m[7], lo, pmuls(m[7], hi)));
+    o[8] = pfma(rx, o[3], pfmas(m[8], lo, pmuls(m[8], hi)));
+    o[9] = pfma(ry, o[3], pfmas(m[9], lo, pmuls(m[9], hi)));
+#pragma unroll
+    for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i0] = o[f].x;
+    if (row1) {
+#pragma unroll
+        for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i1] = o[f].y;
+    }
 }
 
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
@@ -326,43 +347,47 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
 #pragma unroll
     for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
 
+    const P sgn = pk((T)1, (T)-1);                        // D = W * sgn for the (centre, halo) row packing, see below
+    const bool st_ok = col_out && warp_active;
     for (int i = 0; i < nplanes; ++i) {
         const int stg = i % TILE_NS;
         mbar_wait(&full_bar[stg], (uint32_t)((i / TILE_NS) & 1));
-        if (warp_active) {
+        {   // every warp computes (rows beyond the lattice read defined but meaningless smem rows and store nothing):
+            // no divergent region around the shuffles
             const int zs = z0 - 1 + i;
             const T *S = ring + stg * STAGE_ELEMS + (2 * wid) * BXW + (xs - xb) + lane;
 
-            // ---- a1: moments of rows r0-1 .. r0+2 at this column, packed (r0-1,r0) and (r0+1,r0+2) -------------
-            P rlo[TSLB_NF], rhi[TSLB_NF];
+            // ---- a1: moments of rows r0-1 .. r0+2 at this column.  Packing: C = (r0, r0+1) the two output rows,
+            //      H = (r0-1, r0+2) their outer neighbours.  For the output pack: up = (H.x, C.x), dn = (C.y, H.y), so
+            //      up + dn = H + swap(C) and up - dn = (H - swap(C)) * (1,-1): the centre needs no repacking and the swap
+            //      is an operand modifier of the packed instructions. ------------------------------------------------
+            P rc[TSLB_NF], rh[TSLB_NF];
 #pragma unroll
             for (int f = 0; f < TSLB_NF; ++f) {
                 const T *s = S + f * (TILE_BY * BXW);
-                rlo[f] = pk(s[0], s[BXW]);
-                rhi[f] = pk(s[2 * BXW], s[3 * BXW]);
+                rc[f] = pk(s[BXW], s[2 * BXW]);
+                rh[f] = pk(s[0], s[3 * BXW]);
             }
-            // ---- increment form: centre velocities and their exact differences along y, x, z --------------------
-            P uc[3], Ly[3], Dy[3], Lx[3], Dx[3], Lz[3], Dz[3];
+            // ---- increment form: exact differences of the stored velocities along y, x, z ---------------------------
+            P Ly[3], Wy[3], Lx[3], Dx[3], Lz[3], Dz[3];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                P up = rlo[1 + a], dn = rhi[1 + a];
-                uc[a] = pk(up.y, dn.x);
+                const P uc = rc[1 + a];
+                P hs = rh[1 + a], cs = pk(uc.y, uc.x);
                 if (any_ghost) {   // a node beyond a wall enters the differences as u = 0
-                    if (ghost_lo) up.x = (T)0;
-                    if (ghost_hi) dn.y = (T)0;
-                    if (ghost_mid) { dn.x = (T)0; dn.y = (T)0; }
+                    if (ghost_lo) hs.x = (T)0;
+                    if (ghost_hi) hs.y = (T)0;
+                    if (ghost_mid) { cs.x = (T)0; hs.y = (T)0; }
                 }
-                const P dm = psub(up, uc[a]), dp = psub(dn, uc[a]);
-                Ly[a] = padd(dm, dp);
-                Dy[a] = psub(dm, dp);
+                Ly[a] = pfmas(uc, (T)-2, padd(hs, cs));      // (up - c) + (dn - c)
+                Wy[a] = psub(hs, cs);                        // (up - dn) * sgn
                 const T *s = S + (1 + a) * (TILE_BY * BXW);
                 const P xl = pk(s[BXW - 1], s[2 * BXW - 1]), xr = pk(s[BXW + 1], s[2 * BXW + 1]);
-                const P em = psub(xl, uc[a]), ep = psub(xr, uc[a]);
-                Lx[a] = padd(em, ep);
-                Dx[a] = psub(em, ep);
-                const P dcur = psub(uc[a], uprev[a]);        // u(zs) - u(zs-1)
-                Lz[a] = psub(dcur, dprev[a]);               // at the target plane zs-1
-                Dz[a] = psub(pmuls(dprev[a], (T)-1), dcur); // u(zs-2) - u(zs)
+                Lx[a] = pfmas(uc, (T)-2, padd(xl, xr));
+                Dx[a] = psub(xl, xr);
+                const P dcur = psub(uc, uprev[a]);           // u(zs) - u(zs-1)
+                Lz[a] = psub(dcur, dprev[a]);                // at the target plane zs-1
+                Dz[a] = psub(pmuls(dprev[a], (T)-1), dcur);  // u(zs-2) - u(zs)
                 dprev[a] = dcur;
             }
 
@@ -370,47 +395,40 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
 #pragma unroll
             for (int kz = 0; kz < 3; ++kz) {
                 // ---- a2: Hermite coefficients of the four rows for this kz --------------------------------------
-                P Alo[3][3], Ahi[3][3];
-                if (kz == 0) { hermite_round<0, P, T>(rlo, p.beta, p.g, Alo); hermite_round<0, P, T>(rhi, p.beta, p.g, Ahi); }
-                if (kz == 1) { hermite_round<1, P, T>(rlo, p.beta, p.g, Alo); hermite_round<1, P, T>(rhi, p.beta, p.g, Ahi); }
-                if (kz == 2) { hermite_round<2, P, T>(rlo, p.beta, p.g, Alo); hermite_round<2, P, T>(rhi, p.beta, p.g, Ahi); }
-                if (any_ghost) {
-#pragma unroll
-                    for (int kx = 0; kx < 3; ++kx)
-#pragma unroll
-                        for (int ky = 0; ky < 3; ++ky)
-                            if (kvalid(kx, ky, kz)) {
-                                if (ghost_lo) Alo[kx][ky].x = (T)0;
-                                if (ghost_hi) Ahi[kx][ky].y = (T)0;
-                                if (ghost_mid) { Ahi[kx][ky].x = (T)0; Ahi[kx][ky].y = (T)0; }
-                            }
-                }
+                P Ac[3][3], Ah[3][3];
+                if (kz == 0) { hermite_round<0, P, T>(rc, p.beta, p.g, Ac); hermite_round<0, P, T>(rh, p.beta, p.g, Ah); }
+                if (kz == 1) { hermite_round<1, P, T>(rc, p.beta, p.g, Ac); hermite_round<1, P, T>(rh, p.beta, p.g, Ah); }
+                if (kz == 2) { hermite_round<2, P, T>(rc, p.beta, p.g, Ac); hermite_round<2, P, T>(rh, p.beta, p.g, Ah); }
                 // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 -------------------------
                 P G1[3][3];
 #pragma unroll
                 for (int kx = 0; kx < 3; ++kx) {
                     if (!kvalid(kx, 0, kz)) continue;
-                    P Sq[3], Dq[3];
+                    P Sq[3], Wq[3];
 #pragma unroll
                     for (int ky = 0; ky < 3; ++ky)
-                        if (kvalid(kx, ky, kz)) { Sq[ky] = padd(Alo[kx][ky], Ahi[kx][ky]); Dq[ky] = psub(Alo[kx][ky], Ahi[kx][ky]); }
-                    const P c0 = pk(Alo[kx][0].y, Ahi[kx][0].x);
-                    if (kvalid(kx, 2, kz)) {
-                        const P c2 = pk(Alo[kx][2].y, Ahi[kx][2].x);
-                        pass_group<3, P, T>(Sq, Dq, c0, c2, G1[0][kx], G1[1][kx], G1[2][kx]);
-                    } else if (kvalid(kx, 1, kz)) {
-                        pass_group<2, P, T>(Sq, Dq, c0, c0, G1[0][kx], G1[1][kx], G1[2][kx]);
-                    } else {
-                        pass_group<1, P, T>(Sq, Dq, c0, c0, G1[0][kx], G1[1][kx], G1[2][kx]);
-                    }
+                        if (kvalid(kx, ky, kz)) {
+                            P h = Ah[kx][ky], cs = pk(Ac[kx][ky].y, Ac[kx][ky].x);
+                            if (any_ghost) {   // rows beyond a bounce-back wall send nothing (bounce_y_correction adds their part)
+                                if (ghost_lo) h.x = (T)0;
+                                if (ghost_hi) h.y = (T)0;
+                                if (ghost_mid) { cs.x = (T)0; h.y = (T)0; }
+                            }
+                            Sq[ky] = padd(h, cs);
+                            Wq[ky] = psub(h, cs);
+                        }
+                    if (kvalid(kx, 2, kz)) pass_group_y<3, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][2], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    else if (kvalid(kx, 1, kz)) pass_group_y<2, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][0], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    else pass_group_y<1, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][0], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
                 }
                 // y-stage increments of the bases 3 u_a (tap sums along y: 6, 0, 2 for py = 0, 1, 2 when ky = 0; 0, 2, 0 when ky = 1)
+                const P sg3 = pk((T)3, (T)-3);
                 if (kz == 0) {
-                    G1[0][1] = pfmas(Ly[0], (T)3, G1[0][1]); G1[1][1] = pfmas(Dy[0], (T)3, G1[1][1]); G1[2][1] = pfmas(Ly[0], (T)3, G1[2][1]);
-                    G1[0][0] = pfmas(Dy[1], (T)3, G1[0][0]); G1[1][0] = pfmas(Ly[1], (T)3, G1[1][0]); G1[2][0] = pfmas(Dy[1], (T)3, G1[2][0]);
+                    G1[0][1] = pfmas(Ly[0], (T)3, G1[0][1]); G1[1][1] = pfma(Wy[0], sg3, G1[1][1]); G1[2][1] = pfmas(Ly[0], (T)3, G1[2][1]);
+                    G1[0][0] = pfma(Wy[1], sg3, G1[0][0]); G1[1][0] = pfmas(Ly[1], (T)3, G1[1][0]); G1[2][0] = pfma(Wy[1], sg3, G1[2][0]);
                 }
                 if (kz == 1) {
-                    G1[0][0] = pfmas(Ly[2], (T)3, G1[0][0]); G1[1][0] = pfmas(Dy[2], (T)3, G1[1][0]); G1[2][0] = pfmas(Ly[2], (T)3, G1[2][0]);
+                    G1[0][0] = pfmas(Ly[2], (T)3, G1[0][0]); G1[1][0] = pfma(Wy[2], sg3, G1[1][0]); G1[2][0] = pfmas(Ly[2], (T)3, G1[2][0]);
                 }
                 // ---- x pass (warp shuffles): G2[px][py] = sum_kx T^x_{px,kx} G1[py][kx]; then the z bookkeeping ----
 #pragma unroll
@@ -449,7 +467,7 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
             // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
             //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
             const int zt = zs - 1;
-            if (zt >= z0 && col_out) {
+            if (zt >= z0 && st_ok) {
                 P m[TSLB_NF];
                 {
                     const P e00 = padd(vp2[0], vm0[0]);
@@ -467,28 +485,35 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
                     m[5] = pfmas(Dz[2], (T)36, padd(padd(vp2[5], vm0[5]), cc1[5]));   // 020
                 }
                 const long long i0 = lay_idx(L, col, r0, zt);
+                if (WALLY) {   // warp-uniform: only the warps that own a wall row
+                    const bool wlo = r0 == 0 && p.kind[2] == TSLB_BC_BOUNCE_BACK;
+                    const bool whi0 = r0 == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK;
+                    const bool whi1 = r0 + 1 == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK;
+                    if (wlo || whi0) {
+                        T corr[TSLB_NF];
 #pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    const int r = r0 + s;
-                    if (s == 1 && !row1_valid) break;
-                    const long long idx = i0 + (long long)s * L.px;
-                    T ms[TSLB_NF], uo[3];
+                        for (int f = 0; f < TSLB_NF; ++f) corr[f] = (T)0;
+                        if (wlo) bounce_y_correction<T>(Abuf, N, i0, p.beta, p.g, true, corr);
+                        if (whi0) bounce_y_correction<T>(Abuf, N, i0, p.beta, p.g, false, corr);
 #pragma unroll
-                    for (int f = 0; f < TSLB_NF; ++f) ms[f] = s == 0 ? m[f].x : m[f].y;
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) uo[a] = s == 0 ? uprev[a].x : uprev[a].y;
-                    if (WALLY) {
-                        if (r == 0 && p.kind[2] == TSLB_BC_BOUNCE_BACK) bounce_y_correction<T>(Abuf, N, idx, p.beta, p.g, true, ms);
-                        if (r == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK) bounce_y_correction<T>(Abuf, N, idx, p.beta, p.g, false, ms);
+                        for (int f = 0; f < TSLB_NF; ++f) m[f].x += corr[f];
                     }
-                    finalize_store<T>(ms, uo, Bbuf, N, idx);
+                    if (whi1) {
+                        T corr[TSLB_NF];
+#pragma unroll
+                        for (int f = 0; f < TSLB_NF; ++f) corr[f] = (T)0;
+                        bounce_y_correction<T>(Abuf, N, i0 + L.px, p.beta, p.g, false, corr);
+#pragma unroll
+                        for (int f = 0; f < TSLB_NF; ++f) m[f].y += corr[f];
+                    }
                 }
+                finalize_store<P, T>(m, uprev, Bbuf, N, i0, i0 + L.px, row1_valid);
             }
             // ---- shift the march state ---------------------------------------------------------------------------------
 #pragma unroll
             for (int g = 0; g < 6; ++g) { vp2[g] = vp1[g]; vp1[g] = vp0[g]; cc1[g] = cc0[g]; }
 #pragma unroll
-            for (int a = 0; a < 3; ++a) uprev[a] = uc[a];
+            for (int a = 0; a < 3; ++a) uprev[a] = rc[1 + a];
         }
         __syncthreads();                                  // every warp is done with stage `stg`: refill it
         if (threadIdx.x == 0 && i + TILE_NS < nplanes) issue(i + TILE_NS);
