@@ -276,25 +276,37 @@ __device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
 __host__ __device__ constexpr int gidx(int px, int py) { return py == 0 ? px : (py == 1 ? 3 + px : 5); }
 
+// CTA geometry per dtype: WX x WY warps, each 30 output columns x 2 rows; one CTA per SM (the CTAs of an SM then
+// march in lock-step, which keeps the halo re-reads of neighbouring tiles inside L2 -- DESIGN.md "Tile kernel").
 // TMA needs the byte offset of the box origin along x to be a multiple of 16 (measured on B200: an origin at a
-// multiple of 2 floats raises "illegal instruction").  The CTA's first column sits at element 30*seg, so the fp32 box
-// starts at that index rounded down to a multiple of 4 and is 36 wide; lanes read at an offset of 0 or 2.
+// multiple of 2 floats raises "illegal instruction"): the box starts at the CTA's first column rounded down to ALIGN
+// elements and lanes read at the remaining offset (0 for WX = 2).
 template <typename T> struct TileGeom;
-template <> struct TileGeom<float> { static constexpr int BXW = 36, ALIGN = 4; };
-template <> struct TileGeom<double> { static constexpr int BXW = 32, ALIGN = 2; };
-template <typename T> __host__ __device__ constexpr int box_elems() { return TSLB_NF * TILE_BY * TileGeom<T>::BXW; }
-// ring stride per stage in elements: box bytes rounded up to 128 (TMA destination alignment)
-template <typename T> __host__ __device__ constexpr int stage_elems() { return (int)(((box_elems<T>() * sizeof(T) + 127) / 128 * 128) / sizeof(T)); }
+template <> struct TileGeom<float> { static constexpr int WX = 2, WY = 6, NS = 4, ALIGN = 4; };
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 4, ALIGN = 2; };
+template <typename T> struct TileDims {
+    typedef TileGeom<T> G;
+    static constexpr int WARPS = G::WX * G::WY;
+    static constexpr int COLS = TILE_COLS * G::WX;                                   // output columns per CTA
+    static constexpr int ROWS = 2 * G::WY;                                           // output rows per CTA
+    static constexpr int BY = ROWS + 2;                                              // box height
+    static constexpr int MAXOFF = (COLS % G::ALIGN) ? 2 : 0;
+    static constexpr int BXW = (COLS + 2 + MAXOFF + 3) / 4 * 4;                      // box width = smem row pitch
+    static constexpr int BOX_ELEMS = TSLB_NF * BY * BXW;
+    static constexpr int STAGE_ELEMS = (int)(((BOX_ELEMS * sizeof(T) + 127) / 128 * 128) / sizeof(T));
+    static constexpr int SMEM_BYTES = G::NS * STAGE_ELEMS * (int)sizeof(T);
+};
+static_assert(TileDims<float>::BY <= TILE_MAX_BY && TileDims<double>::BY <= TILE_MAX_BY, "layout height");
 
 template <typename T, bool WALLY>
-__global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
+__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
                                                                    T *__restrict__ Bbuf, TileParams<T> p)
 {
     typedef typename PackOf<T>::type P;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    T *ring = reinterpret_cast<T *>(smem_raw);          // TILE_NS stages of [10][TILE_BY][BXW]
-    constexpr int BXW = TileGeom<T>::BXW;
-    constexpr int STAGE_ELEMS = stage_elems<T>();
+    typedef TileDims<T> TD;
+    T *ring = reinterpret_cast<T *>(smem_raw);          // NS stages of [10][BY][BXW]
+    constexpr int BXW = TD::BXW, TILE_BY = TD::BY, TILE_NS = TileGeom<T>::NS, STAGE_ELEMS = TD::STAGE_ELEMS;
     __shared__ uint64_t full_bar[TILE_NS];
 
     const int lane = threadIdx.x & 31;
@@ -302,14 +314,16 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
     const Layout &L = p.L;
     const long long N = L.field;
 
-    // ---- columns: the CTA outputs [xs, xs+30); lane l holds column xs - 1 + l -------------------------------
-    const int xs = blockIdx.x * TILE_COLS;
+    // ---- columns: the warp outputs [xs, xs+30); lane l holds column xs - 1 + l -------------------------------
+    const int wx = wid % TileGeom<T>::WX, wy = wid / TileGeom<T>::WX;
+    const int xs0 = blockIdx.x * TD::COLS;               // first column of the CTA
+    const int xs = xs0 + wx * TILE_COLS;
     const int col = xs - 1 + lane;
-    const int xb = xs & ~(TileGeom<T>::ALIGN - 1);       // box origin (element index in the padded row), 16-byte aligned
+    const int xb = xs0 & ~(TileGeom<T>::ALIGN - 1);      // box origin (element index in the padded row), 16-byte aligned
     const bool col_out = lane >= 1 && lane <= TILE_COLS && col < L.nx;  // this lane produces output
     // ---- rows: pack .x = row r0, .y = row r0+1; halo rows r0-1, r0+2 ------------------------------------------
-    const int row0 = blockIdx.y * (2 * TILE_WY);
-    const int r0 = row0 + 2 * wid;
+    const int row0 = blockIdx.y * TD::ROWS;
+    const int r0 = row0 + 2 * wy;
     const bool warp_active = r0 < L.ny;
     const bool row1_valid = r0 + 1 < L.ny;
     // rows beyond a bounce-back wall contribute nothing (their part is added by bounce_y_correction)
@@ -332,7 +346,7 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
     // plane i of this CTA = source plane z0-1+i: box origin (element xs, padded row row0, padded plane z0+i, field 0)
     auto issue = [&](int i) {
         const int s = i % TILE_NS;
-        mbar_expect_tx(&full_bar[s], (uint32_t)(box_elems<T>() * sizeof(T)));
+        mbar_expect_tx(&full_bar[s], (uint32_t)(TD::BOX_ELEMS * sizeof(T)));
         tma_load_4d(ring + s * STAGE_ELEMS, &tmA, &full_bar[s], xb, row0, z0 + i, 0);
     };
     if (threadIdx.x == 0)
@@ -355,7 +369,7 @@ __global__ void __launch_bounds__(TILE_WY * 32) sweep_tile_kernel(const __grid_c
         {   // every warp computes (rows beyond the lattice read defined but meaningless smem rows and store nothing):
             // no divergent region around the shuffles
             const int zs = z0 - 1 + i;
-            const T *S = ring + stg * STAGE_ELEMS + (2 * wid) * BXW + (xs - xb) + lane;
+            const T *S = ring + stg * STAGE_ELEMS + (2 * wy) * BXW + (xs - xb) + lane;
 
             // ---- a1: moments of rows r0-1 .. r0+2 at this column.  Packing: C = (r0, r0+1) the two output rows,
             //      H = (r0-1, r0+2) their outer neighbours.  For the output pack: up = (H.x, C.x), dn = (C.y, H.y), so
@@ -528,14 +542,22 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
     for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
     p.beta = (T)(1.0 - c->omega);
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
-    const int gx = (c->nx + TILE_COLS - 1) / TILE_COLS;
-    const int gy = (c->ny + 2 * TILE_WY - 1) / (2 * TILE_WY);
-    // z chunks: enough CTAs to fill the SMs a few times over, chunks long enough to amortise the 2 halo planes
+    const int gx = (c->nx + TileDims<T>::COLS - 1) / TileDims<T>::COLS;
+    const int gy = (c->ny + TileDims<T>::ROWS - 1) / TileDims<T>::ROWS;
+    // z chunks (one CTA per SM is resident): pick the chunk count whose number of waves x (chunk length + 2 halo planes)
+    // is smallest
     const long long cols = (long long)gx * gy;
-    int chunks = (int)((8LL * c->sm_count + cols - 1) / cols);
-    if (chunks < 1) chunks = 1;
-    int zc = (c->nz + chunks - 1) / chunks;
-    if (zc < 16) zc = c->nz < 16 ? c->nz : 16;
+    int best = 1;
+    double best_cost = 1e300;
+    for (int k = 1; k <= 64 && k <= c->nz; ++k) {
+        const int zc = (c->nz + k - 1) / k;
+        if (k > 1 && zc < 8) break;
+        const long long ctas = cols * ((c->nz + zc - 1) / zc);
+        const long long waves = (ctas + c->sm_count - 1) / c->sm_count;
+        const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
+        if (cost < best_cost) { best_cost = cost; best = k; }
+    }
+    const int zc = (c->nz + best - 1) / best;
     p.zchunk = zc;
     *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
     return p;
@@ -576,7 +598,8 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     const size_t es = tslb_elem(c);
     const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)L.pz, TSLB_NF};
     const cuuint64_t strides[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
-    const cuuint32_t box[4] = {(cuuint32_t)(c->dtype == TSLB_F64 ? TileGeom<double>::BXW : TileGeom<float>::BXW), TILE_BY, 1, TSLB_NF};
+    const cuuint32_t box[4] = {(cuuint32_t)(c->dtype == TSLB_F64 ? TileDims<double>::BXW : TileDims<float>::BXW),
+                               (cuuint32_t)(c->dtype == TSLB_F64 ? TileDims<double>::BY : TileDims<float>::BY), 1, TSLB_NF};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     for (int b = 0; b < 2; ++b) {
         CUresult r = ((EncodeTiledFn)fn)(&c->tmap[b], c->dtype == TSLB_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
@@ -585,7 +608,7 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
                                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
-    const int smem32 = TILE_NS * stage_elems<float>() * 4, smem64 = TILE_NS * stage_elems<double>() * 8;
+    const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
     e = cudaFuncSetAttribute(sweep_tile_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem64);
@@ -601,14 +624,14 @@ cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
     dim3 grid;
     if (c->dtype == TSLB_F32) {
         TileParams<float> p = make_tile<float>(c, &grid);
-        const size_t smem = (size_t)TILE_NS * stage_elems<float>() * sizeof(float);
-        if (wally) sweep_tile_kernel<float, true><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<float, false><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
+        const size_t smem = TileDims<float>::SMEM_BYTES;
+        if (wally) sweep_tile_kernel<float, true><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<float, false><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
     } else {
         TileParams<double> p = make_tile<double>(c, &grid);
-        const size_t smem = (size_t)TILE_NS * stage_elems<double>() * sizeof(double);
-        if (wally) sweep_tile_kernel<double, true><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<double, false><<<grid, TILE_WY * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
+        const size_t smem = TileDims<double>::SMEM_BYTES;
+        if (wally) sweep_tile_kernel<double, true><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<double, false><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
     }
     c->launches++;
     return cudaGetLastError();

@@ -33,8 +33,8 @@ Layout make_layout(int nx, int ny, int nz)
     Layout L;
     L.nx = nx; L.ny = ny; L.nz = nz;
     L.px = (nx + 2 + 3) & ~3;
-    if (L.px < 64) L.px = 64;
-    L.py = ny + 2 < TILE_BY ? TILE_BY : ny + 2;
+    if (L.px < 72) L.px = 72;
+    L.py = ny + 2 < TILE_MAX_BY ? TILE_MAX_BY : ny + 2;
     L.pz = nz + 2;
     L.plane = (long long)L.px * L.py;
     L.field = L.plane * L.pz;

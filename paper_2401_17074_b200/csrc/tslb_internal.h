@@ -48,12 +48,9 @@ struct FillParams {
     long long t;  // step index the fill belongs to (noise counter)
 };
 
-// geometry of the TMA-staged tile kernel (kernels_tile.cu)
-#define TILE_WY 4                       // warps per CTA, stacked along y; each warp owns 2 rows x 30 columns
-#define TILE_BX 32                      // lanes per warp row: 30 output columns + 1 halo column on each side
-#define TILE_BY (2 * TILE_WY + 2)       // TMA box height (8 output rows + 1 halo row on each side)
-#define TILE_NS 4                       // planes in the shared-memory ring
+// geometry of the TMA-staged tile kernel (kernels_tile.cu): a warp owns 2 rows x 30 columns (+ 1 halo lane per side)
 #define TILE_COLS 30
+#define TILE_MAX_BY 14                  // tallest TMA box of any instantiation (rows): the padded layout is at least this high
 
 struct tslb_ctx {
     int nx, ny, nz, dtype;
@@ -67,7 +64,6 @@ struct tslb_ctx {
     size_t ws_bytes;
     void *buf[2];     // moment buffers, internal form (padded SoA, field 0 holds rho - 1)
     double *scratch;  // diagnostics partials
-    void *stage;      // staging area for the *_host calls (API layout)
     CUtensorMap tmap[2];  // TMA descriptors of buf[0], buf[1]
     int tmap_ok;
     int cur;          // buf[cur] holds time t
