@@ -418,22 +418,24 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
 #pragma unroll
                 for (int kx = 0; kx < 3; ++kx) {
                     if (!kvalid(kx, 0, kz)) continue;
-                    P Sq[3], Wq[3];
-#pragma unroll
-                    for (int ky = 0; ky < 3; ++ky)
-                        if (kvalid(kx, ky, kz)) {
-                            P h = Ah[kx][ky], cs = pk(Ac[kx][ky].y, Ac[kx][ky].x);
-                            if (any_ghost) {   // rows beyond a bounce-back wall send nothing (bounce_y_correction adds their part)
-                                if (ghost_lo) h.x = (T)0;
-                                if (ghost_hi) h.y = (T)0;
-                                if (ghost_mid) { cs.x = (T)0; h.y = (T)0; }
-                            }
-                            Sq[ky] = padd(h, cs);
-                            Wq[ky] = psub(h, cs);
-                        }
-                    if (kvalid(kx, 2, kz)) pass_group_y<3, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][2], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
-                    else if (kvalid(kx, 1, kz)) pass_group_y<2, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][0], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
-                    else pass_group_y<1, P, T>(Sq, Wq, Ac[kx][0], Ac[kx][0], sgn, G1[0][kx], G1[1][kx], G1[2][kx]);
+                    // E = up(P) + dn(M), O = up(P) - dn(M) with P = phi0 + phi1 + phi2, M = phi0 - phi1 + phi2 of the
+                    // neighbour rows.  Per pack Q = (P of its .x row, M of its .y row) = phi0 + phi2 + phi1 * sgn; then
+                    // E = Q_H + swap(Q_C) and O = (Q_H - swap(Q_C)) * sgn.
+                    P qh = Ah[kx][0], qc = Ac[kx][0];
+                    if (kvalid(kx, 2, kz)) { qh = padd(qh, Ah[kx][2]); qc = padd(qc, Ac[kx][2]); }
+                    if (kvalid(kx, 1, kz)) { qh = pfma(Ah[kx][1], sgn, qh); qc = pfma(Ac[kx][1], sgn, qc); }
+                    P qs = pk(qc.y, qc.x);
+                    if (any_ghost) {   // rows beyond a bounce-back wall send nothing (bounce_y_correction adds their part)
+                        if (ghost_lo) qh.x = (T)0;
+                        if (ghost_hi) qh.y = (T)0;
+                        if (ghost_mid) { qs.x = (T)0; qh.y = (T)0; }
+                    }
+                    const P E = padd(qh, qs);
+                    G1[2][kx] = E;
+                    G1[1][kx] = pmul(psub(qh, qs), sgn);
+                    P o0 = pfmas(Ac[kx][0], (T)4, E);
+                    if (kvalid(kx, 2, kz)) o0 = pfmas(Ac[kx][2], (T)-2, o0);
+                    G1[0][kx] = o0;
                 }
                 // y-stage increments of the bases 3 u_a (tap sums along y: 6, 0, 2 for py = 0, 1, 2 when ky = 0; 0, 2, 0 when ky = 1)
                 const P sg3 = pk((T)3, (T)-3);
@@ -447,18 +449,17 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
                 // ---- x pass (warp shuffles): G2[px][py] = sum_kx T^x_{px,kx} G1[py][kx]; then the z bookkeeping ----
 #pragma unroll
                 for (int py = 0; py < 3; ++py) {
-                    P Sq[3], Dq[3];
-#pragma unroll
-                    for (int kx = 0; kx < 3; ++kx)
-                        if (kvalid(kx, 0, kz)) {
-                            const P up = shfl_up1(G1[py][kx]);  // value at column-1  (c_x = +1 pulls from x-1)
-                            const P dn = shfl_dn1(G1[py][kx]);  // value at column+1
-                            Sq[kx] = padd(up, dn);
-                            Dq[kx] = psub(up, dn);
-                        }
+                    // E = up(P) + dn(M), O = up(P) - dn(M): one shuffle up of P = phi0 + phi1 + phi2 and one down of
+                    // M = phi0 - phi1 + phi2 instead of two per field
+                    P t = G1[py][0];
+                    if (kvalid(2, 0, kz)) t = padd(t, G1[py][2]);
+                    const P upP = shfl_up1(padd(t, G1[py][1]));   // from column-1  (c_x = +1 pulls from x-1)
+                    const P dnM = shfl_dn1(psub(t, G1[py][1]));   // from column+1
                     P o[3];
-                    if (kvalid(2, 0, kz)) pass_group<3, P, T>(Sq, Dq, G1[py][0], G1[py][2], o[0], o[1], o[2]);
-                    else pass_group<2, P, T>(Sq, Dq, G1[py][0], G1[py][0], o[0], o[1], o[2]);
+                    o[2] = padd(upP, dnM);
+                    o[1] = psub(upP, dnM);
+                    o[0] = pfmas(G1[py][0], (T)4, o[2]);
+                    if (kvalid(2, 0, kz)) o[0] = pfmas(G1[py][2], (T)-2, o[0]);
                     // x-stage increments: base multipliers after the y stage are 18 (py=0) and 6 (py=2) for ux (kx=1) and uz
                     // (kx=0, kz=1), 6 (py=1) for uy (kx=0)
                     if (kz == 0 && py == 0) { o[0] = pfmas(Dx[0], (T)18, o[0]); o[1] = pfmas(Lx[0], (T)18, o[1]); o[2] = pfmas(Dx[0], (T)18, o[2]); }
