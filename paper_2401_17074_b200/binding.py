@@ -46,7 +46,7 @@ def load_library(path: Optional[str] = None):
     global _lib
     if _lib is not None and path is None:
         return _lib
-    path = path or LIB_PATH
+    path = path or os.environ.get("TSLB_LIBRARY") or LIB_PATH     # TSLB_LIBRARY: use another build of the same library
     if not os.path.exists(path):
         raise FileNotFoundError(
             "%s is missing: build it with `python -m paper_2401_17074_b200.build` (no CPU fallback exists)" % path)

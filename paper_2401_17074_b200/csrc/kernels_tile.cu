@@ -282,7 +282,13 @@ __host__ __device__ constexpr int gidx(int px, int py) { return py == 0 ? px : (
 // multiple of 2 floats raises "illegal instruction"): the box starts at the CTA's first column rounded down to ALIGN
 // elements and lanes read at the remaining offset (0 for WX = 2).
 template <typename T> struct TileGeom;
-template <> struct TileGeom<float> { static constexpr int WX = 2, WY = 6, NS = 4, ALIGN = 4; };
+#ifndef TILE_F32_WY
+#define TILE_F32_WY 7
+#endif
+#ifndef TILE_F32_NS
+#define TILE_F32_NS 4
+#endif
+template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, ALIGN = 4; };
 template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 4, ALIGN = 2; };
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;

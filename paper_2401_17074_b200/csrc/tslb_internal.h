@@ -50,7 +50,7 @@ struct FillParams {
 
 // geometry of the TMA-staged tile kernel (kernels_tile.cu): a warp owns 2 rows x 30 columns (+ 1 halo lane per side)
 #define TILE_COLS 30
-#define TILE_MAX_BY 14                  // tallest TMA box of any instantiation (rows): the padded layout is at least this high
+#define TILE_MAX_BY 18                  // tallest TMA box of any instantiation (rows): the padded layout is at least this high
 
 struct tslb_ctx {
     int nx, ny, nz, dtype;
