@@ -127,6 +127,14 @@ int tslb_get_moments_host(tslb_ctx *ctx, void *host_dst, void *stream);
  * pass (bitwise reproducible).  dev_out5: 5 doubles in device memory. */
 int tslb_diagnostics(tslb_ctx *ctx, double *dev_out5, void *stream);
 
+/* Per-kernel timing of the sweep launches (bench.py's roofline figure).  tslb_set_timing(ctx, m) with m > 0 makes
+ * tslb_step bracket each of its next m sweep-kernel launches with a CUDA event pair recorded on the launching stream
+ * (m = 0 switches it off and frees the events).  tslb_get_timing waits for the recorded launches, returns how many
+ * there were and the sum of their durations in milliseconds, and resets the count.  The events sit between launches
+ * of the same stream, so they add no synchronisation; leave timing off inside a throughput measurement. */
+int tslb_set_timing(tslb_ctx *ctx, int max_launches);
+int tslb_get_timing(tslb_ctx *ctx, int *n_launches, double *total_ms);
+
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);
 /* Number of kernels this context has launched so far (all kinds), for bench.py's gpu_launches. */

@@ -24,7 +24,7 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile
 SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
-           "tslb_launch_count", "tslb_last_error", "tslb_version")
+           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing")
 
 
 class InletParams(C.Structure):
@@ -67,6 +67,8 @@ def load_library(path: Optional[str] = None):
     lib.tslb_get_moments.argtypes = [vp, vp, vp]
     lib.tslb_get_moments_host.argtypes = [vp, vp, vp]
     lib.tslb_diagnostics.argtypes = [vp, vp, vp]
+    lib.tslb_set_timing.argtypes = [vp, ip]
+    lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
     lib.tslb_step_count.restype = C.c_longlong
     lib.tslb_launch_count.argtypes = [vp]
@@ -204,6 +206,15 @@ class TSLB:
         out = torch.empty(5, dtype=torch.float64, device="cuda")
         self._chk(self._lib.tslb_diagnostics(self._h, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "tslb_diagnostics")
         return out
+
+    def set_timing(self, max_launches: int):
+        self._chk(self._lib.tslb_set_timing(self._h, int(max_launches)), "tslb_set_timing")
+
+    def get_timing(self):
+        """(number of timed sweep launches, sum of their durations in ms) since the last call."""
+        n, ms = C.c_int(0), C.c_double(0.0)
+        self._chk(self._lib.tslb_get_timing(self._h, C.byref(n), C.byref(ms)), "tslb_get_timing")
+        return n.value, ms.value
 
     @property
     def step_count(self) -> int:

@@ -238,10 +238,37 @@ __device__ __noinline__ void bounce_y_correction(const T *__restrict__ Abuf, lon
     out[9] += sg * (T)-12 * Bm[0][1];
 }
 
+// Periodic ghost images of the two rows of a pack (rare path).  eflags: bit 0 = column on a periodic x face,
+// bits 1/2 = row r0 / r0+1 on a periodic y face, bit 3 = plane on a periodic z face.
+template <typename P, typename T>
+__device__ __forceinline__ void store_images(const P (&o)[TSLB_NF], T *__restrict__ Bbuf, long long N, long long i0, long long i1, bool row1,
+                                          int eflags, const Layout &L, int col, int r0, int zt)
+{
+    const long long xi = col == 0 ? (long long)L.nx : -(long long)L.nx;
+    const long long zi = zt == 0 ? (long long)L.nz * L.plane : -(long long)L.nz * L.plane;
+    const long long ywrap = (long long)L.ny * L.px;
+    const long long yi0 = r0 == 0 ? ywrap : -ywrap, yi1 = -ywrap;
+    const bool ex = eflags & 1, ey0 = eflags & 2, ey1 = (eflags & 4) && row1, ez = eflags & 8;
+    T *b0 = Bbuf + i0, *b1 = Bbuf + i1;
+#define TSLB_PUT0(off) _Pragma("unroll") for (int f = 0; f < TSLB_NF; ++f) b0[f * N + (off)] = o[f].x;
+#define TSLB_PUT1(off) _Pragma("unroll") for (int f = 0; f < TSLB_NF; ++f) b1[f * N + (off)] = o[f].y;
+    if (ex) { TSLB_PUT0(xi) if (row1) { TSLB_PUT1(xi) } }
+    if (ey0) { TSLB_PUT0(yi0) if (ex) { TSLB_PUT0(yi0 + xi) } }
+    if (ey1) { TSLB_PUT1(yi1) if (ex) { TSLB_PUT1(yi1 + xi) } }
+    if (ez) {
+        TSLB_PUT0(zi) if (row1) { TSLB_PUT1(zi) }
+        if (ex) { TSLB_PUT0(zi + xi) if (row1) { TSLB_PUT1(zi + xi) } }
+        if (ey0) { TSLB_PUT0(zi + yi0) if (ex) { TSLB_PUT0(zi + yi0 + xi) } }
+        if (ey1) { TSLB_PUT1(zi + yi1) if (ex) { TSLB_PUT1(zi + yi1 + xi) } }
+    }
+#undef TSLB_PUT0
+#undef TSLB_PUT1
+}
+
 // finalise the two rows of a pack from their 216-scaled raw moments (m[1..3] lack their base 216 u) and store (Eq. 12)
 template <typename P, typename T>
 __device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&uo)[3], T *__restrict__ Bbuf, long long N, long long i0,
-                                               long long i1, bool row1)
+                                               long long i1, bool row1, int eflags, const Layout &L, int col, int r0, int zt)
 {
     // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
     const T hi = (T)(1.0 / 216.0);
@@ -271,6 +298,9 @@ __device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&
 #pragma unroll
         for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i1] = o[f].y;
     }
+    // periodic images: a node on a periodic face is also the ghost cell beyond the opposite face (and the edge /
+    // corner ghosts when it lies on several), so the next sweep needs no separate ghost-layer refresh
+    if (eflags) store_images<P, T>(o, Bbuf, N, i0, i1, row1, eflags, L, col, r0, zt);
 }
 
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
@@ -367,6 +397,10 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
 #pragma unroll
     for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
 
+    // which of this thread's nodes have periodic ghost images (finalize_store)
+    const int eflags_xy = ((p.kind[0] == TSLB_BC_PERIODIC && (col == 0 || col == L.nx - 1)) ? 1 : 0) |
+                          ((p.kind[2] == TSLB_BC_PERIODIC && (r0 == 0 || r0 == L.ny - 1)) ? 2 : 0) |
+                          ((p.kind[2] == TSLB_BC_PERIODIC && r0 + 1 == L.ny - 1) ? 4 : 0);
     const P sgn = pk((T)1, (T)-1);                        // D = W * sgn for the (centre, halo) row packing, see below
     const bool st_ok = col_out && warp_active;
     for (int i = 0; i < nplanes; ++i) {
@@ -528,7 +562,8 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
                         for (int f = 0; f < TSLB_NF; ++f) m[f].y += corr[f];
                     }
                 }
-                finalize_store<P, T>(m, uprev, Bbuf, N, i0, i0 + L.px, row1_valid);
+                const int eflags = eflags_xy | ((p.kind[4] == TSLB_BC_PERIODIC && (zt == 0 || zt == L.nz - 1)) ? 8 : 0);
+                finalize_store<P, T>(m, uprev, Bbuf, N, i0, i0 + L.px, row1_valid, eflags, L, col, r0, zt);
             }
             // ---- shift the march state ---------------------------------------------------------------------------------
 #pragma unroll

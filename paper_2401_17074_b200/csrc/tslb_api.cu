@@ -57,16 +57,30 @@ int check_boundary_set(tslb_ctx *c)
     return TSLB_OK;
 }
 
-// Boundary nodes of the open faces filled at time t (oracle step 1) and, for the tile kernel, the ghost layers
-// refreshed from the filled state.  Idempotent for a given (buffer, t): skipped when already done.
+bool any_open(const tslb_ctx *c)
+{
+    for (int f = 0; f < 6; ++f)
+        if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT) return true;
+    return false;
+}
+bool any_periodic(const tslb_ctx *c) { return c->kind[0] == TSLB_BC_PERIODIC || c->kind[2] == TSLB_BC_PERIODIC || c->kind[4] == TSLB_BC_PERIODIC; }
+
+// Boundary nodes of the open faces filled at time t (oracle step 1) and, for the tile kernel, valid ghost layers.
+// halo_valid: 0 = nothing done for (buf[cur], t); 1 = boundary nodes filled; 2 = ghost layers valid as well.
+// The tile kernel writes the periodic ghost images of every node it stores, so after a tile step the ghost layers of
+// the new buffer are already valid -- unless open faces exist next to a periodic axis (the fill changes boundary
+// nodes whose images then have to be refreshed).  Ghost cells beyond walls and open faces are never used by a node
+// that is advanced; they only have to be finite (the workspace is zeroed at bind time).
 cudaError_t refresh_boundary(tslb_ctx *c, bool need_halo, cudaStream_t st)
 {
-    if (c->halo_valid >= (need_halo ? 2 : 1)) return cudaSuccess;
     cudaError_t e = cudaSuccess;
-    if (c->halo_valid < 1) e = tslb_launch_fill(c, c->buf[c->cur], st);
-    if (e != cudaSuccess) return e;
-    c->halo_valid = 1;
-    if (need_halo) {
+    const bool refill = any_open(c) && any_periodic(c);
+    if (c->halo_valid < 1 || (c->halo_valid == 3)) {
+        e = tslb_launch_fill(c, c->buf[c->cur], st);
+        if (e != cudaSuccess) return e;
+        c->halo_valid = (c->halo_valid == 3 && !refill) ? 2 : 1;
+    }
+    if (need_halo && c->halo_valid < 2) {
         e = tslb_launch_halo(c, c->buf[c->cur], st);
         if (e != cudaSuccess) return e;
         c->halo_valid = 2;
@@ -104,7 +118,47 @@ int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out)
     return TSLB_OK;
 }
 
-void tslb_destroy(tslb_ctx *c) { free(c); }
+void tslb_destroy(tslb_ctx *c)
+{
+    if (!c) return;
+    for (int i = 0; i < 2 * c->ev_cap; ++i) cudaEventDestroy(c->ev[i]);
+    free(c->ev);
+    free(c);
+}
+
+int tslb_set_timing(tslb_ctx *c, int max_launches)
+{
+    if (!c) return TSLB_EINVAL;
+    if (max_launches < 0 || max_launches > 100000) return fail(c, TSLB_EINVAL, "max_launches out of range");
+    for (int i = 0; i < 2 * c->ev_cap; ++i) cudaEventDestroy(c->ev[i]);
+    free(c->ev);
+    c->ev = nullptr; c->ev_cap = 0; c->ev_n = 0; c->timing = 0;
+    if (max_launches == 0) return TSLB_OK;
+    c->ev = (cudaEvent_t *)calloc(2 * (size_t)max_launches, sizeof(cudaEvent_t));
+    if (!c->ev) return fail(c, TSLB_ENOMEM, "host allocation failed");
+    for (int i = 0; i < 2 * max_launches; ++i) {
+        cudaError_t e = cudaEventCreate(&c->ev[i]);
+        if (e != cudaSuccess) return cuda_fail(c, "cudaEventCreate", e);
+    }
+    c->ev_cap = max_launches; c->timing = 1;
+    return TSLB_OK;
+}
+
+int tslb_get_timing(tslb_ctx *c, int *n_launches, double *total_ms)
+{
+    if (!c || !n_launches || !total_ms) return TSLB_EINVAL;
+    double tot = 0;
+    for (int i = 0; i < c->ev_n; ++i) {
+        float ms = 0;
+        cudaError_t e = cudaEventSynchronize(c->ev[2 * i + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, c->ev[2 * i], c->ev[2 * i + 1]);
+        if (e != cudaSuccess) return cuda_fail(c, "cudaEventElapsedTime", e);
+        tot += ms;
+    }
+    *n_launches = c->ev_n; *total_ms = tot;
+    c->ev_n = 0;
+    return TSLB_OK;
+}
 
 size_t tslb_workspace_bytes(const tslb_ctx *c)
 {
@@ -226,11 +280,14 @@ int tslb_step(tslb_ctx *c, int n, void *stream)
     for (int s = 0; s < n; ++s) {
         cudaError_t e = refresh_boundary(c, k == TSLB_KERNEL_TILE, st);    // step 1: boundary nodes (+ ghost layers) at time t
         if (e != cudaSuccess) return cuda_fail(c, "fill/halo kernel", e);
+        const bool timed = c->timing && c->ev_n < c->ev_cap;
+        if (timed) cudaEventRecord(c->ev[2 * c->ev_n], st);
         e = (k == TSLB_KERNEL_TILE) ? tslb_launch_tile(c, st) : tslb_launch_gather(c, st);  // steps 2-4
+        if (timed) cudaEventRecord(c->ev[2 * c->ev_n++ + 1], st);
         if (e != cudaSuccess) return cuda_fail(c, "sweep kernel", e);
         c->cur = 1 - c->cur;                                               // step 5: AB flip-flop
         c->t += 1;
-        c->halo_valid = 0;
+        c->halo_valid = (k == TSLB_KERNEL_TILE) ? 3 : 0;   // 3: periodic ghost images written by the sweep, fill pending
     }
     return TSLB_OK;
 }

@@ -73,6 +73,10 @@ struct tslb_ctx {
     int kernel_req;   // TSLB_KERNEL_*
     int sm_count;
     long long launches;
+    // optional per-kernel timing of the sweep launches (tslb_set_timing): event pairs on the launching stream
+    int timing;
+    cudaEvent_t *ev;      // 2 * ev_cap events
+    int ev_cap, ev_n;
     char err[256];
 };
 
