@@ -173,6 +173,53 @@ def test_full_size_sampled_subboxes(B, oracle_mod, n, dtype):
     sim.close()
 
 
+def test_config2_full_size_20_steps(B, oracle_mod):
+    """configs[2] at its full 384 x 128 x 192 in the launch configuration of the tile kernel: 20 steps element by
+    element against the oracle (the full 2000 steps run on the reduced cross-section above), mass conserved."""
+    w = W.channel(steps=20)
+    G, R, curve = run_both(oracle_mod, w, 20, B.KERNEL_AUTO, checkpoints=[1])
+    print("channel full size curve: %s" % curve)
+    assert_parity(w, G, R, "full-size channel")
+    assert abs(G[0].sum(dtype=np.float64) / w.sites - 1) < 1e-7
+
+
+def test_config3_full_size_10_steps(B, oracle_mod):
+    """configs[3] at its full 256 x 256 x 768: 10 steps element by element (inlet noise, outlets, fill kernel)."""
+    w = W.jet(steps=10)
+    G, R, curve = run_both(oracle_mod, w, 10, B.KERNEL_AUTO, checkpoints=[1])
+    print("jet full size curve: %s" % curve)
+    assert_parity(w, G, R, "full-size jet")
+    assert 0.9 < G[0].min() and G[0].max() < 1.15
+
+
+def test_kernel_switch_keeps_ghost_layers_valid(B, oracle_mod):
+    """tile -> gather -> tile: the gather kernel does not maintain the ghost layers, the next tile step must refresh them."""
+    for w in (W.config1(n=40, steps=9), with_faces(W.random_state(70, 20, 9, seed=3, dtype="f64", tau=0.6),
+                                                     {W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, g=(1e-4, 0, 0))):
+        o = make_oracle(oracle_mod, w); sim = make_gpu(w, TILE)
+        for k, n in ((TILE, 3), (GATHER, 2), (TILE, 3), (GATHER, 1)):
+            sim.set_kernel(k); sim.step(n); o.step(n)
+        assert_parity(w, gpu_state(sim), o.get_moments(), "kernel switching")
+        sim.close()
+
+
+def test_set_moments_mid_run_and_timing_api(B, oracle_mod):
+    """set_moments invalidates the ghost layers; tslb_set_timing / tslb_get_timing count the sweep launches."""
+    import torch
+    w = W.config1(n=36, steps=4)
+    sim = make_gpu(w, B.KERNEL_AUTO)
+    sim.step(3)
+    sim.set_moments(torch.from_numpy(np.ascontiguousarray(w.moments)).to("cuda"))
+    sim.set_timing(8)
+    sim.step(4)
+    n, ms = sim.get_timing()
+    assert n == 4 and ms > 0.0
+    assert sim.get_timing() == (0, 0.0)
+    sim.set_timing(0)
+    o = make_oracle(oracle_mod, w); o.step(4)
+    assert_parity(w, gpu_state(sim), o.get_moments(), "after set_moments mid-run")
+
+
 # ---------------------------------------------------------------------------------------------
 # library behaviour on the device
 # ---------------------------------------------------------------------------------------------
