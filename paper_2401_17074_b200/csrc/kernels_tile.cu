@@ -389,11 +389,13 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
         for (int i = 0; i < TILE_NS && i < nplanes; ++i) issue(i);
 
     // z-march state per (px,py) group: Vp of plane zs-2, centre term of plane zs-1, Vp of plane zs-1
-    P vp2[6], cc1[6], vp1[6];
+    // (kept as T1 = Vp(zs-2) + centre(zs-1), Vp(zs-2) where it is needed alone -- groups 0, 1, 3 -- and Vp(zs-1):
+    //  15 instead of 18 running pairs, 9 instead of 18 register moves per plane)
+    P vp2[6], tt1[6], vp1[6];
     // increment form along z: velocity of the previous plane and its backward difference, rows r0, r0+1
     P uprev[3], dprev[3];
 #pragma unroll
-    for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); cc1[i] = vp2[i]; vp1[i] = vp2[i]; }
+    for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); tt1[i] = vp2[i]; vp1[i] = vp2[i]; }
 #pragma unroll
     for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
 
@@ -525,19 +527,16 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
             if (zt >= z0 && st_ok) {
                 P m[TSLB_NF];
                 {
-                    const P e00 = padd(vp2[0], vm0[0]);
-                    m[0] = pfmas(Dz[2], (T)108, padd(e00, cc1[0]));            // 000
+                    m[0] = pfmas(Dz[2], (T)108, padd(tt1[0], vm0[0]));          // 000
                     m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));         // 001
-                    m[6] = pfmas(Dz[2], (T)108, e00);                          // 002
-                    const P e10 = padd(vp2[1], vm0[1]);
-                    m[1] = pfmas(Lz[0], (T)36, padd(e10, cc1[1]));             // 100
+                    m[6] = pfmas(Dz[2], (T)108, padd(vp2[0], vm0[0]));         // 002
+                    m[1] = pfmas(Lz[0], (T)36, padd(tt1[1], vm0[1]));           // 100
                     m[8] = pfmas(Dz[0], (T)36, psub(vp2[1], vm0[1]));          // 101
-                    const P e01 = padd(vp2[3], vm0[3]);
-                    m[2] = pfmas(Lz[1], (T)36, padd(e01, cc1[3]));             // 010
+                    m[2] = pfmas(Lz[1], (T)36, padd(tt1[3], vm0[3]));           // 010
                     m[9] = pfmas(Dz[1], (T)36, psub(vp2[3], vm0[3]));          // 011
-                    m[4] = pfmas(Dz[2], (T)36, padd(padd(vp2[2], vm0[2]), cc1[2]));   // 200
-                    m[7] = padd(padd(vp2[4], vm0[4]), cc1[4]);                 // 110
-                    m[5] = pfmas(Dz[2], (T)36, padd(padd(vp2[5], vm0[5]), cc1[5]));   // 020
+                    m[4] = pfmas(Dz[2], (T)36, padd(tt1[2], vm0[2]));           // 200
+                    m[7] = padd(tt1[4], vm0[4]);                               // 110
+                    m[5] = pfmas(Dz[2], (T)36, padd(tt1[5], vm0[5]));           // 020
                 }
                 const long long i0 = lay_idx(L, col, r0, zt);
                 if (WALLY) {   // warp-uniform: only the warps that own a wall row
@@ -567,7 +566,11 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
             }
             // ---- shift the march state ---------------------------------------------------------------------------------
 #pragma unroll
-            for (int g = 0; g < 6; ++g) { vp2[g] = vp1[g]; vp1[g] = vp0[g]; cc1[g] = cc0[g]; }
+            for (int g = 0; g < 6; ++g) {
+                tt1[g] = padd(vp1[g], cc0[g]);               // Vp(zs-1) + centre(zs): used when plane zs+1 arrives
+                if (g == 0 || g == 1 || g == 3) vp2[g] = vp1[g];
+                vp1[g] = vp0[g];
+            }
 #pragma unroll
             for (int a = 0; a < 3; ++a) uprev[a] = rc[1 + a];
         }
