@@ -286,12 +286,13 @@ __device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&
     const P niso = pmuls(dR, (T)(-1.0 / 3.0));
     const P nrho = pmuls(rho, (T)-1);
     const P rx = pmul(nrho, o[1]), ry = pmul(nrho, o[2]), rz = pmul(nrho, o[3]);
-    o[4] = pfma(rx, o[1], padd(pfmas(m[4], lo, pmuls(m[4], hi)), niso));
-    o[5] = pfma(ry, o[2], padd(pfmas(m[5], lo, pmuls(m[5], hi)), niso));
-    o[6] = pfma(rz, o[3], padd(pfmas(m[6], lo, pmuls(m[6], hi)), niso));
-    o[7] = pfma(rx, o[2], pfmas(m[7], lo, pmuls(m[7], hi)));
-    o[8] = pfma(rx, o[3], pfmas(m[8], lo, pmuls(m[8], hi)));
-    o[9] = pfma(ry, o[3], pfmas(m[9], lo, pmuls(m[9], hi)));
+    // (the second moments are rebuilt from scratch every step, so a singly rounded 1/216 cannot compound there)
+    o[4] = pfma(rx, o[1], pfmas(m[4], hi, niso));
+    o[5] = pfma(ry, o[2], pfmas(m[5], hi, niso));
+    o[6] = pfma(rz, o[3], pfmas(m[6], hi, niso));
+    o[7] = pfma(rx, o[2], pmuls(m[7], hi));
+    o[8] = pfma(rx, o[3], pmuls(m[8], hi));
+    o[9] = pfma(ry, o[3], pmuls(m[9], hi));
 #pragma unroll
     for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i0] = o[f].x;
     if (row1) {
@@ -318,8 +319,14 @@ template <typename T> struct TileGeom;
 #ifndef TILE_F32_NS
 #define TILE_F32_NS 4
 #endif
-template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, ALIGN = 4; };
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 4, ALIGN = 2; };
+#ifndef TILE_F32_WX
+#define TILE_F32_WX 2
+#endif
+#ifndef TILE_F32_MINB
+#define TILE_F32_MINB 1
+#endif
+template <> struct TileGeom<float> { static constexpr int WX = TILE_F32_WX, WY = TILE_F32_WY, NS = TILE_F32_NS, ALIGN = 4, MINB = TILE_F32_MINB; };
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 4, ALIGN = 2, MINB = 1; };
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;
     static constexpr int WARPS = G::WX * G::WY;
@@ -335,7 +342,7 @@ template <typename T> struct TileDims {
 static_assert(TileDims<float>::BY <= TILE_MAX_BY && TileDims<double>::BY <= TILE_MAX_BY, "layout height");
 
 template <typename T, bool WALLY>
-__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
+__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
                                                                    T *__restrict__ Bbuf, TileParams<T> p)
 {
     typedef typename PackOf<T>::type P;
@@ -443,7 +450,7 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
                 Dx[a] = psub(xl, xr);
                 const P dcur = psub(uc, uprev[a]);           // u(zs) - u(zs-1)
                 Lz[a] = psub(dcur, dprev[a]);                // at the target plane zs-1
-                Dz[a] = psub(pmuls(dprev[a], (T)-1), dcur);  // u(zs-2) - u(zs)
+                Dz[a] = padd(dprev[a], dcur);                // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
                 dprev[a] = dcur;
             }
 
@@ -527,16 +534,16 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, 1) sweep_tile_kernel(
             if (zt >= z0 && st_ok) {
                 P m[TSLB_NF];
                 {
-                    m[0] = pfmas(Dz[2], (T)108, padd(tt1[0], vm0[0]));          // 000
+                    m[0] = pfmas(Dz[2], (T)-108, padd(tt1[0], vm0[0]));          // 000
                     m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));         // 001
-                    m[6] = pfmas(Dz[2], (T)108, padd(vp2[0], vm0[0]));         // 002
+                    m[6] = pfmas(Dz[2], (T)-108, padd(vp2[0], vm0[0]));         // 002
                     m[1] = pfmas(Lz[0], (T)36, padd(tt1[1], vm0[1]));           // 100
-                    m[8] = pfmas(Dz[0], (T)36, psub(vp2[1], vm0[1]));          // 101
+                    m[8] = pfmas(Dz[0], (T)-36, psub(vp2[1], vm0[1]));          // 101
                     m[2] = pfmas(Lz[1], (T)36, padd(tt1[3], vm0[3]));           // 010
-                    m[9] = pfmas(Dz[1], (T)36, psub(vp2[3], vm0[3]));          // 011
-                    m[4] = pfmas(Dz[2], (T)36, padd(tt1[2], vm0[2]));           // 200
+                    m[9] = pfmas(Dz[1], (T)-36, psub(vp2[3], vm0[3]));          // 011
+                    m[4] = pfmas(Dz[2], (T)-36, padd(tt1[2], vm0[2]));           // 200
                     m[7] = padd(tt1[4], vm0[4]);                               // 110
-                    m[5] = pfmas(Dz[2], (T)36, padd(tt1[5], vm0[5]));           // 020
+                    m[5] = pfmas(Dz[2], (T)-36, padd(tt1[5], vm0[5]));           // 020
                 }
                 const long long i0 = lay_idx(L, col, r0, zt);
                 if (WALLY) {   // warp-uniform: only the warps that own a wall row
@@ -598,7 +605,8 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
         const int zc = (c->nz + k - 1) / k;
         if (k > 1 && zc < 8) break;
         const long long ctas = cols * ((c->nz + zc - 1) / zc);
-        const long long waves = (ctas + c->sm_count - 1) / c->sm_count;
+        const long long slots = (long long)c->sm_count * TileGeom<T>::MINB;
+        const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
         if (cost < best_cost) { best_cost = cost; best = k; }
     }
