@@ -185,59 +185,6 @@ __device__ __forceinline__ void pass_group_y(const P (&S)[3], const P (&W)[3], P
     if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
 }
 
-// Contribution of the bounced directions at a node next to a halfway bounce-back wall on a y face
-// (DESIGN.md "Walls in the separable form"): f_i(x,t+1) = f*_ibar(x,t) for the 9 directions with c_y = sgn_in,
-// evaluated from the node's own 216-scaled Hermite coefficients (FULL first-order coefficients here: the increment
-// form treats the missing ghost row as u = 0, so the whole bounced population is a correction).  Adds to out[10]
-// (216-scaled raw moments in the order 000,100,010,001,200,020,002,110,101,011).  lo_wall: wall below (arrival
-// c_y = +1), else above.
-template <typename T>
-__device__ __noinline__ void bounce_y_correction(const T *__restrict__ Abuf, long long N, long long idx, T beta, const T (&g)[3],
-                                                 bool lo_wall, T (&out)[TSLB_NF])
-{
-    T raw[TSLB_NF];
-#pragma unroll
-    for (int f = 0; f < TSLB_NF; ++f) raw[f] = __ldg(Abuf + f * N + idx);
-    const T rho = (T)1 + raw[0], ux = raw[1], uy = raw[2], uz = raw[3];
-    const T u[3] = {ux, uy, uz};
-    const T Pm[3][3] = {{raw[4], raw[7], raw[8]}, {raw[7], raw[5], raw[9]}, {raw[8], raw[9], raw[6]}};
-    T a2[3][3];
-    for (int a = 0; a < 3; ++a)
-        for (int b = 0; b < 3; ++b) a2[a][b] = rho * u[a] * u[b] + beta * Pm[a][b];
-    // A(kx,ky,kz), scaled as in hermite_round
-    T A[3][3][3];
-    for (int i = 0; i < 27; ++i) (&A[0][0][0])[i] = (T)0;
-    A[0][0][0] = raw[0];
-    A[1][0][0] = (T)3 * rho * (ux + g[0]); A[0][1][0] = (T)3 * rho * (uy + g[1]); A[0][0][1] = (T)3 * rho * (uz + g[2]);
-    A[2][0][0] = (T)3 * a2[0][0]; A[0][2][0] = (T)3 * a2[1][1]; A[0][0][2] = (T)3 * a2[2][2];
-    A[1][1][0] = (T)9 * a2[0][1]; A[1][0][1] = (T)9 * a2[0][2]; A[0][1][1] = (T)9 * a2[1][2];
-    // a3_aab = a2_aa u_b + 2 u_a beta P_ab
-    A[2][1][0] = (T)9 * (a2[0][0] * uy + (T)2 * ux * beta * Pm[0][1]);
-    A[2][0][1] = (T)9 * (a2[0][0] * uz + (T)2 * ux * beta * Pm[0][2]);
-    A[1][2][0] = (T)9 * (a2[1][1] * ux + (T)2 * uy * beta * Pm[0][1]);
-    A[0][2][1] = (T)9 * (a2[1][1] * uz + (T)2 * uy * beta * Pm[1][2]);
-    A[1][0][2] = (T)9 * (a2[2][2] * ux + (T)2 * uz * beta * Pm[0][2]);
-    A[0][1][2] = (T)9 * (a2[2][2] * uy + (T)2 * uz * beta * Pm[1][2]);
-    A[1][1][1] = (T)27 * (a2[0][1] * uz + beta * (Pm[0][2] * uy + Pm[1][2] * ux));
-    // B(kx,kz) = sum_ky s^ky A(kx,ky,kz), s = t_ky(-c_y): wall below -> t(-1) = (1,-1,1); above -> t(+1) = (1,1,1)
-    const T s1 = lo_wall ? (T)-1 : (T)1;
-    T Bm[3][3];
-    for (int kx = 0; kx < 3; ++kx)
-        for (int kz = 0; kz < 3; ++kz) Bm[kx][kz] = A[kx][0][kz] + s1 * A[kx][1][kz] + A[kx][2][kz];
-    const T sg = lo_wall ? (T)1 : (T)-1;  // c_y^py of the arrival direction
-    // local sums L(p,q) = sum_c c^p t_q(-c): L(0,0)=6, L(1,1)=-2, L(2,0)=2, L(2,2)=2, others 0
-    out[0] += (T)36 * Bm[0][0];
-    out[1] += (T)-12 * Bm[1][0];
-    out[2] += sg * (T)36 * Bm[0][0];
-    out[3] += (T)-12 * Bm[0][1];
-    out[4] += (T)12 * (Bm[0][0] + Bm[2][0]);
-    out[5] += (T)36 * Bm[0][0];
-    out[6] += (T)12 * (Bm[0][0] + Bm[0][2]);
-    out[7] += sg * (T)-12 * Bm[1][0];
-    out[8] += (T)4 * Bm[1][1];
-    out[9] += sg * (T)-12 * Bm[0][1];
-}
-
 // Periodic ghost images of the two rows of a pack (rare path).  eflags: bit 0 = column on a periodic x face,
 // bits 1/2 = row r0 / r0+1 on a periodic y face, bit 3 = plane on a periodic z face.
 template <typename P, typename T>
@@ -342,7 +289,7 @@ template <typename T> struct TileDims {
 static_assert(TileDims<float>::BY <= TILE_MAX_BY && TileDims<double>::BY <= TILE_MAX_BY, "layout height");
 
 template <typename T, bool WALLY>
-__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA, const T *__restrict__ Abuf,
+__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA,
                                                                    T *__restrict__ Bbuf, TileParams<T> p)
 {
     typedef typename PackOf<T>::type P;
@@ -373,7 +320,11 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
     const bool ghost_lo = WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && r0 == 0;                 // row r0-1
     const bool ghost_mid = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 1 == L.ny;         // rows r0+1, r0+2
     const bool ghost_hi = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 2 == L.ny;          // row r0+2
-    const bool any_ghost = ghost_lo || ghost_mid || ghost_hi;
+    const bool any_ghost = ghost_lo || ghost_mid || ghost_hi;   // warp-uniform: this warp owns a wall-adjacent row
+    // multiplicative masks of the rows beyond a wall (no selects in the marching loop): mh for the halo pack (r0-1, r0+2),
+    // ms for the swapped centre pack (r0+1, r0)
+    const P mh = pk(ghost_lo ? (T)0 : (T)1, (ghost_hi || ghost_mid) ? (T)0 : (T)1);
+    const P ms = pk(ghost_mid ? (T)0 : (T)1, (T)1);
 
     const int z0 = blockIdx.z * p.zchunk;
     const int z1 = min(z0 + p.zchunk, L.nz);
@@ -401,6 +352,9 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
     P vp2[6], tt1[6], vp1[6];
     // increment form along z: velocity of the previous plane and its backward difference, rows r0, r0+1
     P uprev[3], dprev[3];
+    P kw[4];                                              // carried bounce-back terms of the moments with c_z (walls only)
+#pragma unroll
+    for (int k = 0; k < 4; ++k) kw[k] = pbc<P, T>((T)0);
 #pragma unroll
     for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); tt1[i] = vp2[i]; vp1[i] = vp2[i]; }
 #pragma unroll
@@ -437,11 +391,7 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
             for (int a = 0; a < 3; ++a) {
                 const P uc = rc[1 + a];
                 P hs = rh[1 + a], cs = pk(uc.y, uc.x);
-                if (any_ghost) {   // a node beyond a wall enters the differences as u = 0
-                    if (ghost_lo) hs.x = (T)0;
-                    if (ghost_hi) hs.y = (T)0;
-                    if (ghost_mid) { cs.x = (T)0; hs.y = (T)0; }
-                }
+                if (WALLY) { hs = pmul(hs, mh); cs = pmul(cs, ms); }   // a node beyond a wall enters the differences as u = 0
                 Ly[a] = pfmas(uc, (T)-2, padd(hs, cs));      // (up - c) + (dn - c)
                 Wy[a] = psub(hs, cs);                        // (up - dn) * sgn
                 const T *s = S + (1 + a) * (TILE_BY * BXW);
@@ -455,6 +405,11 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
             }
 
             P vp0[6], vm0[6], cc0[6];  // this plane's Vp, Vm, centre term per group
+            // halfway bounce-back on a y face: for a wall-adjacent row the 9
+            // populations arriving from beyond the wall are f*_ibar of the node itself, a local combination of its own
+            // coefficients: B(kx,kz) with the local sums L(0,0)=6, L(1,1)=-2, L(2,0)=L(2,2)=2.  .x = row r0, .y = row r0+1.
+            P WB[3][3];
+            const P wsp = pk(ghost_lo ? (T)-1 : (T)1, (T)1);
 #pragma unroll
             for (int kz = 0; kz < 3; ++kz) {
                 // ---- a2: Hermite coefficients of the four rows for this kz --------------------------------------
@@ -474,10 +429,16 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                     if (kvalid(kx, 2, kz)) { qh = padd(qh, Ah[kx][2]); qc = padd(qc, Ac[kx][2]); }
                     if (kvalid(kx, 1, kz)) { qh = pfma(Ah[kx][1], sgn, qh); qc = pfma(Ac[kx][1], sgn, qc); }
                     P qs = pk(qc.y, qc.x);
-                    if (any_ghost) {   // rows beyond a bounce-back wall send nothing (bounce_y_correction adds their part)
-                        if (ghost_lo) qh.x = (T)0;
-                        if (ghost_hi) qh.y = (T)0;
-                        if (ghost_mid) { qs.x = (T)0; qh.y = (T)0; }
+                    if (WALLY) {   // rows beyond a bounce-back wall send nothing; the bounced populations are added below
+                        qh = pmul(qh, mh);
+                        qs = pmul(qs, ms);
+                        // B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz) of the own rows: wall below -> (1,-1,1), above -> (1,1,1)
+                        if (kx + kz <= 2 && !(kx == 1 && kz == 2) && !(kx == 2 && kz == 1)) {
+                            P bq = Ac[kx][0];
+                            if (kvalid(kx, 2, kz)) bq = padd(bq, Ac[kx][2]);
+                            if (kvalid(kx, 1, kz)) bq = pfma(Ac[kx][1], wsp, bq);
+                            WB[kx][kz] = bq;
+                        }
                     }
                     const P E = padd(qh, qs);
                     G1[2][kx] = E;
@@ -528,6 +489,28 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                 }
             }
 
+            P kw_new[4];
+            if (WALLY && any_ghost) {
+                // full first-order coefficients (the passes carry them without their base 3 u)
+                WB[1][0] = pfmas(rc[1], (T)3, WB[1][0]);
+                WB[0][0] = pfma(rc[2], pmuls(wsp, (T)3), WB[0][0]);
+                WB[0][1] = pfmas(rc[3], (T)3, WB[0][1]);
+                const P wm = pk((ghost_lo || ghost_mid) ? (T)1 : (T)0, ghost_hi ? (T)1 : (T)0);   // which row of the pack is at a wall
+                const P sgp = pk(ghost_lo ? (T)1 : (T)-1, (T)-1);                              // c_y of the arrival direction
+                const P w12 = pmuls(wm, (T)12), w36 = pmuls(wm, (T)36), w12s = pmul(w12, sgp), w36s = pmul(w36, sgp);
+                // arrival c_z = 0: into this plane's centre terms (they reach the target plane through tt1)
+                cc0[0] = pfma(WB[0][0], w36, cc0[0]);                         // 000
+                cc0[1] = pfma(WB[1][0], pmuls(w12, (T)-1), cc0[1]);           // 100
+                cc0[3] = pfma(WB[0][0], w36s, cc0[3]);                        // 010
+                cc0[2] = pfma(padd(WB[0][0], WB[2][0]), w12, cc0[2]);         // 200
+                cc0[5] = pfma(WB[0][0], w36, cc0[5]);                         // 020
+                cc0[4] = pfma(WB[1][0], pmuls(w12s, (T)-1), cc0[4]);          // 110
+                // moments with c_z: carried to the next iteration, where this plane is the target
+                kw_new[0] = pmul(WB[0][1], pmuls(w12, (T)-1));                // 001
+                kw_new[1] = pmul(padd(WB[0][0], WB[0][2]), w12);              // 002
+                kw_new[2] = pmul(WB[1][1], pmuls(wm, (T)4));                  // 101
+                kw_new[3] = pmul(WB[0][1], pmuls(w12s, (T)-1));               // 011
+            }
             // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
             //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
             const int zt = zs - 1;
@@ -546,30 +529,13 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                     m[5] = pfmas(Dz[2], (T)-36, padd(tt1[5], vm0[5]));           // 020
                 }
                 const long long i0 = lay_idx(L, col, r0, zt);
-                if (WALLY) {   // warp-uniform: only the warps that own a wall row
-                    const bool wlo = r0 == 0 && p.kind[2] == TSLB_BC_BOUNCE_BACK;
-                    const bool whi0 = r0 == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK;
-                    const bool whi1 = r0 + 1 == L.ny - 1 && p.kind[3] == TSLB_BC_BOUNCE_BACK;
-                    if (wlo || whi0) {
-                        T corr[TSLB_NF];
-#pragma unroll
-                        for (int f = 0; f < TSLB_NF; ++f) corr[f] = (T)0;
-                        if (wlo) bounce_y_correction<T>(Abuf, N, i0, p.beta, p.g, true, corr);
-                        if (whi0) bounce_y_correction<T>(Abuf, N, i0, p.beta, p.g, false, corr);
-#pragma unroll
-                        for (int f = 0; f < TSLB_NF; ++f) m[f].x += corr[f];
-                    }
-                    if (whi1) {
-                        T corr[TSLB_NF];
-#pragma unroll
-                        for (int f = 0; f < TSLB_NF; ++f) corr[f] = (T)0;
-                        bounce_y_correction<T>(Abuf, N, i0 + L.px, p.beta, p.g, false, corr);
-#pragma unroll
-                        for (int f = 0; f < TSLB_NF; ++f) m[f].y += corr[f];
-                    }
-                }
+                if (WALLY) { m[3] = padd(m[3], kw[0]); m[6] = padd(m[6], kw[1]); m[8] = padd(m[8], kw[2]); m[9] = padd(m[9], kw[3]); }
                 const int eflags = eflags_xy | ((p.kind[4] == TSLB_BC_PERIODIC && (zt == 0 || zt == L.nz - 1)) ? 8 : 0);
                 finalize_store<P, T>(m, uprev, Bbuf, N, i0, i0 + L.px, row1_valid, eflags, L, col, r0, zt);
+            }
+            if (WALLY && any_ghost) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) kw[k] = kw_new[k];
             }
             // ---- shift the march state ---------------------------------------------------------------------------------
 #pragma unroll
@@ -678,13 +644,13 @@ cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
     if (c->dtype == TSLB_F32) {
         TileParams<float> p = make_tile<float>(c, &grid);
         const size_t smem = TileDims<float>::SMEM_BYTES;
-        if (wally) sweep_tile_kernel<float, true><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<float, false><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur], p);
+        if (wally) sweep_tile_kernel<float, true><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (float *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<float, false><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (float *)c->buf[1 - c->cur], p);
     } else {
         TileParams<double> p = make_tile<double>(c, &grid);
         const size_t smem = TileDims<double>::SMEM_BYTES;
-        if (wally) sweep_tile_kernel<double, true><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<double, false><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (const double *)c->buf[c->cur], (double *)c->buf[1 - c->cur], p);
+        if (wally) sweep_tile_kernel<double, true><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (double *)c->buf[1 - c->cur], p);
+        else sweep_tile_kernel<double, false><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (double *)c->buf[1 - c->cur], p);
     }
     c->launches++;
     return cudaGetLastError();
