@@ -188,8 +188,12 @@ int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
     e = cudaMemset(dev_ptr, 0, 2 * buffer_bytes(c));
     if (e != cudaSuccess) return cuda_fail(c, "cudaMemset(workspace)", e);
     c->tmap_ok = 0;
-    e = tslb_tile_prepare(c);            // TMA descriptors of the two buffers (no-op failure => gather kernel only)
-    if (e != cudaSuccess) return cuda_fail(c, "TMA descriptor setup", e);
+    e = tslb_tile_prepare(c);            // TMA descriptors of the two buffers
+    if (e != cudaSuccess) {              // not fatal: the gather kernel covers everything; TSLB_KERNEL_TILE then reports why
+        (void)cudaGetLastError();
+        c->tmap_ok = 0;
+        snprintf(c->err, sizeof c->err, "TMA descriptor setup failed (%s): tile kernel disabled", cudaGetErrorString(e));
+    }
     return TSLB_OK;
 }
 
