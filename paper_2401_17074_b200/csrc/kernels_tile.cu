@@ -8,14 +8,16 @@
 // With every field scaled by 216 (and the q = 2 fields by a further 2/3) all taps are the small integers
 // 1, 4, -2, so no rounded lattice weight ever multiplies the data.
 //
-// Data path: a CTA owns a 30 x 8 column of nodes and marches along z.  One elected
-// thread streams the z-planes of the 10 moment fields, 32 x 10 nodes each (the tile plus a 1-node halo), from the
-// padded SoA buffer into a 4-deep shared-memory ring with TMA (cp.async.bulk.tensor.4d, mbarrier complete_tx);
-// ghost layers in the buffer stand for the periodic images, so the kernel has no wrap logic.  Every warp owns
-// 2 rows (packed in a 2-wide register pair so fp32 issues as FFMA2/FADD2) x 32 columns (30 outputs + 2 halo lanes):
+// Data path: one CTA per SM owns a 60 x 14 column of nodes (fp32: 2 x 7 warps; fp64: 60 x 8,
+// 2 x 4 warps) and marches along z.  One elected thread streams the z-planes of the 10 moment fields, 64 x 16 nodes
+// each (the tile plus a 1-node halo, rows 16-byte aligned), from the padded SoA buffer into a 4-deep shared-memory
+// ring with TMA (cp.async.bulk.tensor.4d, mbarrier complete_tx); ghost layers in the buffer stand for the periodic
+// images, so the kernel has no wrap logic, and it keeps them current itself by storing the images of the nodes it
+// writes on periodic faces.  Every warp owns 2 rows (packed in a 2-wide register pair so fp32 issues as FFMA2/FADD2)
+// x 32 columns (30 outputs + 2 halo lanes):
 //   y pass: in registers, from the A_k of rows r0-1 .. r0+2 read from shared memory (packs (r0,r0+1) and (r0-1,r0+2)),
-//   x pass: neighbours' values by warp shuffles,
-//   z pass: by marching -- 3 running values per (px,py) group, no plane is staged twice.
+//   x pass: neighbours' values by warp shuffles (one combination up, one down per group),
+//   z pass: by marching -- 15 running pairs per thread, no plane is staged twice.
 // Each node's moments leave HBM once per tile (halo re-reads hit L2) and the 10 new moments are written once:
 // 80 B (fp32) / 160 B (fp64) of compulsory traffic per node update.
 //
