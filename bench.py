@@ -296,13 +296,19 @@ def run_ours(args):
         return 0
 
     peak, peak_src = hbm_peak()
-    achieved = BYTES_PER_SITE[args.dtype] * w.sites / (sweep_ms * 1e-3) / 1e9
+    # Dominant kernel = the sweep.  When the timed region holds exactly one launch per step (periodic / wall runs: the
+    # sweep keeps the ghost layers current itself) its average duration is taken over the timed region itself; otherwise
+    # from the event pairs around the sweep launches of the extra pass.
+    one_per_step = launches == args.steps
+    kernel_ms = ms / args.steps if one_per_step else sweep_ms
+    achieved = BYTES_PER_SITE[args.dtype] * w.sites / (kernel_ms * 1e-3) / 1e9
     roof = {"bound": "hbm", "kernel": "sweep_%s_kernel<%s>" % (kname, args.dtype), "achieved": achieved, "peak": peak,
             "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
             "algorithmic_bytes_per_site": BYTES_PER_SITE[args.dtype],
-            "kernel_ms": sweep_ms, "kernel_launches_timed": sweep_n, "kernel_share_of_step": sweep_ms / (ms / args.steps),
-            "how": "CUDA event pairs around each sweep launch on the launching stream (tslb_set_timing), %d steps run "
-                   "after the timed region" % sweep_n,
+            "kernel_ms": kernel_ms, "kernel_share_of_step": kernel_ms / (ms / args.steps),
+            "how": ("CUDA events around the timed region, %d sweep launches = %d steps" % (launches, args.steps)) if one_per_step
+                   else ("CUDA event pairs around each sweep launch (tslb_set_timing), %d steps run after the timed region" % sweep_n),
+            "kernel_ms_event_pairs": sweep_ms, "kernel_launches_event_pairs": sweep_n,
             "traffic": ncu_traffic("%s_%d_%s" % (kname, args.n, args.dtype))}
     line = {"metric": "GLUPS", "value": value, "unit": "GLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
