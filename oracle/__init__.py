@@ -49,6 +49,9 @@ def _load():
         ip = C.POINTER(C.c_int)
         lib.oracle_fstar.restype = C.c_double
         lib.oracle_fstar.argtypes = [dp, ip, C.c_double, dp, C.c_int]
+        lib.oracle_fstar_order.restype = C.c_double
+        lib.oracle_fstar_order.argtypes = [dp, ip, C.c_double, dp, C.c_int, C.c_int]
+        lib.oracle_set_order.argtypes = [C.c_void_p, C.c_int]
         lib.oracle_mix64.restype = C.c_uint64
         lib.oracle_mix64.argtypes = [C.c_uint64]
         lib.oracle_noise_r24.restype = C.c_uint32
@@ -75,13 +78,13 @@ def _dptr(a: np.ndarray):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def fstar(M10, c3, omega: float, g3=(0.0, 0.0, 0.0), mode: int = MODE_CLOSED) -> float:
-    """Post-collision population f*_c(M) of Eq. 18 for one direction c."""
+def fstar(M10, c3, omega: float, g3=(0.0, 0.0, 0.0), mode: int = MODE_CLOSED, order: int = 3) -> float:
+    """Post-collision population f*_c(M) of Eq. 18 (order 3) or Eq. 8 (order 2)."""
     M = np.ascontiguousarray(M10, dtype=np.float64)
     c = np.ascontiguousarray(c3, dtype=np.intc)
     g = np.ascontiguousarray(g3, dtype=np.float64)
     assert M.shape == (10,) and c.shape == (3,) and g.shape == (3,)
-    return float(_load().oracle_fstar(_dptr(M), c.ctypes.data_as(C.POINTER(C.c_int)), omega, _dptr(g), mode))
+    return float(_load().oracle_fstar_order(_dptr(M), c.ctypes.data_as(C.POINTER(C.c_int)), omega, _dptr(g), mode, order))
 
 
 def mix64(z: int) -> int:
@@ -132,6 +135,10 @@ class Oracle:
         A = np.ascontiguousarray(M, dtype=np.float64)
         assert A.shape == (10,) + self.shape, A.shape
         self._chk(self._lib.oracle_set_moments(self._h, _dptr(A)), "oracle_set_moments")
+
+    def set_order(self, order: int):
+        """Hermite order of the reconstruction: 3 (Eq. 18, default) or 2 (Eq. 8)."""
+        self._chk(self._lib.oracle_set_order(self._h, int(order)), "oracle_set_order")
 
     def set_force(self, g3):
         g = np.ascontiguousarray(g3, dtype=np.float64)

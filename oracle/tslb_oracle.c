@@ -11,6 +11,7 @@
  *   - third-order regularised non-equilibrium                          PAPER.md:150 (Eq. 17)
  *   - recursive a^3_neq = Pi u + u Pi + u Pi                            PAPER.md:146-150 (Eq. 16-17)
  *   - thread-safe fused stream+collide: f_i(x+c_i,t+1)=f_eq+(1-w)f_neq  PAPER.md:68 (Eq. 6), :154 (Eq. 18)
+ *   - second-order variant (oracle_set_order(ctx, 2)): Eq. 2 + (1-w) Eq. 7     PAPER.md:86-89 (Eq. 8)
  *   - new moments by linear local sums                                 PAPER.md:45, :126 (Eq. 12)
  *   - body force term rho w_i c_i.F / c_s^2
  *   - NEQ-extrapolation open boundaries (Dirichlet u / zero gradient)  PAPER.md:181-202 (Eq. 22-23), :258
@@ -52,6 +53,7 @@ typedef struct {
     int n[3];              /* nx, ny, nz */
     double tau, omega;     /* omega = 1/tau, nu = cs2 (1/omega - 1/2) */
     double g[3];           /* body acceleration */
+    int order;             /* Hermite order of the expansion: 3 (Eq. 18, default) or 2 (Eq. 8) */
     int kind[6];           /* per face */
     double *uin[6];        /* inlet planes [3][n_b][n_a], owned copy, or NULL */
     double noise_amp[6];
@@ -84,7 +86,7 @@ static void unpack(const double M[NF], double *rho, double u[3], double Pi[3][3]
  *               + rho c.g/cs2 ]
  * with a3_abg = Pi_ab u_g + u_a Pi_bg + u_b Pi_ag                                  Eq. 17
  * Mode 0: tensors built from the definitions, all index values summed.            */
-static double fstar_brute(const double M[NF], const int c[3], double omega, const double g[3])
+static double fstar_brute(const double M[NF], const int c[3], double omega, const double g[3], int order)
 {
     double rho, u[3], Pi[3][3];
     unpack(M, &rho, u, Pi);
@@ -112,6 +114,7 @@ static double fstar_brute(const double M[NF], const int c[3], double omega, cons
     }
     const double cs4 = CS2 * CS2, cs6 = cs4 * CS2;
     double w = w1(c[0]) * w1(c[1]) * w1(c[2]);
+    if (order < 3) { eq3 = 0.0; ne3 = 0.0; }   /* Eq. 8: the expansion stops at the second-order Hermite terms */
     return w * (rho * (1.0 + cu / CS2 + eq2 / (2.0 * cs4) + eq3 / (6.0 * cs6))
                 + (1.0 - omega) * (ne2 / (2.0 * cs4) + ne3 / (6.0 * cs6))
                 + rho * cg / CS2);
@@ -123,7 +126,7 @@ static double fstar_brute(const double M[NF], const int c[3], double omega, cons
  *   H2:Pi  = c.Pi.c - cs2 tr Pi
  *   H3:a3  = ccc:a3 - 3 cs2 c_g a3_aag            (a3 is fully symmetric)
  *          = 3 (c.Pi.c)(c.u) - 3 cs2 [ trPi (c.u) + 2 c.Pi.u ]                       */
-static double fstar_closed(const double M[NF], const int c[3], double omega, const double g[3])
+static double fstar_closed(const double M[NF], const int c[3], double omega, const double g[3], int order)
 {
     double rho, u[3], Pi[3][3];
     unpack(M, &rho, u, Pi);
@@ -144,14 +147,19 @@ static double fstar_closed(const double M[NF], const int c[3], double omega, con
     double ne2 = cPc - CS2 * trP;
     double ne3 = 3.0 * cPc * cu - 3.0 * CS2 * (trP * cu + 2.0 * cPu);
     double w = w1(c[0]) * w1(c[1]) * w1(c[2]);
+    if (order < 3) { eq3 = 0.0; ne3 = 0.0; }   /* Eq. 8: the expansion stops at the second-order Hermite terms */
     return w * (rho * (1.0 + cu / CS2 + eq2 / (2.0 * cs4) + eq3 / (6.0 * cs6))
                 + (1.0 - omega) * (ne2 / (2.0 * cs4) + ne3 / (6.0 * cs6))
                 + rho * cg / CS2);
 }
 
+double oracle_fstar_order(const double *M10, const int *c3, double omega, const double *g3, int mode, int order)
+{
+    return mode == 0 ? fstar_brute(M10, c3, omega, g3, order) : fstar_closed(M10, c3, omega, g3, order);
+}
 double oracle_fstar(const double *M10, const int *c3, double omega, const double *g3, int mode)
 {
-    return mode == 0 ? fstar_brute(M10, c3, omega, g3) : fstar_closed(M10, c3, omega, g3);
+    return oracle_fstar_order(M10, c3, omega, g3, mode, 3);
 }
 
 /* ---- inlet noise (reading A14 in DESIGN.md) ---------------------------------------------
@@ -185,6 +193,7 @@ int oracle_create(int nx, int ny, int nz, double tau, oracle_ctx **out)
     if (!c) return 2;
     c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
     c->tau = tau; c->omega = 1.0 / tau;
+    c->order = 3;
     size_t N = (size_t)nx * ny * nz;
     c->M[0] = (double *)malloc(sizeof(double) * NF * N);
     c->M[1] = (double *)malloc(sizeof(double) * NF * N);
@@ -206,6 +215,14 @@ int oracle_set_moments(oracle_ctx *c, const double *src)
     size_t N = (size_t)c->n[0] * c->n[1] * c->n[2];
     memcpy(c->M[c->cur], src, sizeof(double) * NF * N);
     c->t = 0; c->have_state = 1;
+    return 0;
+}
+
+/* Hermite order of the reconstruction: 3 = Eq. 18 (high-order TSLB), 2 = Eq. 8 (the second-order TSLB of ref. 10). */
+int oracle_set_order(oracle_ctx *c, int order)
+{
+    if (!c || (order != 2 && order != 3)) return 1;
+    c->order = order;
     return 0;
 }
 
@@ -347,12 +364,12 @@ static void sweep(oracle_ctx *c, int mode)
                             double f;
                             if (bounced) {          /* halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) */
                                 const int cb[3] = { -cx, -cy, -cz };
-                                f = oracle_fstar(Mx, cb, c->omega, c->g, mode);
+                                f = oracle_fstar_order(Mx, cb, c->omega, c->g, mode, c->order);
                             } else {
                                 double Ms[NF];
                                 size_t iq = lin(c, q);
                                 for (int k = 0; k < NF; ++k) Ms[k] = A[k * N + iq];
-                                f = oracle_fstar(Ms, ci, c->omega, c->g, mode);
+                                f = oracle_fstar_order(Ms, ci, c->omega, c->g, mode, c->order);
                             }
                             R += f;
                             for (int a = 0; a < 3; ++a) {

@@ -463,3 +463,79 @@ def test_paper_parameter_sets():
     assert abs(w.tau - (0.5 + 3 * 0.0035 * 4 / 180)) < 1e-15 and abs(w.g[0] - 0.0035**2 / 4) < 1e-20
     j = W.jet(8, 8, 8, steps=1)
     assert abs(j.tau - (0.5 + 3 * 0.05 * 20 / 7000)) < 1e-15
+
+
+# ---------------------------------------------------------------------------------------------
+# Second-order variant (Eq. 8): oracle_set_order(2).  SURVEY.md 8(f) rank 2.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+def test_order2_moments(oracle_mod, mode):
+    """Eq. 8 reproduces rho, rho u and rho cs2 I + rho uu + (1-w) Pi exactly like Eq. 18; its third moments carry
+    only the lattice part cs2 rho (u delta)_sym: no rho uuu, no a3 (that is what 'second order' means)."""
+    rng = np.random.default_rng(23)
+    for _ in range(10):
+        M = rand_M(rng)
+        omega = rng.uniform(0.6, 1.9)
+        rho, u, Pi = M[0], M[1:4], Pi_of(M)
+        f = np.array([oracle_mod.fstar(M, c, omega, mode=mode, order=2) for c in DIRS])
+        c = np.array(DIRS, float)
+        assert abs(f.sum() - rho) < 1e-15
+        assert np.abs(c.T @ f - rho * u).max() < 1e-15
+        S = np.einsum("i,ia,ib->ab", f, c, c)
+        assert np.abs(S - (rho * CS2 * np.eye(3) + rho * np.outer(u, u) + (1 - omega) * Pi)).max() < 1e-15
+        Q = np.einsum("i,ia,ib,ig->abg", f, c, c, c)
+        d = np.eye(3)
+        lattice = CS2 * rho * (np.einsum("a,bg->abg", u, d) + np.einsum("b,ag->abg", u, d) + np.einsum("g,ab->abg", u, d))
+        for a, b, g in itertools.product(range(3), repeat=3):
+            if not (a == b == g):
+                assert abs(Q[a, b, g] - lattice[a, b, g]) < 1e-15
+        # and it differs from the third-order population by exactly the H3 terms
+        f3 = np.array([oracle_mod.fstar(M, c_, omega, mode=mode, order=3) for c_ in DIRS])
+        assert np.abs(f3 - f).max() > 1e-7
+
+
+def test_order2_population_code_equivalence(oracle_mod):
+    """Order-2 TSLB == explicit collide-and-stream BGK with second-order equilibrium and the projected (Eq. 7)
+    non-equilibrium part, at every step, walls and force included."""
+    class Pop2(PopulationLB):
+        def feq(self, rho, u):
+            cu = np.einsum("ia,a...->i...", self.cf, u)
+            e2 = np.einsum("iab,a...,b...->i...", self.H2, u, u)
+            wb = self.w.reshape((-1,) + (1,) * (u.ndim - 1))
+            return wb * rho[None] * (1 + cu / CS2 + e2 / (2 * CS2**2))             # Eq. 2
+
+        def fneq_reg(self, a2, u):
+            wb = self.w.reshape((-1,) + (1,) * (u.ndim - 1))
+            return wb * np.einsum("iab,ab...->i...", self.H2, a2) / (2 * CS2**2)   # Eq. 7
+    w = W.random_state(6, 5, 7, seed=8, tau=0.7)
+    g = (1e-4, 2e-4, -3e-4)
+    for walls in (False, True):
+        o = oracle_mod.Oracle(6, 5, 7, w.tau)
+        o.set_order(2)
+        if walls:
+            o.set_face(W.FACE_YLO, W.BC_BOUNCE_BACK); o.set_face(W.FACE_YHI, W.BC_BOUNCE_BACK)
+        o.set_force(g); o.set_moments(w.moments)
+        p = Pop2(w.moments, w.tau, g, walls_y=walls)
+        for s in range(5):
+            o.step(1); p.step()
+            assert np.abs(o.get_moments() - p.M()).max() < 5e-15, (walls, s)
+
+
+def test_order2_brute_vs_closed_and_decay(oracle_mod):
+    """Brute-force and closed-form modes agree at order 2; the viscosity is unchanged (nu = (tau - 1/2)/3)."""
+    w = W.random_state(5, 4, 6, seed=2, tau=0.66)
+    a = oracle_mod.Oracle(5, 4, 6, w.tau); b = oracle_mod.Oracle(5, 4, 6, w.tau)
+    for o in (a, b):
+        o.set_order(2); o.set_force((1e-4, 0, -1e-4)); o.set_moments(w.moments)
+    a.step(3, mode=oracle_mod.MODE_BRUTE); b.step(3, mode=oracle_mod.MODE_CLOSED)
+    assert np.abs(a.get_moments() - b.get_moments()).max() < 1e-15
+    w = W.taylor_green_2d(n=32, nz=3, tau=0.8, U0=0.01, steps=100)
+    o = oracle_mod.Oracle(w.nx, w.ny, w.nz, w.tau); o.set_order(2); o.set_moments(w.moments); o.step(100)
+    M = o.get_moments()
+    k = 2 * np.pi / 32
+    nu = (0.8 - 0.5) / 3
+    ratio = np.abs(M[1]).max() / 0.01
+    nu_eff = -np.log(ratio) / (2 * k * k * 100)
+    assert abs(nu_eff / nu - 1) < 0.02
+    with pytest.raises(RuntimeError):
+        o.set_order(4)
