@@ -40,6 +40,8 @@ def parse_args(argv=None):
     ap.add_argument("--n", type=int, default=512, help="cube edge of the configs[4] workload")
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"])
     ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "tile"])
+    ap.add_argument("--order", type=int, default=3, choices=[2, 3],
+                    help="Hermite order of the reconstruction: 3 = the paper's high-order TSLB (the headline), 2 = Eq. 8")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
@@ -222,6 +224,7 @@ def run_ours(args):
     kernel = {"auto": B.KERNEL_AUTO, "gather": B.KERNEL_GATHER, "tile": B.KERNEL_TILE}[args.kernel]
 
     w = W.throughput(args.n, args.dtype, args.steps)
+    w.order = args.order
     sim = B.from_workload(w, kernel)
     host = torch.from_numpy(w.moments)
     sim.set_moments(host.to("cuda"))
@@ -312,7 +315,7 @@ def run_ours(args):
             "traffic": ncu_traffic("%s_%d_%s" % (kname, args.n, args.dtype))}
     line = {"metric": "GLUPS", "value": value, "unit": "GLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": args.dtype, "data": "synthetic", "config": dict(workload_config(args), kernel=kname),
+            "vs_baseline": None, "dtype": args.dtype, "data": "synthetic", "config": dict(workload_config(args), kernel=kname, order=args.order),
             "roofline": roof, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches)}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_budget_s)

@@ -105,6 +105,11 @@ int tslb_set_moments_host(tslb_ctx *ctx, const void *host_src, void *stream);
  * set (PERIODIC must be on both faces of an axis) is checked by tslb_step. */
 int tslb_set_boundary(tslb_ctx *ctx, int face, int kind, const void *params);
 
+/* Hermite order of the reconstruction: 3 (default) = the high-order TSLB of PAPER.md:154 (Eq. 18); 2 = the second-order
+ * TSLB of PAPER.md:86-89 (Eq. 8: second-order equilibrium, Eq. 2, plus (1 - omega) times the projected non-equilibrium
+ * part, Eq. 7).  Same stored state, same traffic; only the arithmetic changes.  TSLB_EINVAL for any other value. */
+int tslb_set_order(tslb_ctx *ctx, int order);
+
 /* Choose the sweep kernel (TSLB_KERNEL_*).  TSLB_EINVAL if TILE is forced on a configuration it does not
  * cover (reported by tslb_step). */
 int tslb_set_kernel(tslb_ctx *ctx, int kernel);

@@ -24,7 +24,7 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile
 SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
-           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing")
+           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order")
 
 
 class InletParams(C.Structure):
@@ -62,6 +62,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_set_moments_host.argtypes = [vp, vp, vp]
     lib.tslb_set_boundary.argtypes = [vp, ip, ip, vp]
     lib.tslb_set_kernel.argtypes = [vp, ip]
+    lib.tslb_set_order.argtypes = [vp, ip]
     lib.tslb_active_kernel.argtypes = [vp]
     lib.tslb_step.argtypes = [vp, ip, vp]
     lib.tslb_get_moments.argtypes = [vp, vp, vp]
@@ -178,6 +179,10 @@ class TSLB:
         arr = (C.c_double * 3)(*[float(v) for v in g])
         self._chk(self._lib.tslb_set_boundary(self._h, 0, BC_BODY_FORCE, C.cast(arr, C.c_void_p)), "tslb_set_boundary")
 
+    def set_order(self, order: int):
+        """Hermite order of the reconstruction: 3 (Eq. 18, default) or 2 (Eq. 8)."""
+        self._chk(self._lib.tslb_set_order(self._h, int(order)), "tslb_set_order")
+
     def set_kernel(self, kernel: int):
         self._chk(self._lib.tslb_set_kernel(self._h, int(kernel)), "tslb_set_kernel")
 
@@ -250,5 +255,7 @@ def from_workload(w, kernel: int = KERNEL_AUTO) -> TSLB:
             sim.set_boundary(face, kind)
     if any(w.g):
         sim.set_body_force(w.g)
+    if getattr(w, "order", 3) != 3:
+        sim.set_order(w.order)
     sim.set_kernel(kernel)
     return sim

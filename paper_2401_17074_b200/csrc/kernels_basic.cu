@@ -42,7 +42,7 @@ __device__ __forceinline__ Site<T> load_site(const T *__restrict__ A, long long 
 // the base never passes through rounded arithmetic and only `lin` (a difference of neighbouring velocities plus
 // small terms) does.  The caller passes lin = c.(u_src - u_x) + c.(g + drho_src (u_src + g)).
 template <typename T>
-__device__ __forceinline__ T fstar_incr(const Site<T> &m, int cx, int cy, int cz, T sgn, T w, T beta, T lin)
+__device__ __forceinline__ T fstar_incr(const Site<T> &m, int cx, int cy, int cz, T sgn, T w, T beta, T lin, T o3)
 {
     const T fx = (T)cx, fy = (T)cy, fz = (T)cz;
     const T rho = (T)1 + m.dr;
@@ -58,7 +58,8 @@ __device__ __forceinline__ T fstar_incr(const Site<T> &m, int cx, int cy, int cz
     const T odd_eq = (T)4.5 * cu * (cu * cu - uu);
     const T even_ne = (T)4.5 * cPc - (T)1.5 * trP;
     const T odd_ne = (T)4.5 * ((T)3 * cPc * cu - trP * cu - (T)2 * cPu);
-    return w * (m.dr + (T)3 * lin + rho * (even_eq + sgn * odd_eq) + beta * (even_ne + sgn * odd_ne));
+    // o3 = 0 drops the third-order Hermite terms: the second-order TSLB of Eq. 8
+    return w * (m.dr + (T)3 * lin + rho * (even_eq + sgn * o3 * odd_eq) + beta * (even_ne + sgn * o3 * odd_ne));
 }
 
 __device__ __forceinline__ bool is_open_kind(int k)
@@ -135,7 +136,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                 const T w = (T)((cx ? 1 : 4) * (cy ? 1 : 4) * (cz ? 1 : 4));
                 T f;
                 if (cx == 0 && cy == 0 && cz == 0) {
-                    f = fstar_incr(own, 0, 0, 0, (T)1, w, p.beta, (T)0);
+                    f = fstar_incr(own, 0, 0, 0, (T)1, w, p.beta, (T)0, p.o3);
                 } else {
                     // halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) from the node's own moments
                     const long long is = bounced ? ip : lay_idx(p.L, sx[cx + 1], sy[cy + 1], sz[cz + 1]);
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                         lin = -((T)cx * ((T)2 * own.ux + smx) + (T)cy * ((T)2 * own.uy + smy) + (T)cz * ((T)2 * own.uz + smz));
                     else
                         lin = (T)cx * ((m.ux - own.ux) + smx) + (T)cy * ((m.uy - own.uy) + smy) + (T)cz * ((m.uz - own.uz) + smz);
-                    f = fstar_incr(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, lin);
+                    f = fstar_incr(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, lin, p.o3);
                 }
                 dR += f;                                  // arrival direction c_i in every sum
                 if (cx) Jx += (T)cx * f;
@@ -380,6 +381,7 @@ SweepParams<T> make_params(const tslb_ctx *c)
     for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
     p.beta = (T)(1.0 - c->omega);
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
+    p.o3 = c->order >= 3 ? (T)1 : (T)0;
     return p;
 }
 

@@ -103,8 +103,9 @@ struct TileParams {
     int zchunk;  // planes per z chunk
 };
 
-// valid Hermite index: each <= 2, sum <= 3 (H3_aaa == 0 on this lattice)
-__host__ __device__ constexpr bool kvalid(int kx, int ky, int kz) { return kx <= 2 && ky <= 2 && kz <= 2 && kx + ky + kz <= 3; }
+// valid Hermite index: each <= 2, sum <= ORDER (3: Eq. 18, H3_aaa == 0 on this lattice; 2: the second-order TSLB of Eq. 8)
+template <int ORDER>
+__host__ __device__ constexpr bool kvalid(int kx, int ky, int kz) { return kx <= 2 && ky <= 2 && kz <= 2 && kx + ky + kz <= ORDER; }
 
 // ---- Hermite coefficients of one pack of two nodes, round kz (216-scaled, integer prefactors) -----------
 //   A000 = drho                       A100 = 3 [rho (ux+gx) - ux]  (increment form: base 3 ux handled apart)
@@ -290,7 +291,7 @@ template <typename T> struct TileDims {
 };
 static_assert(TileDims<float>::BY <= TILE_MAX_BY && TileDims<double>::BY <= TILE_MAX_BY, "layout height");
 
-template <typename T, bool WALLY>
+template <typename T, bool WALLY, int ORDER>
 __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA,
                                                                    T *__restrict__ Bbuf, TileParams<T> p)
 {
@@ -423,13 +424,13 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                 P G1[3][3];
 #pragma unroll
                 for (int kx = 0; kx < 3; ++kx) {
-                    if (!kvalid(kx, 0, kz)) continue;
+                    if (!kvalid<ORDER>(kx, 0, kz)) continue;
                     // E = up(P) + dn(M), O = up(P) - dn(M) with P = phi0 + phi1 + phi2, M = phi0 - phi1 + phi2 of the
                     // neighbour rows.  Per pack Q = (P of its .x row, M of its .y row) = phi0 + phi2 + phi1 * sgn; then
                     // E = Q_H + swap(Q_C) and O = (Q_H - swap(Q_C)) * sgn.
                     P qh = Ah[kx][0], qc = Ac[kx][0];
-                    if (kvalid(kx, 2, kz)) { qh = padd(qh, Ah[kx][2]); qc = padd(qc, Ac[kx][2]); }
-                    if (kvalid(kx, 1, kz)) { qh = pfma(Ah[kx][1], sgn, qh); qc = pfma(Ac[kx][1], sgn, qc); }
+                    if (kvalid<ORDER>(kx, 2, kz)) { qh = padd(qh, Ah[kx][2]); qc = padd(qc, Ac[kx][2]); }
+                    if (kvalid<ORDER>(kx, 1, kz)) { qh = pfma(Ah[kx][1], sgn, qh); qc = pfma(Ac[kx][1], sgn, qc); }
                     P qs = pk(qc.y, qc.x);
                     if (WALLY) {   // rows beyond a bounce-back wall send nothing; the bounced populations are added below
                         qh = pmul(qh, mh);
@@ -437,8 +438,8 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                         // B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz) of the own rows: wall below -> (1,-1,1), above -> (1,1,1)
                         if (kx + kz <= 2 && !(kx == 1 && kz == 2) && !(kx == 2 && kz == 1)) {
                             P bq = Ac[kx][0];
-                            if (kvalid(kx, 2, kz)) bq = padd(bq, Ac[kx][2]);
-                            if (kvalid(kx, 1, kz)) bq = pfma(Ac[kx][1], wsp, bq);
+                            if (kvalid<ORDER>(kx, 2, kz)) bq = padd(bq, Ac[kx][2]);
+                            if (kvalid<ORDER>(kx, 1, kz)) bq = pfma(Ac[kx][1], wsp, bq);
                             WB[kx][kz] = bq;
                         }
                     }
@@ -446,7 +447,7 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                     G1[2][kx] = E;
                     G1[1][kx] = pmul(psub(qh, qs), sgn);
                     P o0 = pfmas(Ac[kx][0], (T)4, E);
-                    if (kvalid(kx, 2, kz)) o0 = pfmas(Ac[kx][2], (T)-2, o0);
+                    if (kvalid<ORDER>(kx, 2, kz)) o0 = pfmas(Ac[kx][2], (T)-2, o0);
                     G1[0][kx] = o0;
                 }
                 // y-stage increments of the bases 3 u_a (tap sums along y: 6, 0, 2 for py = 0, 1, 2 when ky = 0; 0, 2, 0 when ky = 1)
@@ -464,14 +465,16 @@ __global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sw
                     // E = up(P) + dn(M), O = up(P) - dn(M): one shuffle up of P = phi0 + phi1 + phi2 and one down of
                     // M = phi0 - phi1 + phi2 instead of two per field
                     P t = G1[py][0];
-                    if (kvalid(2, 0, kz)) t = padd(t, G1[py][2]);
-                    const P upP = shfl_up1(padd(t, G1[py][1]));   // from column-1  (c_x = +1 pulls from x-1)
-                    const P dnM = shfl_dn1(psub(t, G1[py][1]));   // from column+1
+                    if (kvalid<ORDER>(2, 0, kz)) t = padd(t, G1[py][2]);
+                    P pp = t, mm = t;
+                    if (kvalid<ORDER>(1, 0, kz)) { pp = padd(t, G1[py][1]); mm = psub(t, G1[py][1]); }
+                    const P upP = shfl_up1(pp);   // from column-1  (c_x = +1 pulls from x-1)
+                    const P dnM = shfl_dn1(mm);   // from column+1
                     P o[3];
                     o[2] = padd(upP, dnM);
                     o[1] = psub(upP, dnM);
                     o[0] = pfmas(G1[py][0], (T)4, o[2]);
-                    if (kvalid(2, 0, kz)) o[0] = pfmas(G1[py][2], (T)-2, o[0]);
+                    if (kvalid<ORDER>(2, 0, kz)) o[0] = pfmas(G1[py][2], (T)-2, o[0]);
                     // x-stage increments: base multipliers after the y stage are 18 (py=0) and 6 (py=2) for ux (kx=1) and uz
                     // (kx=0, kz=1), 6 (py=1) for uy (kx=0)
                     if (kz == 0 && py == 0) { o[0] = pfmas(Dx[0], (T)18, o[0]); o[1] = pfmas(Lx[0], (T)18, o[1]); o[2] = pfmas(Dx[0], (T)18, o[2]); }
@@ -630,29 +633,36 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
     const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
-    e = cudaFuncSetAttribute(sweep_tile_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem32);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem64);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem64);
+    e = cudaSuccess;
+#define TSLB_SMEM_ATTR(T, W, O, B) if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
+    TSLB_SMEM_ATTR(float, false, 3, smem32); TSLB_SMEM_ATTR(float, true, 3, smem32);
+    TSLB_SMEM_ATTR(float, false, 2, smem32); TSLB_SMEM_ATTR(float, true, 2, smem32);
+    TSLB_SMEM_ATTR(double, false, 3, smem64); TSLB_SMEM_ATTR(double, true, 3, smem64);
+    TSLB_SMEM_ATTR(double, false, 2, smem64); TSLB_SMEM_ATTR(double, true, 2, smem64);
+#undef TSLB_SMEM_ATTR
     if (e != cudaSuccess) return e;
     c->tmap_ok = 1;
     return cudaSuccess;
 }
 
+template <typename T, bool WALLY, int ORDER>
+static void launch_tile(tslb_ctx *c, cudaStream_t st)
+{
+    dim3 grid;
+    TileParams<T> p = make_tile<T>(c, &grid);
+    sweep_tile_kernel<T, WALLY, ORDER><<<grid, TileDims<T>::WARPS * 32, TileDims<T>::SMEM_BYTES, st>>>(c->tmap[c->cur], (T *)c->buf[1 - c->cur], p);
+}
+
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
 {
     const bool wally = c->kind[2] == TSLB_BC_BOUNCE_BACK || c->kind[3] == TSLB_BC_BOUNCE_BACK;
-    dim3 grid;
+    const bool o3 = c->order >= 3;
     if (c->dtype == TSLB_F32) {
-        TileParams<float> p = make_tile<float>(c, &grid);
-        const size_t smem = TileDims<float>::SMEM_BYTES;
-        if (wally) sweep_tile_kernel<float, true><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (float *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<float, false><<<grid, TileDims<float>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (float *)c->buf[1 - c->cur], p);
+        if (wally) { if (o3) launch_tile<float, true, 3>(c, st); else launch_tile<float, true, 2>(c, st); }
+        else { if (o3) launch_tile<float, false, 3>(c, st); else launch_tile<float, false, 2>(c, st); }
     } else {
-        TileParams<double> p = make_tile<double>(c, &grid);
-        const size_t smem = TileDims<double>::SMEM_BYTES;
-        if (wally) sweep_tile_kernel<double, true><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (double *)c->buf[1 - c->cur], p);
-        else sweep_tile_kernel<double, false><<<grid, TileDims<double>::WARPS * 32, smem, st>>>(c->tmap[c->cur], (double *)c->buf[1 - c->cur], p);
+        if (wally) { if (o3) launch_tile<double, true, 3>(c, st); else launch_tile<double, true, 2>(c, st); }
+        else { if (o3) launch_tile<double, false, 3>(c, st); else launch_tile<double, false, 2>(c, st); }
     }
     c->launches++;
     return cudaGetLastError();

@@ -111,6 +111,7 @@ int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out)
     if (!c) return fail(nullptr, TSLB_ENOMEM, "host allocation failed");
     c->nx = nx; c->ny = ny; c->nz = nz; c->dtype = dtype;
     c->tau = tau; c->omega = 1.0 / tau;
+    c->order = 3;
     c->kernel_req = TSLB_KERNEL_AUTO;
     c->sm_count = 148;
     c->L = make_layout(nx, ny, nz);
@@ -252,6 +253,14 @@ int tslb_set_boundary(tslb_ctx *c, int face, int kind, const void *params)
     }
     c->kind[face] = kind;
     c->halo_valid = 0;
+    return TSLB_OK;
+}
+
+int tslb_set_order(tslb_ctx *c, int order)
+{
+    if (!c) return TSLB_EINVAL;
+    if (order != 2 && order != 3) return fail(c, TSLB_EINVAL, "order must be 2 (Eq. 8) or 3 (Eq. 18)");
+    c->order = order;
     return TSLB_OK;
 }
 

@@ -32,6 +32,7 @@ struct SweepParams {
     int kind[6];   // TSLB_BC_* per face
     T beta;        // 1 - omega = 1 - 1/tau, formed in double and rounded once (Eq. 5)
     T g[3];        // body acceleration
+    T o3;          // 1 for the third-order expansion (Eq. 18), 0 for the second-order one (Eq. 8)
 };
 
 struct InletDev {
@@ -55,6 +56,7 @@ struct FillParams {
 struct tslb_ctx {
     int nx, ny, nz, dtype;
     double tau, omega;
+    int order;        // Hermite order of the reconstruction, 3 (Eq. 18) or 2 (Eq. 8)
     double g[3];
     int kind[6];
     InletDev inlet[6];

@@ -47,6 +47,7 @@ class Workload:
     faces: Dict[int, int] = field(default_factory=dict)   # face -> kind (default periodic)
     g: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     inlet: Optional[Inlet] = None
+    order: int = 3               # Hermite order of the reconstruction (3: Eq. 18, 2: Eq. 8)
 
     @property
     def sites(self) -> int:

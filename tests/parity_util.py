@@ -21,6 +21,8 @@ def make_oracle(oracle_mod, w):
         else:
             o.set_face(f, k)
     o.set_force(w.g)
+    if getattr(w, "order", 3) != 3:
+        o.set_order(w.order)
     o.set_moments(w.moments)          # the run-dtype array, converted exactly to fp64
     return o
 

@@ -221,6 +221,37 @@ def test_set_moments_mid_run_and_timing_api(B, oracle_mod):
 
 
 # ---------------------------------------------------------------------------------------------
+# second-order variant (Eq. 8, tslb_set_order(2)): SURVEY.md 8(f) rank 2
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_order2_parity(B, oracle_mod, dtype):
+    cases = [W.random_state(70, 21, 9, seed=12, dtype=dtype, tau=0.64),
+             with_faces(W.random_state(66, 11, 7, seed=13, dtype=dtype, tau=0.6),
+                        {W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, g=(2e-4, 0, -1e-4)),
+             with_faces(W.random_state(12, 10, 14, seed=14, dtype=dtype, tau=0.58), **BC_SETS["jet_like"])]
+    for w in cases:
+        w.order = 2
+        for k in kernels_for(B, w):
+            G, R, _ = run_both(oracle_mod, w, 4, k)
+            assert_parity(w, G, R, "order 2, kernel %d" % k)
+            # and it is not the third-order result
+            w3 = W.Workload(**{**w.__dict__, "order": 3})
+            G3, _, _ = run_both(oracle_mod, w3, 4, k)
+            assert np.abs(G3 - G).max() > 1e-9
+
+
+def test_order2_config1_reduced(B, oracle_mod):
+    """configs[1] inputs at 32^3, 300 steps, second-order reconstruction (near-inviscid: the case where the paper expects
+    the higher order to matter for stability; here only parity and boundedness over a short run)."""
+    w = W.config1(n=32, steps=300)
+    w.order = 2
+    for k in kernels_for(B, w):
+        G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 100])
+        print("config1@32 order 2 kernel %d curve: %s" % (k, curve))
+        assert_parity(w, G, R, "order 2 kernel %d" % k)
+
+
+# ---------------------------------------------------------------------------------------------
 # library behaviour on the device
 # ---------------------------------------------------------------------------------------------
 def test_checkpoint_resume(B):
