@@ -140,6 +140,15 @@ int tslb_diagnostics(tslb_ctx *ctx, double *dev_out5, void *stream);
 int tslb_set_timing(tslb_ctx *ctx, int max_launches);
 int tslb_get_timing(tslb_ctx *ctx, int *n_launches, double *total_ms);
 
+/* Running plane statistics for the turbulence statistics of PAPER.md:236 (Eq. 24) and :242 (Eq. 25).  For every plane j
+ * of constant coordinate along `axis` (0 = x, 1 = y, 2 = z) the sums over the nodes of the plane of
+ *     1 | ux uy uz | ux ux, uy uy, uz uz, ux uy, ux uz, uy uz | ux^3 uy^3 uz^3
+ * at the current time (open-face boundary nodes refilled first) are ADDED to dev_sums, 13 rows of n_axis doubles in
+ * device memory ([13][n_axis], row order as listed).  The caller zeroes the array once and calls once per sample; means,
+ * Reynolds stresses <u'_i u'_j> and skewness follow from the raw sums.  fp64 accumulation, warp-shuffle reduction,
+ * fixed-order final pass (bitwise reproducible).  TSLB_EINVAL: bad axis or NULL; TSLB_ESTATE: no state. */
+int tslb_plane_statistics(tslb_ctx *ctx, int axis, double *dev_sums, void *stream);
+
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);
 /* Number of kernels this context has launched so far (all kinds), for bench.py's gpu_launches. */

@@ -67,6 +67,7 @@ def _load():
         lib.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
         lib.oracle_get_moments.argtypes = [C.c_void_p, dp]
         lib.oracle_diagnostics.argtypes = [C.c_void_p, dp]
+        lib.oracle_plane_statistics.argtypes = [C.c_void_p, C.c_int, dp]
         lib.oracle_step_count.argtypes = [C.c_void_p]
         lib.oracle_step_count.restype = C.c_longlong
         lib.oracle_num_threads.restype = C.c_int
@@ -166,6 +167,13 @@ class Oracle:
         out = np.empty(5, dtype=np.float64)
         self._chk(self._lib.oracle_diagnostics(self._h, _dptr(out)), "oracle_diagnostics")
         return out
+
+    def plane_statistics(self, axis: int, sums: np.ndarray) -> np.ndarray:
+        """Add one sample of the plane sums (Eq. 24-25 raw sums) to sums[13][n_axis] (fp64, C-contiguous)."""
+        n_axis = self.shape[2 - axis]
+        assert sums.dtype == np.float64 and sums.shape == (13, n_axis) and sums.flags["C_CONTIGUOUS"]
+        self._chk(self._lib.oracle_plane_statistics(self._h, int(axis), _dptr(sums)), "oracle_plane_statistics")
+        return sums
 
     @property
     def step_count(self) -> int:

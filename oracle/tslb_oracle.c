@@ -433,6 +433,39 @@ int oracle_diagnostics(oracle_ctx *c, double *out5)
     return 0;
 }
 
+/* Running plane statistics (PAPER.md:236 Eq. 24, :242 Eq. 25): for every plane j of constant coordinate along `axis`
+ * ADD to sums[13][n_axis] the sums over the nodes of the plane of
+ *   1 | u_x u_y u_z | u_x u_x, u_y u_y, u_z u_z, u_x u_y, u_x u_z, u_y u_z | u_x^3 u_y^3 u_z^3
+ * at the current time (boundary nodes refilled first).  Means, Reynolds stresses <u'_i u'_j> and skewness follow from
+ * these raw sums; the caller zeroes the array once and calls once per sample. */
+int oracle_plane_statistics(oracle_ctx *c, int axis, double *sums)
+{
+    if (!c || !sums || axis < 0 || axis > 2) return 1;
+    if (!c->have_state) return 4;
+    const size_t N = (size_t)c->n[0] * c->n[1] * c->n[2];
+    const int na = c->n[axis];
+    double *M = c->M[c->cur];
+    ghost_fill(c, M);
+    for (int z = 0; z < c->n[2]; ++z)
+        for (int y = 0; y < c->n[1]; ++y)
+            for (int x = 0; x < c->n[0]; ++x) {
+                const int p[3] = { x, y, z };
+                const size_t i = lin(c, p);
+                const int j = p[axis];
+                const double u[3] = { M[N + i], M[2 * N + i], M[3 * N + i] };
+                sums[0 * na + j] += 1.0;
+                for (int a = 0; a < 3; ++a) {
+                    sums[(1 + a) * na + j] += u[a];
+                    sums[(4 + a) * na + j] += u[a] * u[a];
+                    sums[(10 + a) * na + j] += u[a] * u[a] * u[a];
+                }
+                sums[7 * na + j] += u[0] * u[1];
+                sums[8 * na + j] += u[0] * u[2];
+                sums[9 * na + j] += u[1] * u[2];
+            }
+    return 0;
+}
+
 long long oracle_step_count(const oracle_ctx *c) { return c ? c->t : -1; }
 
 int oracle_num_threads(void)

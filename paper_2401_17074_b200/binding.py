@@ -24,7 +24,7 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile
 SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
-           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order")
+           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics")
 
 
 class InletParams(C.Structure):
@@ -68,6 +68,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_get_moments.argtypes = [vp, vp, vp]
     lib.tslb_get_moments_host.argtypes = [vp, vp, vp]
     lib.tslb_diagnostics.argtypes = [vp, vp, vp]
+    lib.tslb_plane_statistics.argtypes = [vp, ip, vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
@@ -211,6 +212,18 @@ class TSLB:
         out = torch.empty(5, dtype=torch.float64, device="cuda")
         self._chk(self._lib.tslb_diagnostics(self._h, C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "tslb_diagnostics")
         return out
+
+    def plane_statistics(self, axis: int, sums=None, stream=None):
+        """Add one sample of the plane sums (1, u, uu, uuu; Eq. 24-25) along `axis` to sums[13][n_axis] (CUDA fp64)."""
+        import torch
+        n_axis = self.shape[2 - axis]
+        if sums is None:
+            sums = torch.zeros((13, n_axis), dtype=torch.float64, device="cuda")
+        if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == (13, n_axis)):
+            raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
+        self._chk(self._lib.tslb_plane_statistics(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
+                  "tslb_plane_statistics")
+        return sums
 
     def set_timing(self, max_launches: int):
         self._chk(self._lib.tslb_set_timing(self._h, int(max_launches)), "tslb_set_timing")

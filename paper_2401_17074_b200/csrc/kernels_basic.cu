@@ -373,6 +373,58 @@ __global__ void diag_final_kernel(const double *__restrict__ partial, int nblock
     if (lane == 0) out5[k] = v;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Plane statistics (PAPER.md:236 Eq. 24, :242 Eq. 25): raw sums of 1, u, uu, uuu over every plane
+// of constant coordinate along `axis`.  Grid (n_axis, PARTS): each CTA reduces a share of one plane in fp64 (warp shuffles,
+// then a fixed-order pass over the warps), writes 13 partials; stats_final_kernel adds the PARTS partials of each plane
+// in a fixed order to the caller's running sums.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) stats_partial_kernel(const T *__restrict__ A, Layout L, int axis, double *__restrict__ partial)
+{
+    const int j = blockIdx.x, part = blockIdx.y, nparts = gridDim.y;
+    const int n[3] = {L.nx, L.ny, L.nz};
+    const int a = (axis == 0) ? 1 : 0;              // fastest in-plane axis
+    const int b = (axis == 2) ? 1 : 2;
+    const long long cnt = (long long)n[a] * n[b];
+    double acc[TSLB_STAT_ROWS];
+#pragma unroll
+    for (int k = 0; k < TSLB_STAT_ROWS; ++k) acc[k] = 0.0;
+    for (long long i = (long long)part * blockDim.x + threadIdx.x; i < cnt; i += (long long)nparts * blockDim.x) {
+        int q[3];
+        q[axis] = j; q[a] = (int)(i % n[a]); q[b] = (int)(i / n[a]);
+        const long long idx = lay_idx(L, q[0], q[1], q[2]);
+        const double ux = A[L.field + idx], uy = A[2 * L.field + idx], uz = A[3 * L.field + idx];
+        acc[0] += 1.0;
+        acc[1] += ux; acc[2] += uy; acc[3] += uz;
+        acc[4] += ux * ux; acc[5] += uy * uy; acc[6] += uz * uz;
+        acc[7] += ux * uy; acc[8] += ux * uz; acc[9] += uy * uz;
+        acc[10] += ux * ux * ux; acc[11] += uy * uy * uy; acc[12] += uz * uz * uz;
+    }
+    __shared__ double sh[TSLB_STAT_ROWS][8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < TSLB_STAT_ROWS; ++k) {
+        const double v = warp_sum(acc[k]);
+        if (lane == 0) sh[k][wid] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < TSLB_STAT_ROWS) {
+        double v = 0;
+        for (int w = 0; w < 8; ++w) v += sh[threadIdx.x][w];
+        partial[((long long)threadIdx.x * gridDim.x + j) * nparts + part] = v;
+    }
+}
+
+__global__ void stats_final_kernel(const double *__restrict__ partial, int n_axis, int nparts, double *__restrict__ sums)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;     // over 13 * n_axis
+    if (i >= TSLB_STAT_ROWS * n_axis) return;
+    double v = 0;
+    for (int p = 0; p < nparts; ++p) v += partial[(long long)i * nparts + p];
+    sums[i] += v;
+}
+
 template <typename T>
 SweepParams<T> make_params(const tslb_ctx *c)
 {
@@ -462,6 +514,18 @@ cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st)
     else
         diag_partial_kernel<double><<<TSLB_DIAG_BLOCKS, TSLB_DIAG_THREADS, 0, st>>>((const double *)c->buf[c->cur], make_fill(c), c->scratch);
     diag_final_kernel<<<1, 160, 0, st>>>(c->scratch, TSLB_DIAG_BLOCKS, dev_out5);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st)
+{
+    const int na = axis == 0 ? c->nx : (axis == 1 ? c->ny : c->nz);
+    dim3 grid(na, TSLB_STAT_PARTS);
+    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, c->scratch);
+    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, c->scratch);
+    const int tot = TSLB_STAT_ROWS * na;
+    stats_final_kernel<<<(tot + 127) / 128, 128, 0, st>>>(c->scratch, na, TSLB_STAT_PARTS, dev_sums);
     c->launches += 2;
     return cudaGetLastError();
 }

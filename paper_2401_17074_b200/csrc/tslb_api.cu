@@ -25,6 +25,16 @@ int cuda_fail(tslb_ctx *c, const char *what, cudaError_t e)
 
 size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// scratch: per-CTA partials of the diagnostics or of the plane statistics (whichever is larger)
+size_t scratch_bytes(const tslb_ctx *c)
+{
+    int nmax = c->nx > c->ny ? c->nx : c->ny;
+    if (c->nz > nmax) nmax = c->nz;
+    size_t a = 5 * TSLB_DIAG_BLOCKS * sizeof(double);
+    size_t b = (size_t)TSLB_STAT_ROWS * TSLB_STAT_PARTS * nmax * sizeof(double);
+    return ((a > b ? a : b) + 255) & ~(size_t)255;
+}
+
 size_t buffer_bytes(const tslb_ctx *c) { return align256((size_t)TSLB_NF * (size_t)c->L.field * tslb_elem(c)); }
 
 // padded internal layout (tslb_internal.h): one ghost layer on every side, 16-byte rows, never smaller than a TMA box
@@ -164,7 +174,7 @@ int tslb_get_timing(tslb_ctx *c, int *n_launches, double *total_ms)
 size_t tslb_workspace_bytes(const tslb_ctx *c)
 {
     if (!c) return 0;
-    return 2 * buffer_bytes(c) + align256(5 * TSLB_DIAG_BLOCKS * sizeof(double));
+    return 2 * buffer_bytes(c) + scratch_bytes(c);
 }
 
 int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
@@ -343,6 +353,20 @@ int tslb_diagnostics(tslb_ctx *c, double *dev_out5, void *stream)
     if (!dev_out5) return fail(c, TSLB_EINVAL, "dev_out5 == NULL");
     cudaError_t e = tslb_launch_diag(c, dev_out5, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, "diagnostics kernels", e);
+    return TSLB_OK;
+}
+
+int tslb_plane_statistics(tslb_ctx *c, int axis, double *dev_sums, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (axis < 0 || axis > 2) return fail(c, TSLB_EINVAL, "axis must be 0, 1 or 2");
+    if (!dev_sums) return fail(c, TSLB_EINVAL, "dev_sums == NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = refresh_boundary(c, false, st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_plane_stats(c, axis, dev_sums, st);
+    if (e != cudaSuccess) return cuda_fail(c, "plane statistics kernels", e);
     return TSLB_OK;
 }
 

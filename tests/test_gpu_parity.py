@@ -252,6 +252,44 @@ def test_order2_config1_reduced(B, oracle_mod):
 
 
 # ---------------------------------------------------------------------------------------------
+# plane statistics (Eq. 24-25 raw sums, tslb_plane_statistics): SURVEY.md 8(f) rank 1
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_plane_statistics_match_oracle(B, oracle_mod, dtype):
+    import torch
+    for w, axis in ((W.channel(40, 24, 18, steps=30, dtype=dtype), 1), (W.jet(16, 20, 24, steps=30, dtype=dtype, D=5.0), 2),
+                    (W.config1(n=24, steps=30, dtype=dtype), 0)):
+        o = make_oracle(oracle_mod, w); sim = make_gpu(w, B.KERNEL_AUTO)
+        n_axis = (w.nx, w.ny, w.nz)[axis]
+        So = np.zeros((13, n_axis)); Sg = None
+        for _ in range(3):                                # three samples, 10 steps apart
+            o.step(10); sim.step(10)
+            o.plane_statistics(axis, So); Sg = sim.plane_statistics(axis, Sg)
+        torch.cuda.synchronize()
+        G = Sg.cpu().numpy()
+        tol = 1e-12 if dtype == "f64" else 2e-5
+        # a plane sum of u^k is compared relative to (number of samples in the sum) x max|u|^k (the sums themselves may cancel)
+        umax = np.abs(o.get_moments()[1:4]).max()
+        power = np.array([0, 1, 1, 1, 2, 2, 2, 2, 2, 2, 3, 3, 3])[:, None]
+        scale = So[0].max() * umax ** power
+        assert np.array_equal(G[0], So[0])                # sample counts are exact
+        assert (np.abs(G - So) / scale).max() < tol, (w.name, (np.abs(G - So) / scale).max())
+        # fixed-order reduction: a second context gives the same bits
+        sim2 = make_gpu(w, B.KERNEL_AUTO); S2 = None
+        for _ in range(3):
+            sim2.step(10); S2 = sim2.plane_statistics(axis, S2)
+        assert torch.equal(Sg, S2)
+        # Reynolds stress <u'x u'y> and variance from the raw sums against numpy on the GPU state itself
+        M = gpu_state(sim)
+        one = sim.plane_statistics(axis).cpu().numpy()
+        ax_np = {0: (0, 1), 1: (0, 2), 2: (1, 2)}[axis]   # axes of [nz][ny][nx] to average over
+        mean = one[1:4] / one[0]
+        var = one[4:7] / one[0] - mean**2
+        assert np.abs(var - M[1:4].var(axis=tuple(a + 1 for a in ax_np))).max() < 1e-9
+        sim.close(); sim2.close()
+
+
+# ---------------------------------------------------------------------------------------------
 # library behaviour on the device
 # ---------------------------------------------------------------------------------------------
 def test_checkpoint_resume(B):

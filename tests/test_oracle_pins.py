@@ -539,3 +539,41 @@ def test_order2_brute_vs_closed_and_decay(oracle_mod):
     assert abs(nu_eff / nu - 1) < 0.02
     with pytest.raises(RuntimeError):
         o.set_order(4)
+
+
+# ---------------------------------------------------------------------------------------------
+# Plane statistics (Eq. 24-25 raw sums).  SURVEY.md 8(f) rank 1.
+# ---------------------------------------------------------------------------------------------
+def test_plane_statistics_closed_forms(oracle_mod):
+    """Taylor-Green field u = U0 (sinX cosY cosZ, -cosX sinY cosZ, 0): over a plane of constant y the sums have closed
+    forms (sum of sin^2 or cos^2 over a full period of n >= 3 nodes is n/2, odd powers and mixed products vanish)."""
+    n, U0 = 16, 0.01
+    w = W.config0(n=n, steps=0)
+    o = oracle_mod.Oracle(n, n, n, w.tau); o.set_moments(w.moments)
+    S = np.zeros((13, n)); o.plane_statistics(1, S)
+    Y = 2 * np.pi * np.arange(n) / n
+    assert np.abs(S[0] - n * n).max() == 0
+    assert np.abs(S[1:4]).max() < 1e-15 and np.abs(S[10:13]).max() < 1e-16          # odd moments vanish
+    assert np.abs(S[4] - U0**2 * np.cos(Y)**2 * n * n / 4).max() < 1e-16
+    assert np.abs(S[5] - U0**2 * np.sin(Y)**2 * n * n / 4).max() < 1e-16
+    assert np.abs(S[6]).max() == 0 and np.abs(S[7:10]).max() < 1e-17
+    # along x the roles change: sum over (y,z) of u_x^2 = U0^2 sin^2 X n^2/4; two samples accumulate
+    S = np.zeros((13, n)); o.plane_statistics(0, S); o.plane_statistics(0, S)
+    assert np.abs(S[4] - 2 * U0**2 * np.sin(Y)**2 * n * n / 4).max() < 1e-16 and np.abs(S[0] - 2 * n * n).max() == 0
+
+
+def test_plane_statistics_vs_numpy_central_moments(oracle_mod):
+    """Reynolds stresses and skewness derived from the raw sums equal numpy's central moments of the same field."""
+    w = W.random_state(7, 9, 5, seed=21)
+    o = oracle_mod.Oracle(7, 9, 5, w.tau); o.set_moments(w.moments)
+    S = np.zeros((13, 9)); o.plane_statistics(1, S)
+    u = w.moments[1:4]                                  # [3][nz][ny][nx]
+    mean = S[1:4] / S[0]
+    assert np.abs(mean - u.mean(axis=(1, 3))).max() < 1e-15
+    var = S[4:7] / S[0] - mean**2
+    assert np.abs(var - u.var(axis=(1, 3))).max() < 1e-15
+    rxy = S[7] / S[0] - mean[0] * mean[1]
+    up = u - u.mean(axis=(1, 3), keepdims=True)
+    assert np.abs(rxy - (up[0] * up[1]).mean(axis=(0, 2))).max() < 1e-15
+    m3 = S[10:13] / S[0] - 3 * mean * S[4:7] / S[0] + 2 * mean**3
+    assert np.abs(m3 - (up**3).mean(axis=(1, 3))).max() < 1e-16
