@@ -31,7 +31,11 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): moment reproduction (orders 0-3), uniform-flow
  * fixed point, equivalence with a two-lattice population code, mass conservation, Taylor-Green
  * viscous decay, forced Poiseuille curvature, shear stress Pi_xy = -(tau/3) rho du/dy, lattice
- * symmetries, brute-vs-closed.  Inlet/outlet physics (readings A13-A16): PARITY UNPINNED.
+ * symmetries, brute-vs-closed; open faces: the populations pulled from inlet / outlet nodes equal Eq. 23 as printed
+ * (built with independent numpy Hermite tensors, two time levels), uniform through-flow is a fixed point; diagnostics
+ * equal the plain numpy sums.  Still PARITY UNPINNED (readings, nothing in the paper or the mathematics fixes them):
+ * A13's nozzle geometry (top-hat disc on a full inlet plane), A14's noise law (uniform, relative) and A16's clamp rule
+ * where several open faces meet.
  *
  * Layout of every moment array: [10][nz][ny][nx] doubles, x fastest;
  * field order rho, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz  (Pi = non-equilibrium momentum flux).

@@ -409,6 +409,121 @@ def test_ghost_fill_definition(oracle_mod):
     np.testing.assert_array_equal(R[4:, 0, :, 2], M[4:, 1, :, 2])                 # Pi from x_F
 
 
+def _fstar_all(p, M):
+    """Post-collision populations f* = f_eq + (1-w) f_neq (+ force) of every node from its moments M[10,nz,ny,nx],
+    with the independent numpy tensors of PopulationLB (Eq. 5, 14, 17)."""
+    rho, u = M[0], M[1:4]
+    Pi = np.array([[M[4], M[7], M[8]], [M[7], M[5], M[9]], [M[8], M[9], M[6]]])
+    wb = p.w.reshape(-1, 1, 1, 1)
+    cg = (p.cf @ p.g).reshape(-1, 1, 1, 1)
+    return p.feq(rho, u) + (1 - p.omega) * p.fneq_reg(Pi, u) + wb * rho[None] * cg / CS2
+
+
+def _pull_plane(p, src_by_cz):
+    """Moments of one z-plane (x, y periodic) from the populations arriving from the planes below (c_z = +1), at
+    (c_z = 0) and above (c_z = -1): src_by_cz[cz][i] is population i on the source plane.  Eq. 6 + Eq. 12."""
+    arr = np.stack([np.roll(src_by_cz[cz][i], shift=(cy, cx), axis=(0, 1)) for i, (cx, cy, cz) in enumerate(DIRS)])
+    R = arr.sum(0)
+    J = np.einsum("ia,i...->a...", p.cf, arr)
+    S = np.einsum("ia,ib,i...->ab...", p.cf, p.cf, arr)
+    u = J / R
+    Pi = S - R * (CS2 * np.eye(3)[:, :, None, None] + np.einsum("a...,b...->ab...", u, u))
+    return np.stack([R, u[0], u[1], u[2], Pi[0, 0], Pi[1, 1], Pi[2, 2], Pi[0, 1], Pi[0, 2], Pi[1, 2]])
+
+
+def test_inlet_and_outlet_populations_are_eq23_as_printed(oracle_mod):
+    """PAPER.md:181-196 (Eq. 22-23), :202: the population an interior node pulls from a velocity-inlet node is
+    f_eq(rho_B, u_B) + (1 - omega) f_neq(Pi(x_F), u_B), with u_B imposed, rho_B and Pi taken from the fluid neighbour
+    x_F AT THE CURRENT TIME LEVEL (readings A13, A15); from a zero-gradient outlet node it is the post-collision
+    population of x_F's own moments.  Built here with the independent numpy Hermite tensors and compared with the
+    oracle's first interior planes over two steps (the second step fixes the time level of the fill).
+    Mutations that fail: rho or Pi of the boundary node's own old value instead of x_F's; u copied instead of imposed;
+    x_F taken at the previous time level."""
+    nx, ny, nz, tau = 6, 5, 7, 0.63
+    w = W.random_state(nx, ny, nz, seed=41, tau=tau)
+    up = np.random.default_rng(7).uniform(-0.03, 0.03, (3, ny, nx))
+    o = oracle_mod.Oracle(nx, ny, nz, tau)
+    o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.0, 3, 0)
+    o.set_face(W.FACE_ZHI, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_moments(w.moments)
+    p = PopulationLB(w.moments, tau, (0.0, 0.0, 0.0))
+    Pi_at = lambda M, z: np.array([[M[4, z], M[7, z], M[8, z]], [M[7, z], M[5, z], M[9, z]], [M[8, z], M[9, z], M[6, z]]])
+    M_prev = None
+    M = w.moments.copy()
+    for step in range(2):
+        post = _fstar_all(p, M)
+        # inlet node x_B = (x, y, 0), x_F = (x, y, 1): Eq. 23 as printed
+        fB = p.feq(M[0, 1], up) + (1 - p.omega) * p.fneq_reg(Pi_at(M, 1), up)
+        want_lo = _pull_plane(p, {1: fB, 0: post[:, 1], -1: post[:, 2]})
+        # outlet node x_B = (x, y, nz-1), x_F = (x, y, nz-2): all ten moments of x_F
+        want_hi = _pull_plane(p, {1: post[:, nz - 3], 0: post[:, nz - 2], -1: post[:, nz - 2]})
+        o.step(1)
+        R = o.get_moments()
+        assert np.abs(R[:, 1] - want_lo).max() < 2e-15, step
+        assert np.abs(R[:, nz - 2] - want_hi).max() < 2e-15, step
+        # mutations
+        f_own = p.feq(M[0, 0], up) + (1 - p.omega) * p.fneq_reg(Pi_at(M, 0), up)          # boundary node's own rho, Pi
+        f_copy = p.feq(M[0, 1], M[1:4, 1]) + (1 - p.omega) * p.fneq_reg(Pi_at(M, 1), M[1:4, 1])   # u not imposed
+        # (get_moments returns the boundary nodes already refilled, so "own old value" is a mutation at step 0 only)
+        for bad in ((f_own, f_copy) if step == 0 else (f_copy,)):
+            assert np.abs(_pull_plane(p, {1: bad, 0: post[:, 1], -1: post[:, 2]}) - R[:, 1]).max() > 1e-5
+        if M_prev is not None:                                                                  # stale time level
+            f_stale = p.feq(M_prev[0, 1], up) + (1 - p.omega) * p.fneq_reg(Pi_at(M_prev, 1), up)
+            assert np.abs(_pull_plane(p, {1: f_stale, 0: post[:, 1], -1: post[:, 2]}) - R[:, 1]).max() > 1e-5
+        M_prev, M = M, R
+
+
+def test_uniform_through_flow_is_a_fixed_point(oracle_mod):
+    """A uniform state (rho0, u0, Pi = 0) entering through an inlet with u_in = u0 and leaving through zero-gradient
+    outlets on the five other faces is an exact fixed point of fill + sweep: every copy, every imposed value and every
+    pulled population reproduces it (Eq. 22-23 with a uniform neighbour; P3 for the interior)."""
+    nx, ny, nz = 5, 6, 7
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.03; M[1] = 0.01; M[2] = -0.02; M[3] = 0.04
+    up = np.empty((3, ny, nx)); up[0] = 0.01; up[1] = -0.02; up[2] = 0.04
+    o = oracle_mod.Oracle(nx, ny, nz, 0.56)
+    o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.0, 1, 0)
+    for f in (W.FACE_ZHI, W.FACE_XLO, W.FACE_XHI, W.FACE_YLO, W.FACE_YHI):
+        o.set_face(f, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_moments(M)
+    o.step(10)
+    assert np.abs(o.get_moments() - M).max() < 1e-15
+    # and it is the imposed velocity that holds it there: a different u_in moves the first interior plane
+    up2 = up.copy(); up2[2] = 0.05
+    o2 = oracle_mod.Oracle(nx, ny, nz, 0.56)
+    o2.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up2, 0.0, 1, 0)
+    for f in (W.FACE_ZHI, W.FACE_XLO, W.FACE_XHI, W.FACE_YLO, W.FACE_YHI):
+        o2.set_face(f, W.BC_OUTLET_ZERO_GRADIENT)
+    o2.set_moments(M); o2.step(1)
+    assert np.abs(o2.get_moments()[:, 1, 2, 2] - M[:, 1, 2, 2]).max() > 1e-4
+
+
+def test_diagnostics_are_the_plain_sums(oracle_mod):
+    """oracle_diagnostics (reading A26): mass = sum rho, momentum = sum rho u, kinetic energy = 1/2 sum rho |u|^2 over the
+    nodes that are not on an open face -- against numpy sums of get_moments(), without and with open faces.
+    Mutations that fail: a missing 1/2 or rho in the energy, u instead of rho u, open-face nodes included."""
+    w = W.random_state(7, 6, 5, seed=23)
+    for open_faces in ((), (W.FACE_ZLO, W.FACE_ZHI, W.FACE_XHI)):
+        o = oracle_mod.Oracle(7, 6, 5, 0.7)
+        for f in open_faces:
+            o.set_face(f, W.BC_OUTLET_ZERO_GRADIENT)
+        if open_faces:
+            o.set_face(W.FACE_XLO, W.BC_OUTLET_ZERO_GRADIENT)
+        o.set_moments(w.moments); o.step(2)
+        M = o.get_moments()
+        m = np.ones(M.shape[1:], dtype=bool)
+        if open_faces:
+            m[0] = m[-1] = False; m[:, :, 0] = m[:, :, -1] = False
+        rho, u = M[0][m], M[1:4][:, m]
+        want = np.array([rho.sum(), (rho * u[0]).sum(), (rho * u[1]).sum(), (rho * u[2]).sum(),
+                         0.5 * (rho * (u * u).sum(0)).sum()])
+        d = o.diagnostics()
+        np.testing.assert_allclose(d, want, rtol=1e-13, atol=1e-15)
+        assert abs(d[4] - (rho * (u * u).sum(0)).sum()) > 1e-3 * d[4]           # the 1/2 is there
+        assert abs(d[1] - u[0].sum()) > 1e-6                                     # rho u, not u
+        if open_faces:                                                           # the exclusion is exercised
+            assert abs(d[0] - M[0].sum()) > 1.0
+
+
 def test_inlet_noise_is_relative_and_reproducible(oracle_mod):
     w = W.jet(12, 12, 8, steps=1, dtype="f64", D=6.0)
     a = _mk(oracle_mod, w); b = _mk(oracle_mod, w)
