@@ -1,5 +1,5 @@
 // kernels_basic.cu -- the per-direction "gather" sweep (covers every boundary set and lattice shape),
-// the boundary-node fill, the ghost-layer (halo) refresh, layout import/export and the diagnostics reduction.  sm_100a.
+// the boundary-node fill, the ghost-column (halo) refresh, layout import/export and the diagnostics reduction.  sm_100a.
 //
 // Arithmetic follows PAPER.md:154 (Eq. 18) with the readings of DESIGN.md; contractions are reduced by
 // hand.  Internal storage is the SHIFTED form: field 0 holds drho = rho - 1
@@ -254,46 +254,24 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
 }
 
 // ---------------------------------------------------------------------------------------------
-// Ghost-layer refresh: every ghost cell (a coordinate equal to -1 or n) takes the
-// 10 moments of the interior node obtained by wrapping its coordinates on periodic axes and clamping
-// them on the others.  The TMA-staged sweep reads neighbours through these layers, so it carries no
-// wrap logic; ghost cells behind a wall or an open face are never used by a node that is advanced
-// (they only keep the staged tiles finite).  Launched after the boundary-node fill.
-// One thread per ghost cell of one of the three slab pairs: x slabs (full y,z extent incl. ghosts),
-// y slabs (x interior only), z slabs (x,y interior only) -- together every ghost cell exactly once.
+// Ghost-column refresh: the cells x = -1 and x = nx of every row take the 10 moments of the
+// node obtained by wrapping x on a periodic axis (clamping it otherwise).  The TMA-staged sweep reads its x neighbours
+// through these columns (a TMA row is contiguous and cannot wrap); it keeps them current itself, so this kernel runs
+// only after set_moments, a boundary change, a gather step, or a fill next to a periodic x axis.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void halo_kernel(T *__restrict__ M, FillParams p)
 {
     const Layout &L = p.L;
-    const long long nXs = 2LL * (L.ny + 2) * (L.nz + 2);   // x = -1 / nx, all y,z incl. ghosts
-    const long long nYs = 2LL * L.nx * (L.nz + 2);          // y = -1 / ny, x interior, all z incl. ghosts
-    const long long nZs = 2LL * L.nx * L.ny;                // z = -1 / nz, x,y interior
-    const long long tot = nXs + nYs + nZs;
+    const long long tot = 2LL * L.ny * L.nz;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += stride) {
-        int x, y, z;
-        if (i < nZs) {                       // z slabs first: rows are contiguous in x
-            const long long j = i >> 1;
-            z = (i & 1) ? L.nz : -1;
-            x = (int)(j % L.nx); y = (int)(j / L.nx);
-        } else if (i < nZs + nYs) {
-            const long long j = (i - nZs) >> 1;
-            y = ((i - nZs) & 1) ? L.ny : -1;
-            x = (int)(j % L.nx); z = (int)(j / L.nx) - 1;
-        } else {
-            const long long j = (i - nZs - nYs) >> 1;
-            x = ((i - nZs - nYs) & 1) ? L.nx : -1;
-            y = (int)(j % (L.ny + 2)) - 1; z = (int)(j / (L.ny + 2)) - 1;
-        }
-        const int n[3] = {L.nx, L.ny, L.nz};
-        int q[3] = {x, y, z};
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            if (q[a] < 0) q[a] = (p.kind[2 * a] == TSLB_BC_PERIODIC) ? n[a] - 1 : 0;
-            else if (q[a] >= n[a]) q[a] = (p.kind[2 * a + 1] == TSLB_BC_PERIODIC) ? 0 : n[a] - 1;
-        }
-        const long long ig = lay_idx(L, x, y, z), is = lay_idx(L, q[0], q[1], q[2]);
+        const long long j = i >> 1;
+        const int y = (int)(j % L.ny), z = (int)(j / L.ny);
+        const bool hi = i & 1;
+        const int x = hi ? L.nx : -1;
+        const int xs = hi ? (p.kind[1] == TSLB_BC_PERIODIC ? 0 : L.nx - 1) : (p.kind[0] == TSLB_BC_PERIODIC ? L.nx - 1 : 0);
+        const long long ig = lay_idx(L, x, y, z), is = lay_idx(L, xs, y, z);
 #pragma unroll
         for (int k = 0; k < TSLB_NF; ++k) M[k * L.field + ig] = M[k * L.field + is];
     }
@@ -484,7 +462,7 @@ cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st)
 
 cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st)
 {
-    const long long tot = 2LL * (c->ny + 2) * (c->nz + 2) + 2LL * c->nx * (c->nz + 2) + 2LL * c->nx * c->ny;
+    const long long tot = 2LL * c->ny * c->nz;
     long long blocks = (tot + 255) / 256;
     if (blocks > (long long)c->sm_count * 16) blocks = (long long)c->sm_count * 16;
     if (c->dtype == TSLB_F32) halo_kernel<float><<<(unsigned)blocks, 256, 0, st>>>((float *)buf, make_fill(c));

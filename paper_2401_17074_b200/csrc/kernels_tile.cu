@@ -8,18 +8,22 @@
 // With every field scaled by 216 (and the q = 2 fields by a further 2/3) all taps are the small integers
 // 1, 4, -2, so no rounded lattice weight ever multiplies the data.
 //
-// Data path: one CTA per SM owns a 60 x 14 column of nodes (fp32: 2 x 7 warps; fp64: 60 x 8,
-// 2 x 4 warps) and marches along z.  One elected thread streams the z-planes of the 10 moment fields, 64 x 16 nodes
-// each (the tile plus a 1-node halo, rows 16-byte aligned), from the padded SoA buffer into a 4-deep shared-memory
-// ring with TMA (cp.async.bulk.tensor.4d, mbarrier complete_tx); ghost layers in the buffer stand for the periodic
-// images, so the kernel has no wrap logic, and it keeps them current itself by storing the images of the nodes it
-// writes on periodic faces.  Every warp owns 2 rows (packed in a 2-wide register pair so fp32 issues as FFMA2/FADD2)
-// x 32 columns (30 outputs + 2 halo lanes):
-//   y pass: in registers, from the A_k of rows r0-1 .. r0+2 read from shared memory (packs (r0,r0+1) and (r0-1,r0+2)),
-//   x pass: neighbours' values by warp shuffles (one combination up, one down per group),
-//   z pass: by marching -- 15 running pairs per thread, no plane is staged twice.
-// Each node's moments leave HBM once per tile (halo re-reads hit L2) and the 10 new moments are written once:
-// 80 B (fp32) / 160 B (fp64) of compulsory traffic per node update.
+// Data path.  One CTA per SM owns a 60 x 14 column of nodes (fp32: 2 x 7 "main" warps; fp64:
+// 60 x 8, 2 x 4) and marches along z.  Warp roles:
+//   main warps   2 rows (packed in a 2-wide register pair, so fp32 issues as FFMA2/FADD2) x 32 columns (30 outputs + 2
+//                halo lanes).  Per source plane: Hermite coefficients of the OWN two rows only; the y pass needs, from
+//                the row below, P = phi0+phi1+phi2 and, from the row above, M = phi0-phi1+phi2 of 8 coefficient groups:
+//                every warp publishes these two combinations of its rows in shared memory and reads its neighbours'
+//                (per-row-pair mbarriers, double-buffered: no CTA-wide barrier anywhere in the plane loop);
+//                x pass by warp shuffles; z pass by marching (15 running pairs per thread).
+//   halo warps   2 warps: the rows just below and above the tile (Hermite coefficients + the published combinations
+//                only).  Lane 0 of the first is the TMA PRODUCER (3-stage ring of source planes: the 14 tile rows and
+//                the two halo rows as three boxes, y and z wrapped by coordinate, walls / open faces by out-of-bounds
+//                zero fill; full/empty mbarriers, a stage is released as soon as its values sit in registers).
+//                Lane 0 of the second is the STORE thread: the finished 60 x 14 x 10 output tile is staged in shared
+//                memory and written with one TMA store (cp.async.bulk.tensor shared -> global, SASS UTMASTG).
+// Each node's moments leave HBM once per tile (halo re-reads hit L2) and the 10 new moments are written once, in full
+// rows: 80 B (fp32) / 160 B (fp64) of compulsory traffic per node update.
 //
 // INCREMENT FORM: the base 3 u_a of the first-order coefficients never enters the
 // passes.  A pass with taps (t-, t0, t+) applied to B*u gives (t- + t0 + t+) B u(x) + B [t- (u(x-1) - u(x)) + t+ (u(x+1) - u(x))];
@@ -37,17 +41,10 @@ template <> struct PackOf<double> { typedef D2 type; };
 
 __device__ __forceinline__ float2 pk(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ D2 pk(double a, double b) { D2 r; r.x = a; r.y = b; return r; }
-#ifndef TSLB_SCALAR_F32
 __device__ __forceinline__ float2 padd(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 pmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 psub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
-#else
-__device__ __forceinline__ float2 padd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return make_float2(a.x * b.x, a.y * b.y); }
-__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
-__device__ __forceinline__ float2 psub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-#endif
 __device__ __forceinline__ D2 padd(D2 a, D2 b) { return pk(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ D2 pmul(D2 a, D2 b) { return pk(a.x * b.x, a.y * b.y); }
 __device__ __forceinline__ D2 pfma(D2 a, D2 b, D2 c) { return pk(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
@@ -56,6 +53,7 @@ template <typename P, typename T> __device__ __forceinline__ P pbc(T s) { return
 // a*s + c and a*s with a scalar s
 template <typename P, typename T> __device__ __forceinline__ P pfmas(P a, T s, P c) { return pfma(a, pbc<P, T>(s), c); }
 template <typename P, typename T> __device__ __forceinline__ P pmuls(P a, T s) { return pmul(a, pbc<P, T>(s)); }
+template <typename P> __device__ __forceinline__ P pswap(P a) { return pk(a.y, a.x); }
 
 template <typename P> __device__ __forceinline__ P shfl_up1(P v)
 {
@@ -66,17 +64,25 @@ template <typename P> __device__ __forceinline__ P shfl_dn1(P v)
     return pk(__shfl_down_sync(0xffffffffu, v.x, 1), __shfl_down_sync(0xffffffffu, v.y, 1));
 }
 
-// ---- TMA / mbarrier (PTX; SASS: UTMALDG, SYNCS) ----------------------------------------------------------
+// ---- TMA / mbarrier / shared memory by 32-bit shared address (PTX; SASS: UTMALDG, UTMASTG, SYNCS, LDS, STS) ------------
+// Every shared-memory access of the kernel goes through a 32-bit shared-window address held in a register plus an
+// immediate: the addresses are formed once before the plane loop (keep(): an empty asm the compiler cannot
+// rematerialise through), so the loop carries no address arithmetic beyond the stage / slot offsets.
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+__device__ __forceinline__ uint32_t keep(uint32_t v) { asm volatile("" : "+r"(v)); return v; }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     asm volatile(
         "{\n"
@@ -86,14 +92,43 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+        "}" ::"r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3)
+// one warp signals: every lane's earlier shared-memory accesses are ordered before the arrive of lane 0
+__device__ __forceinline__ void warp_arrive(uint32_t bar, int lane)
+{
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar);
+}
+__device__ __forceinline__ float lds(uint32_t a, float)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds(uint32_t a, double)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void sts(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2, int c3)
 {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+__device__ __forceinline__ void tma_store_4d(uint32_t src, const CUtensorMap *map, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
+                 ::"l"(map), "r"(src), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <typename T>
 struct TileParams {
@@ -159,401 +194,533 @@ __device__ __forceinline__ void hermite_round(const P (&raw)[TSLB_NF], T beta, c
     }
 }
 
-// ---- one 1-D pass on a group of up to three fields q = 0,1,2 given S_q = phi(-1)+phi(+1), D_q = phi(-1)-phi(+1)
-//      and the centre values c0, c2:      out0 = E + 4 c0 - 2 c2,  out1 = D0 + S1 + D2,  out2 = E = S0 + D1 + S2
-template <int NQ, typename P, typename T>
-__device__ __forceinline__ void pass_group(const P (&S)[3], const P (&D)[3], P c0, P c2, P &o0, P &o1, P &o2)
+// The y-pass combinations of one pack (rows .x, .y) for the coefficient group (kx, kz), from A[kx][ky]:
+//   t = A0 + A2,   qc = t + A1*sgn = (P of row .x, M of row .y)   -- what the pack's own rows exchange with each other
+//                  qp = t - A1*sgn = (M of row .x, P of row .y)   -- what the rows outside the pack need: PUBLISHED
+//   cen = 4 A0 - 2 A2                                              -- the centre taps
+// with P = phi0 + phi1 + phi2 (goes up, c_y = +1), M = phi0 - phi1 + phi2 (goes down), sgn = (1, -1).
+template <int ORDER, int KX, int KZ, typename P, typename T>
+__device__ __forceinline__ void ycombos(const P (&A)[3][3], P &qc, P &qp, P &cen)
 {
-    P E = S[0];
-    P O = D[0];
-    if (NQ >= 2) { E = padd(E, D[1]); O = padd(O, S[1]); }
-    if (NQ >= 3) { E = padd(E, S[2]); O = padd(O, D[2]); }
-    o2 = E;
-    o1 = O;
-    o0 = pfmas(c0, (T)4, E);
-    if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
-}
-
-// The same pass for the y stage, where the rows are packed (centre, halo): W_q = D_q * sgn with sgn = (1,-1).
-template <int NQ, typename P, typename T>
-__device__ __forceinline__ void pass_group_y(const P (&S)[3], const P (&W)[3], P c0, P c2, P sgn, P &o0, P &o1, P &o2)
-{
-    P E, O;
-    if (NQ == 1) { E = S[0]; O = pmul(W[0], sgn); }
-    if (NQ == 2) { E = pfma(W[1], sgn, S[0]); O = pfma(W[0], sgn, S[1]); }
-    if (NQ == 3) { E = pfma(W[1], sgn, padd(S[0], S[2])); O = pfma(padd(W[0], W[2]), sgn, S[1]); }
-    o2 = E;
-    o1 = O;
-    o0 = pfmas(c0, (T)4, E);
-    if (NQ >= 3) o0 = pfmas(c2, (T)-2, o0);
-}
-
-// Periodic ghost images of the two rows of a pack (rare path).  eflags: bit 0 = column on a periodic x face,
-// bits 1/2 = row r0 / r0+1 on a periodic y face, bit 3 = plane on a periodic z face.
-template <typename P, typename T>
-__device__ __forceinline__ void store_images(const P (&o)[TSLB_NF], T *__restrict__ Bbuf, long long N, long long i0, long long i1, bool row1,
-                                          int eflags, const Layout &L, int col, int r0, int zt)
-{
-    const long long xi = col == 0 ? (long long)L.nx : -(long long)L.nx;
-    const long long zi = zt == 0 ? (long long)L.nz * L.plane : -(long long)L.nz * L.plane;
-    const long long ywrap = (long long)L.ny * L.px;
-    const long long yi0 = r0 == 0 ? ywrap : -ywrap, yi1 = -ywrap;
-    const bool ex = eflags & 1, ey0 = eflags & 2, ey1 = (eflags & 4) && row1, ez = eflags & 8;
-    T *b0 = Bbuf + i0, *b1 = Bbuf + i1;
-#define TSLB_PUT0(off) _Pragma("unroll") for (int f = 0; f < TSLB_NF; ++f) b0[f * N + (off)] = o[f].x;
-#define TSLB_PUT1(off) _Pragma("unroll") for (int f = 0; f < TSLB_NF; ++f) b1[f * N + (off)] = o[f].y;
-    if (ex) { TSLB_PUT0(xi) if (row1) { TSLB_PUT1(xi) } }
-    if (ey0) { TSLB_PUT0(yi0) if (ex) { TSLB_PUT0(yi0 + xi) } }
-    if (ey1) { TSLB_PUT1(yi1) if (ex) { TSLB_PUT1(yi1 + xi) } }
-    if (ez) {
-        TSLB_PUT0(zi) if (row1) { TSLB_PUT1(zi) }
-        if (ex) { TSLB_PUT0(zi + xi) if (row1) { TSLB_PUT1(zi + xi) } }
-        if (ey0) { TSLB_PUT0(zi + yi0) if (ex) { TSLB_PUT0(zi + yi0 + xi) } }
-        if (ey1) { TSLB_PUT1(zi + yi1) if (ex) { TSLB_PUT1(zi + yi1 + xi) } }
-    }
-#undef TSLB_PUT0
-#undef TSLB_PUT1
-}
-
-// finalise the two rows of a pack from their 216-scaled raw moments (m[1..3] lack their base 216 u) and store (Eq. 12)
-template <typename P, typename T>
-__device__ __forceinline__ void finalize_store(const P (&m)[TSLB_NF], const P (&uo)[3], T *__restrict__ Bbuf, long long N, long long i0,
-                                               long long i1, bool row1, int eflags, const Layout &L, int col, int r0, int zt)
-{
-    // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
-    const T hi = (T)(1.0 / 216.0);
-    const T lo = (T)(1.0 / 216.0 - (double)hi);
-    const P dR = pfmas(m[0], lo, pmuls(m[0], hi));
-    const P rho = padd(pbc<P, T>((T)1), dR);
-    const P den = padd(pbc<P, T>((T)216), m[0]);
-    const P inv = pk((T)1 / den.x, (T)1 / den.y);
-    const P nm0 = pmuls(m[0], (T)-1);
-    // u' = (216 u + J) / (216 + dR216) = u + (J - u dR216) / (216 + dR216)
-    P o[TSLB_NF];
-    o[0] = dR;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) o[1 + a] = pfma(pfma(uo[a], nm0, m[1 + a]), inv, uo[a]);
-    const P niso = pmuls(dR, (T)(-1.0 / 3.0));
-    const P nrho = pmuls(rho, (T)-1);
-    const P rx = pmul(nrho, o[1]), ry = pmul(nrho, o[2]), rz = pmul(nrho, o[3]);
-    // (the second moments are rebuilt from scratch every step, so a singly rounded 1/216 cannot compound there)
-    o[4] = pfma(rx, o[1], pfmas(m[4], hi, niso));
-    o[5] = pfma(ry, o[2], pfmas(m[5], hi, niso));
-    o[6] = pfma(rz, o[3], pfmas(m[6], hi, niso));
-    o[7] = pfma(rx, o[2], pmuls(m[7], hi));
-    o[8] = pfma(rx, o[3], pmuls(m[8], hi));
-    o[9] = pfma(ry, o[3], pmuls(m[9], hi));
-#pragma unroll
-    for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i0] = o[f].x;
-    if (row1) {
-#pragma unroll
-        for (int f = 0; f < TSLB_NF; ++f) Bbuf[f * N + i1] = o[f].y;
-    }
-    // periodic images: a node on a periodic face is also the ghost cell beyond the opposite face (and the edge /
-    // corner ghosts when it lies on several), so the next sweep needs no separate ghost-layer refresh
-    if (eflags) store_images<P, T>(o, Bbuf, N, i0, i1, row1, eflags, L, col, r0, zt);
+    const P sgn = pk((T)1, (T)-1), nsg = pk((T)-1, (T)1);
+    const P a0 = A[KX][0];
+    P t = a0;
+    cen = pmuls(a0, (T)4);
+    if (kvalid<ORDER>(KX, 2, KZ)) { t = padd(a0, A[KX][2]); cen = pfmas(A[KX][2], (T)-2, cen); }
+    qc = t; qp = t;
+    if (kvalid<ORDER>(KX, 1, KZ)) { qc = pfma(A[KX][1], sgn, t); qp = pfma(A[KX][1], nsg, t); }
 }
 
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
 __host__ __device__ constexpr int gidx(int px, int py) { return py == 0 ? px : (py == 1 ? 3 + px : 5); }
+// index of the coefficient group (kx, kz) among the 8 exchanged ones
+__host__ __device__ constexpr int qidx(int kx, int kz) { return kz * 3 + kx; }
 
-// CTA geometry per dtype: WX x WY warps, each 30 output columns x 2 rows; one CTA per SM (the CTAs of an SM then
-// march in lock-step, which keeps the halo re-reads of neighbouring tiles inside L2 -- DESIGN.md "Tile kernel").
-// TMA needs the byte offset of the box origin along x to be a multiple of 16 (measured on B200: an origin at a
-// multiple of 2 floats raises "illegal instruction"): the box starts at the CTA's first column rounded down to ALIGN
-// elements and lanes read at the remaining offset (0 for WX = 2).
+// ---- CTA geometry -------------------------------------------------------------------------------------------------
+// WX x WY main warps, each 30 output columns x 2 rows, + 2 halo warps; one CTA per SM (the CTAs of an SM then march in
+// lock-step, which keeps the halo re-reads of neighbouring tiles inside L2).  TMA needs the byte offset of a box origin
+// along x to be a multiple of 16 (measured on B200: an origin at a multiple of 2 floats raises "illegal instruction"):
+// the source box starts XPAD = 4 columns left of the tile (the layout puts node x = 0 on a 16-byte boundary).
 template <typename T> struct TileGeom;
 #ifndef TILE_F32_WY
 #define TILE_F32_WY 7
 #endif
 #ifndef TILE_F32_NS
-#define TILE_F32_NS 4
+#define TILE_F32_NS 3
 #endif
-#ifndef TILE_F32_WX
-#define TILE_F32_WX 2
-#endif
-#ifndef TILE_F32_MINB
-#define TILE_F32_MINB 1
-#endif
-template <> struct TileGeom<float> { static constexpr int WX = TILE_F32_WX, WY = TILE_F32_WY, NS = TILE_F32_NS, ALIGN = 4, MINB = TILE_F32_MINB; };
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 4, ALIGN = 2, MINB = 1; };
+template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS; };
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2; };
+constexpr int rup128(int bytes) { return (bytes + 127) / 128 * 128; }
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;
-    static constexpr int WARPS = G::WX * G::WY;
-    static constexpr int COLS = TILE_COLS * G::WX;                                   // output columns per CTA
-    static constexpr int ROWS = 2 * G::WY;                                           // output rows per CTA
-    static constexpr int BY = ROWS + 2;                                              // box height
-    static constexpr int MAXOFF = (COLS % G::ALIGN) ? 2 : 0;
-    static constexpr int BXW = (COLS + 2 + MAXOFF + 3) / 4 * 4;                      // box width = smem row pitch
-    static constexpr int BOX_ELEMS = TSLB_NF * BY * BXW;
-    static constexpr int STAGE_ELEMS = (int)(((BOX_ELEMS * sizeof(T) + 127) / 128 * 128) / sizeof(T));
-    static constexpr int SMEM_BYTES = G::NS * STAGE_ELEMS * (int)sizeof(T);
+    static constexpr int WX = G::WX, WY = G::WY, NS = G::NS;
+    static constexpr int NMAIN = WX * WY, NHALO = 2, WARPS = NMAIN + NHALO, THREADS = WARPS * 32;
+    // one CTA per SM: the whole register file, 16384 registers per SM sub-partition, warps dealt round-robin to the four
+    static constexpr int MAXREG = (16384 / (((WARPS + 3) / 4) * 32)) / 8 * 8;     // 128 (fp32, 16 warps), 168 (fp64, 10 warps)
+    static constexpr int COLS = TILE_COLS * WX;                  // output columns per CTA (60)
+    static constexpr int ROWS = 2 * WY;                          // output rows per CTA
+    static constexpr int XPAD = 4;                               // box origin = first tile column - XPAD
+    static constexpr int BXW = COLS + 2 * XPAD;                  // box width (68): tile columns -4 .. 63
+    static constexpr int FS = ROWS * BXW;                        // field stride inside the main region [10][ROWS][BXW]
+    static constexpr int MAIN_ELEMS = rup128(TSLB_NF * FS * (int)sizeof(T)) / (int)sizeof(T);
+    static constexpr int HALO_ELEMS = rup128(TSLB_NF * BXW * (int)sizeof(T)) / (int)sizeof(T);   // one row [10][BXW]
+    static constexpr int STAGE_ELEMS = MAIN_ELEMS + 2 * HALO_ELEMS;                               // main | row -1 | row ROWS
+    static constexpr int STAGE_TX = (TSLB_NF * FS + 2 * TSLB_NF * BXW) * (int)sizeof(T);         // bytes landing per plane
+    static constexpr int NPACK = WY + 1;                         // row pairs that publish (main + the halo pair)
+    static constexpr int NGRP = 8;                               // coefficient groups (kx, kz) exchanged
+    static constexpr int EXW = 64;                               // exchange columns: tile columns -1 .. 62
+    static constexpr int EX_SLOT = NPACK * NGRP * EXW;           // elements per component and slot
+    static constexpr int OUT_ELEMS = TSLB_NF * ROWS * COLS;      // output tile [10][ROWS][COLS]
+    static constexpr int OFF_OUT = NS * STAGE_ELEMS * (int)sizeof(T);
+    static constexpr int OFF_EX = OFF_OUT + rup128(OUT_ELEMS * (int)sizeof(T));
+    static constexpr int OFF_BAR = OFF_EX + 4 * EX_SLOT * (int)sizeof(T);     // 2 components x 2 slots
+    static constexpr int NBAR = 2 * NS + 2 * NPACK + 2;
+    static constexpr int SMEM_BYTES = OFF_BAR + NBAR * 8;
 };
-static_assert(TileDims<float>::BY <= TILE_MAX_BY && TileDims<double>::BY <= TILE_MAX_BY, "layout height");
+static_assert(TileDims<float>::SMEM_BYTES <= 232448 && TileDims<double>::SMEM_BYTES <= 232448, "shared memory budget");
+static_assert(TileGeom<float>::WX == 2 && TileGeom<double>::WX == 2, "two warps per row pair publish; two halo warps");
 
 template <typename T, bool WALLY, int ORDER>
-__global__ void __launch_bounds__(TileDims<T>::WARPS * 32, TileGeom<T>::MINB) sweep_tile_kernel(const __grid_constant__ CUtensorMap tmA,
-                                                                   T *__restrict__ Bbuf, TileParams<T> p)
+__global__ void __maxnreg__(TileDims<T>::MAXREG)
+sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
+                  const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p)
 {
     typedef typename PackOf<T>::type P;
-    extern __shared__ __align__(1024) unsigned char smem_raw[];
     typedef TileDims<T> TD;
-    T *ring = reinterpret_cast<T *>(smem_raw);          // NS stages of [10][BY][BXW]
-    constexpr int BXW = TD::BXW, TILE_BY = TD::BY, TILE_NS = TileGeom<T>::NS, STAGE_ELEMS = TD::STAGE_ELEMS;
-    __shared__ uint64_t full_bar[TILE_NS];
+    constexpr int NS = TD::NS, BXW = TD::BXW, FS = TD::FS, ROWS = TD::ROWS, COLS = TD::COLS, WY = TD::WY, WX = TD::WX;
+    constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
+    constexpr int ES = (int)sizeof(T);
+    constexpr int STAGE_BYTES = TD::STAGE_ELEMS * ES, SLOT_BYTES = TD::EX_SLOT * ES;
+    constexpr int OFF_EXY = TD::OFF_EX + 2 * SLOT_BYTES;           // exX: [2][NPACK][NGRP][EXW] M of a pack's row .x; exY: P of its row .y
+    // barriers (8 bytes each): full[NS], empty[NS], q[NPACK][2], ofull, oempty
+    constexpr int B_FULL = TD::OFF_BAR, B_EMPTY = B_FULL + 8 * NS, B_Q = B_EMPTY + 8 * NS, B_OFULL = B_Q + 16 * NPACK, B_OEMPTY = B_OFULL + 8;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    const uint32_t sb = keep(smem_u32(smem_raw));
 
     const int lane = threadIdx.x & 31;
     const int wid = threadIdx.x >> 5;
     const Layout &L = p.L;
-    const long long N = L.field;
 
-    // ---- columns: the warp outputs [xs, xs+30); lane l holds column xs - 1 + l -------------------------------
-    const int wx = wid % TileGeom<T>::WX, wy = wid / TileGeom<T>::WX;
-    const int xs0 = blockIdx.x * TD::COLS;               // first column of the CTA
-    const int xs = xs0 + wx * TILE_COLS;
-    const int col = xs - 1 + lane;
-    const int xb = xs0 & ~(TileGeom<T>::ALIGN - 1);      // box origin (element index in the padded row), 16-byte aligned
-    const bool col_out = lane >= 1 && lane <= TILE_COLS && col < L.nx;  // this lane produces output
-    // ---- rows: pack .x = row r0, .y = row r0+1; halo rows r0-1, r0+2 ------------------------------------------
-    const int row0 = blockIdx.y * TD::ROWS;
-    const int r0 = row0 + 2 * wy;
-    const bool warp_active = r0 < L.ny;
-    const bool row1_valid = r0 + 1 < L.ny;
-    // rows beyond a bounce-back wall contribute nothing (their part is added by bounce_y_correction)
-    const bool ghost_lo = WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && r0 == 0;                 // row r0-1
-    const bool ghost_mid = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 1 == L.ny;         // rows r0+1, r0+2
-    const bool ghost_hi = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 2 == L.ny;          // row r0+2
-    const bool any_ghost = ghost_lo || ghost_mid || ghost_hi;   // warp-uniform: this warp owns a wall-adjacent row
-    // multiplicative masks of the rows beyond a wall (no selects in the marching loop): mh for the halo pack (r0-1, r0+2),
-    // ms for the swapped centre pack (r0+1, r0)
-    const P mh = pk(ghost_lo ? (T)0 : (T)1, (ghost_hi || ghost_mid) ? (T)0 : (T)1);
-    const P ms = pk(ghost_mid ? (T)0 : (T)1, (T)1);
-
+    // tile origin; the last tile of the y axis is shifted back so that every tile is full (ny >= ROWS is required; overlapped
+    // rows are computed twice, to identical values)
+    const int x0 = blockIdx.x * COLS;
+    const int row0 = min((int)blockIdx.y * ROWS, L.ny - ROWS);
     const int z0 = blockIdx.z * p.zchunk;
     const int z1 = min(z0 + p.zchunk, L.nz);
     const int nplanes = z1 - z0 + 2;                     // source planes z0-1 .. z1
 
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int s = 0; s < TILE_NS; ++s) mbar_init(&full_bar[s], 1);
+        for (int s = 0; s < NS; ++s) { mbar_init(sb + B_FULL + 8 * s, 1); mbar_init(sb + B_EMPTY + 8 * s, TD::WARPS); }
+#pragma unroll
+        for (int s = 0; s < 2 * NPACK; ++s) mbar_init(sb + B_Q + 8 * s, WX);
+        mbar_init(sb + B_OFULL, TD::NMAIN);
+        mbar_init(sb + B_OEMPTY, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_async_smem();
     }
     __syncthreads();
-    // plane i of this CTA = source plane z0-1+i: box origin (element xs, padded row row0, padded plane z0+i, field 0)
-    auto issue = [&](int i) {
-        const int s = i % TILE_NS;
-        mbar_expect_tx(&full_bar[s], (uint32_t)(TD::BOX_ELEMS * sizeof(T)));
-        tma_load_4d(ring + s * STAGE_ELEMS, &tmA, &full_bar[s], xb, row0, z0 + i, 0);
-    };
-    if (threadIdx.x == 0)
-        for (int i = 0; i < TILE_NS && i < nplanes; ++i) issue(i);
 
-    // z-march state per (px,py) group: Vp of plane zs-2, centre term of plane zs-1, Vp of plane zs-1
-    // (kept as T1 = Vp(zs-2) + centre(zs-1), Vp(zs-2) where it is needed alone -- groups 0, 1, 3 -- and Vp(zs-1):
-    //  15 instead of 18 running pairs, 9 instead of 18 register moves per plane)
+    if (wid >= TD::NMAIN) {
+        // =================================================== halo warps ===================================================
+        const int h = wid - TD::NMAIN;
+        const int ecol = 32 * h + lane;                    // exchange column = tile column + 1
+        const int bcol = ecol - 1 + XPAD;                  // box column
+        // pack .x = tile row ROWS (above the tile), .y = tile row -1 (below): it publishes (M of .x, P of .y) like any pack
+        const uint32_t aA = keep(sb + (TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol) * ES), aB = keep(sb + (TD::MAIN_ELEMS + bcol) * ES);
+        const uint32_t aW = keep(sb + TD::OFF_EX + ((NPACK - 1) * NGRP * EXW + ecol) * ES);
+        // source rows of the two halo rows: wrapped on a periodic axis, out of bounds (zero fill) beyond a wall / open face
+        const bool yper = p.kind[2] == TSLB_BC_PERIODIC;
+        const int ylo = row0 > 0 ? row0 - 1 : (yper ? L.ny - 1 : -1);
+        const int yhi = row0 + ROWS < L.ny ? row0 + ROWS : (yper ? 0 : L.ny);
+        const bool zper = p.kind[4] == TSLB_BC_PERIODIC;
+        auto issue = [&](int j) {                          // source plane z0-1+j into stage j % NS
+            int zs = z0 - 1 + j;
+            if (zs < 0) zs = zper ? L.nz - 1 : -1;
+            else if (zs >= L.nz) zs = zper ? 0 : L.nz;
+            const int s = j % NS;
+            const uint32_t dst = sb + s * STAGE_BYTES, bar = sb + B_FULL + 8 * s;
+            mbar_expect_tx(bar, (uint32_t)TD::STAGE_TX);
+            tma_load_4d(dst, &tmMain, bar, x0, row0, zs, 0);
+            tma_load_4d(dst + TD::MAIN_ELEMS * ES, &tmRow, bar, x0, ylo, zs, 0);
+            tma_load_4d(dst + (TD::MAIN_ELEMS + TD::HALO_ELEMS) * ES, &tmRow, bar, x0, yhi, zs, 0);
+        };
+        const bool producer = h == 0 && lane == 0, storer = h == 1 && lane == 0;
+        if (producer)
+            for (int j = 0; j < NS - 1 && j < nplanes; ++j) issue(j);
+        // rows beyond a bounce-back wall send nothing (their raw moments are zero-filled, but A100 = 3 g is not zero)
+        const P hm = pk((WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && row0 + ROWS >= L.ny) ? (T)0 : (T)1,
+                        (WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && row0 == 0) ? (T)0 : (T)1);
+        auto store_tile = [&](int m) {                     // output plane m of this chunk: z = z0 + m
+            mbar_wait(sb + B_OFULL, (uint32_t)(m & 1));
+            tma_store_4d(sb + TD::OFF_OUT, &tmStore, x0 + TSLB_XOFF, row0, z0 + m, 0);
+            tma_store_commit();
+            tma_store_wait_read();
+            mbar_arrive(sb + B_OEMPTY);
+        };
+        int stg = 0;
+        uint32_t fpar = 0;
+        for (int i = 0; i < nplanes; ++i) {
+            if (producer) {
+                const int j = i + NS - 1;                  // refill the stage of plane i-1 with plane j
+                if (j < nplanes) {
+                    if (i >= 1) mbar_wait(sb + B_EMPTY + 8 * (j % NS), (uint32_t)((j / NS - 1) & 1));
+                    issue(j);
+                }
+            }
+            __syncwarp();
+            const uint32_t so = stg * STAGE_BYTES;
+            mbar_wait(sb + B_FULL + 8 * stg, fpar);
+            P rh[TSLB_NF];
+#pragma unroll
+            for (int f = 0; f < TSLB_NF; ++f) rh[f] = pk(lds(aA + so + f * BXW * ES, T()), lds(aB + so + f * BXW * ES, T()));
+            warp_arrive(sb + B_EMPTY + 8 * stg, lane);
+            const uint32_t w = aW + (i & 1) * SLOT_BYTES;
+            // the exchange slot is reused every second plane: its readers (the first and the last row pair of the tile) have
+            // finished reading plane i-2 once they have published plane i-1.  (The main warps get the same guarantee from
+            // waiting for the pairs they read from; the halo warps read nothing, so they wait explicitly.)
+            if (i >= 2) {
+                mbar_wait(sb + B_Q + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
+                mbar_wait(sb + B_Q + 16 * (WY - 1) + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
+            }
+#define TSLB_HALO_GROUP(KX, KZ)                                                                   \
+            if (kvalid<ORDER>(KX, 0, KZ)) {                                                       \
+                P qc, qp, cen;                                                                    \
+                ycombos<ORDER, KX, KZ, P, T>(A, qc, qp, cen);                                     \
+                if (WALLY) qp = pmul(qp, hm);                                                     \
+                sts(w + qidx(KX, KZ) * EXW * ES, qp.x);                                           \
+                sts(w + 2 * SLOT_BYTES + qidx(KX, KZ) * EXW * ES, qp.y);                          \
+            }
+#define TSLB_HALO_ROUND(KZ)                                                                       \
+            {                                                                                     \
+                P A[3][3];                                                                        \
+                hermite_round<KZ, P, T>(rh, p.beta, p.g, A);                                      \
+                TSLB_HALO_GROUP(0, KZ) TSLB_HALO_GROUP(1, KZ) TSLB_HALO_GROUP(2, KZ)              \
+            }
+            TSLB_HALO_ROUND(0)
+            TSLB_HALO_ROUND(1)
+            TSLB_HALO_ROUND(2)
+#undef TSLB_HALO_ROUND
+#undef TSLB_HALO_GROUP
+            warp_arrive(sb + B_Q + 16 * (NPACK - 1) + 8 * (i & 1), lane);
+            // the output tile the main warps finished in their iteration i-1 (output plane i-3)
+            if (storer && i >= 3) store_tile(i - 3);
+            if (++stg == NS) { stg = 0; fpar ^= 1; }
+        }
+        if (storer) {
+            if (nplanes >= 3) store_tile(nplanes - 3);
+            tma_store_wait_all();
+        }
+        return;
+    }
+
+    // ===================================================== main warps =====================================================
+    // ---- columns: the warp outputs tile columns [30 wx, 30 wx + 30); lane l holds tile column 30 wx - 1 + l -----------------
+    const int wx = wid % WX, wy = wid / WX;
+    const int tc = TILE_COLS * wx - 1 + lane;
+    const int col = x0 + tc;
+    const bool lane_out = lane >= 1 && lane <= TILE_COLS;
+    // ---- rows: pack .x = row r0, .y = row r0+1; outer neighbours r0-1, r0+2 -------------------------------------------------
+    const int r0 = row0 + 2 * wy;
+    // this warp owns a row next to a bounce-back wall (warp-uniform): .x row at the wall below / .y row at the wall above
+    const bool ghost_lo = WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && r0 == 0;
+    const bool ghost_hi = WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && r0 + 2 == L.ny;
+    const bool any_ghost = ghost_lo || ghost_hi;
+
+    // shared-memory addresses of this thread
+    const int bcol = tc + XPAD;
+    const uint32_t aC = keep(sb + ((2 * wy) * BXW + bcol) * ES);                 // row r0 in the main region (r0+1: + BXW)
+    // u of rows r0-1 / r0+2: in the main region (field stride FS) or, at the tile edge, in a halo-row slot (field stride BXW)
+    const int fsLo = wy == 0 ? BXW : FS, fsHi = wy == WY - 1 ? BXW : FS;
+    const uint32_t aLo = keep(sb + ((wy == 0 ? TD::MAIN_ELEMS + bcol : (2 * wy - 1) * BXW + bcol) + fsLo) * ES);
+    const uint32_t aHi = keep(sb + ((wy == WY - 1 ? TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol : (2 * wy + 2) * BXW + bcol) + fsHi) * ES);
+    const uint32_t stLo = keep((uint32_t)(fsLo * ES)), stHi = keep((uint32_t)(fsHi * ES));
+    // exchange: own pack wy publishes at column tc+1 (columns 30, 31 belong to the wx = 0 warp: lanes 0, 1 of the wx = 1 warp
+    // write into the unused columns 62, 63 instead); the halo pair is pack NPACK-1: below wy = 0 and above wy = WY-1
+    const int ecol = tc + 1;
+    const int ecol_w = (wx == 0 || lane >= 2) ? ecol : 62 + lane;
+    const uint32_t aW = keep(sb + TD::OFF_EX + (wy * NGRP * EXW + ecol_w) * ES);
+    const uint32_t aDn = keep(sb + OFF_EXY + (((wy + NPACK - 1) % NPACK) * NGRP * EXW + ecol) * ES);   // P of the row below
+    const uint32_t aUp = keep(sb + TD::OFF_EX + ((wy + 1) * NGRP * EXW + ecol) * ES);                  // M of the row above
+    const uint32_t aO = keep(sb + TD::OFF_OUT + ((2 * wy) * COLS + (tc < 0 ? 0 : tc)) * ES);           // output tile [f][row][tc]
+    const uint32_t bQown = sb + B_Q + 16 * wy, bQdn = sb + B_Q + 16 * ((wy + NPACK - 1) % NPACK), bQup = sb + B_Q + 16 * (wy + 1);
+
+    // z-march state per (px,py) group g: tt1 = Vp(zs-2) + centre(zs-1), vp1 = Vp(zs-1), and vp2 = Vp(zs-2) where it is needed
+    // alone (groups 0, 1, 3): 15 running pairs
     P vp2[6], tt1[6], vp1[6];
     // increment form along z: velocity of the previous plane and its backward difference, rows r0, r0+1
     P uprev[3], dprev[3];
-    P kw[4];                                              // carried bounce-back terms of the moments with c_z (walls only)
-#pragma unroll
-    for (int k = 0; k < 4; ++k) kw[k] = pbc<P, T>((T)0);
 #pragma unroll
     for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); tt1[i] = vp2[i]; vp1[i] = vp2[i]; }
 #pragma unroll
     for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
 
-    // which of this thread's nodes have periodic ghost images (finalize_store)
-    const int eflags_xy = ((p.kind[0] == TSLB_BC_PERIODIC && (col == 0 || col == L.nx - 1)) ? 1 : 0) |
-                          ((p.kind[2] == TSLB_BC_PERIODIC && (r0 == 0 || r0 == L.ny - 1)) ? 2 : 0) |
-                          ((p.kind[2] == TSLB_BC_PERIODIC && r0 + 1 == L.ny - 1) ? 4 : 0);
-    const P sgn = pk((T)1, (T)-1);                        // D = W * sgn for the (centre, halo) row packing, see below
-    const bool st_ok = col_out && warp_active;
+    const P sgn = pk((T)1, (T)-1), nsg = pk((T)-1, (T)1);
+    const bool xper = p.kind[0] == TSLB_BC_PERIODIC;
+    // periodic x: the node at x = 0 is also the ghost column x = nx, the node at x = nx-1 the ghost column x = -1
+    const bool xedge = xper && lane_out && (col == 0 || col == L.nx - 1);
+    const long long gcol = col == 0 ? (long long)L.nx + TSLB_XOFF : (long long)TSLB_XOFF - 1;
+    // The TMA store works in 16-byte units: the output tensor is clipped at the last 16-byte boundary inside the row (a
+    // partly covered unit would be written whole, over the ghost column), the columns beyond it are stored from registers
+    const bool xtail = lane_out && col >= (L.nx & ~(16 / ES - 1)) && col < L.nx;
+
+    int stg = 0;
+    uint32_t fpar = 0;
     for (int i = 0; i < nplanes; ++i) {
-        const int stg = i % TILE_NS;
-        mbar_wait(&full_bar[stg], (uint32_t)((i / TILE_NS) & 1));
-        {   // every warp computes (rows beyond the lattice read defined but meaningless smem rows and store nothing):
-            // no divergent region around the shuffles
-            const int zs = z0 - 1 + i;
-            const T *S = ring + stg * STAGE_ELEMS + (2 * wy) * BXW + (xs - xb) + lane;
+        const uint32_t so = stg * STAGE_BYTES;
+        const uint32_t xo = (i & 1) * SLOT_BYTES;
+        mbar_wait(sb + B_FULL + 8 * stg, fpar);
 
-            // ---- a1: moments of rows r0-1 .. r0+2 at this column.  Packing: C = (r0, r0+1) the two output rows,
-            //      H = (r0-1, r0+2) their outer neighbours.  For the output pack: up = (H.x, C.x), dn = (C.y, H.y), so
-            //      up + dn = H + swap(C) and up - dn = (H - swap(C)) * (1,-1): the centre needs no repacking and the swap
-            //      is an operand modifier of the packed instructions. ------------------------------------------------
-            P rc[TSLB_NF], rh[TSLB_NF];
+        // ---- a1: moments of the own rows r0, r0+1 and the velocities of the rows r0-1, r0+2 at this column ------------------
+        P rc[TSLB_NF], hu[3];
+        {
+            const uint32_t a = aC + so;
 #pragma unroll
-            for (int f = 0; f < TSLB_NF; ++f) {
-                const T *s = S + f * (TILE_BY * BXW);
-                rc[f] = pk(s[BXW], s[2 * BXW]);
-                rh[f] = pk(s[0], s[3 * BXW]);
-            }
-            // ---- increment form: exact differences of the stored velocities along y, x, z ---------------------------
-            P Ly[3], Wy[3], Lx[3], Dx[3], Lz[3], Dz[3];
+            for (int f = 0; f < TSLB_NF; ++f) rc[f] = pk(lds(a + f * FS * ES, T()), lds(a + (f * FS + BXW) * ES, T()));
+            uint32_t al = aLo + so, ah = aHi + so;
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const P uc = rc[1 + a];
-                P hs = rh[1 + a], cs = pk(uc.y, uc.x);
-                if (WALLY) { hs = pmul(hs, mh); cs = pmul(cs, ms); }   // a node beyond a wall enters the differences as u = 0
-                Ly[a] = pfmas(uc, (T)-2, padd(hs, cs));      // (up - c) + (dn - c)
-                Wy[a] = psub(hs, cs);                        // (up - dn) * sgn
-                const T *s = S + (1 + a) * (TILE_BY * BXW);
-                const P xl = pk(s[BXW - 1], s[2 * BXW - 1]), xr = pk(s[BXW + 1], s[2 * BXW + 1]);
-                Lx[a] = pfmas(uc, (T)-2, padd(xl, xr));
-                Dx[a] = psub(xl, xr);
-                const P dcur = psub(uc, uprev[a]);           // u(zs) - u(zs-1)
-                Lz[a] = psub(dcur, dprev[a]);                // at the target plane zs-1
-                Dz[a] = padd(dprev[a], dcur);                // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
-                dprev[a] = dcur;
-            }
-
-            P vp0[6], vm0[6], cc0[6];  // this plane's Vp, Vm, centre term per group
-            // halfway bounce-back on a y face: for a wall-adjacent row the 9
-            // populations arriving from beyond the wall are f*_ibar of the node itself, a local combination of its own
-            // coefficients: B(kx,kz) with the local sums L(0,0)=6, L(1,1)=-2, L(2,0)=L(2,2)=2.  .x = row r0, .y = row r0+1.
-            P WB[3][3];
-            const P wsp = pk(ghost_lo ? (T)-1 : (T)1, (T)1);
-#pragma unroll
-            for (int kz = 0; kz < 3; ++kz) {
-                // ---- a2: Hermite coefficients of the four rows for this kz --------------------------------------
-                P Ac[3][3], Ah[3][3];
-                if (kz == 0) { hermite_round<0, P, T>(rc, p.beta, p.g, Ac); hermite_round<0, P, T>(rh, p.beta, p.g, Ah); }
-                if (kz == 1) { hermite_round<1, P, T>(rc, p.beta, p.g, Ac); hermite_round<1, P, T>(rh, p.beta, p.g, Ah); }
-                if (kz == 2) { hermite_round<2, P, T>(rc, p.beta, p.g, Ac); hermite_round<2, P, T>(rh, p.beta, p.g, Ah); }
-                // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 -------------------------
-                P G1[3][3];
-#pragma unroll
-                for (int kx = 0; kx < 3; ++kx) {
-                    if (!kvalid<ORDER>(kx, 0, kz)) continue;
-                    // E = up(P) + dn(M), O = up(P) - dn(M) with P = phi0 + phi1 + phi2, M = phi0 - phi1 + phi2 of the
-                    // neighbour rows.  Per pack Q = (P of its .x row, M of its .y row) = phi0 + phi2 + phi1 * sgn; then
-                    // E = Q_H + swap(Q_C) and O = (Q_H - swap(Q_C)) * sgn.
-                    P qh = Ah[kx][0], qc = Ac[kx][0];
-                    if (kvalid<ORDER>(kx, 2, kz)) { qh = padd(qh, Ah[kx][2]); qc = padd(qc, Ac[kx][2]); }
-                    if (kvalid<ORDER>(kx, 1, kz)) { qh = pfma(Ah[kx][1], sgn, qh); qc = pfma(Ac[kx][1], sgn, qc); }
-                    P qs = pk(qc.y, qc.x);
-                    if (WALLY) {   // rows beyond a bounce-back wall send nothing; the bounced populations are added below
-                        qh = pmul(qh, mh);
-                        qs = pmul(qs, ms);
-                        // B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz) of the own rows: wall below -> (1,-1,1), above -> (1,1,1)
-                        if (kx + kz <= 2 && !(kx == 1 && kz == 2) && !(kx == 2 && kz == 1)) {
-                            P bq = Ac[kx][0];
-                            if (kvalid<ORDER>(kx, 2, kz)) bq = padd(bq, Ac[kx][2]);
-                            if (kvalid<ORDER>(kx, 1, kz)) bq = pfma(Ac[kx][1], wsp, bq);
-                            WB[kx][kz] = bq;
-                        }
-                    }
-                    const P E = padd(qh, qs);
-                    G1[2][kx] = E;
-                    G1[1][kx] = pmul(psub(qh, qs), sgn);
-                    P o0 = pfmas(Ac[kx][0], (T)4, E);
-                    if (kvalid<ORDER>(kx, 2, kz)) o0 = pfmas(Ac[kx][2], (T)-2, o0);
-                    G1[0][kx] = o0;
-                }
-                // y-stage increments of the bases 3 u_a (tap sums along y: 6, 0, 2 for py = 0, 1, 2 when ky = 0; 0, 2, 0 when ky = 1)
-                const P sg3 = pk((T)3, (T)-3);
-                if (kz == 0) {
-                    G1[0][1] = pfmas(Ly[0], (T)3, G1[0][1]); G1[1][1] = pfma(Wy[0], sg3, G1[1][1]); G1[2][1] = pfmas(Ly[0], (T)3, G1[2][1]);
-                    G1[0][0] = pfma(Wy[1], sg3, G1[0][0]); G1[1][0] = pfmas(Ly[1], (T)3, G1[1][0]); G1[2][0] = pfma(Wy[1], sg3, G1[2][0]);
-                }
-                if (kz == 1) {
-                    G1[0][0] = pfmas(Ly[2], (T)3, G1[0][0]); G1[1][0] = pfma(Wy[2], sg3, G1[1][0]); G1[2][0] = pfmas(Ly[2], (T)3, G1[2][0]);
-                }
-                // ---- x pass (warp shuffles): G2[px][py] = sum_kx T^x_{px,kx} G1[py][kx]; then the z bookkeeping ----
-#pragma unroll
-                for (int py = 0; py < 3; ++py) {
-                    // E = up(P) + dn(M), O = up(P) - dn(M): one shuffle up of P = phi0 + phi1 + phi2 and one down of
-                    // M = phi0 - phi1 + phi2 instead of two per field
-                    P t = G1[py][0];
-                    if (kvalid<ORDER>(2, 0, kz)) t = padd(t, G1[py][2]);
-                    P pp = t, mm = t;
-                    if (kvalid<ORDER>(1, 0, kz)) { pp = padd(t, G1[py][1]); mm = psub(t, G1[py][1]); }
-                    const P upP = shfl_up1(pp);   // from column-1  (c_x = +1 pulls from x-1)
-                    const P dnM = shfl_dn1(mm);   // from column+1
-                    P o[3];
-                    o[2] = padd(upP, dnM);
-                    o[1] = psub(upP, dnM);
-                    o[0] = pfmas(G1[py][0], (T)4, o[2]);
-                    if (kvalid<ORDER>(2, 0, kz)) o[0] = pfmas(G1[py][2], (T)-2, o[0]);
-                    // x-stage increments: base multipliers after the y stage are 18 (py=0) and 6 (py=2) for ux (kx=1) and uz
-                    // (kx=0, kz=1), 6 (py=1) for uy (kx=0)
-                    if (kz == 0 && py == 0) { o[0] = pfmas(Dx[0], (T)18, o[0]); o[1] = pfmas(Lx[0], (T)18, o[1]); o[2] = pfmas(Dx[0], (T)18, o[2]); }
-                    if (kz == 0 && py == 2) { o[0] = pfmas(Dx[0], (T)6, o[0]); }
-                    if (kz == 0 && py == 1) { o[0] = pfmas(Lx[1], (T)6, o[0]); o[1] = pfmas(Dx[1], (T)6, o[1]); }
-                    if (kz == 1 && py == 0) { o[0] = pfmas(Lx[2], (T)18, o[0]); o[1] = pfmas(Dx[2], (T)18, o[1]); o[2] = pfmas(Lx[2], (T)18, o[2]); }
-                    if (kz == 1 && py == 2) { o[0] = pfmas(Lx[2], (T)6, o[0]); }
-#pragma unroll
-                    for (int px = 0; px + py <= 2; ++px) {
-                        const int gi = gidx(px, py);
-                        const P v = o[px];
-                        // Vp = phi0 + phi1 + phi2, Vm = phi0 - phi1 + phi2, centre = 4 phi0 - 2 phi2   (over kz)
-                        if (kz == 0) { vp0[gi] = v; vm0[gi] = v; cc0[gi] = pmuls(v, (T)4); }
-                        if (kz == 1) { vp0[gi] = padd(vp0[gi], v); vm0[gi] = psub(vm0[gi], v); }
-                        if (kz == 2) { vp0[gi] = padd(vp0[gi], v); vm0[gi] = padd(vm0[gi], v); cc0[gi] = pfmas(v, (T)-2, cc0[gi]); }
-                    }
-                }
-            }
-
-            P kw_new[4];
-            if (WALLY && any_ghost) {
-                // full first-order coefficients (the passes carry them without their base 3 u)
-                WB[1][0] = pfmas(rc[1], (T)3, WB[1][0]);
-                WB[0][0] = pfma(rc[2], pmuls(wsp, (T)3), WB[0][0]);
-                WB[0][1] = pfmas(rc[3], (T)3, WB[0][1]);
-                const P wm = pk((ghost_lo || ghost_mid) ? (T)1 : (T)0, ghost_hi ? (T)1 : (T)0);   // which row of the pack is at a wall
-                const P sgp = pk(ghost_lo ? (T)1 : (T)-1, (T)-1);                              // c_y of the arrival direction
-                const P w12 = pmuls(wm, (T)12), w36 = pmuls(wm, (T)36), w12s = pmul(w12, sgp), w36s = pmul(w36, sgp);
-                // arrival c_z = 0: into this plane's centre terms (they reach the target plane through tt1)
-                cc0[0] = pfma(WB[0][0], w36, cc0[0]);                         // 000
-                cc0[1] = pfma(WB[1][0], pmuls(w12, (T)-1), cc0[1]);           // 100
-                cc0[3] = pfma(WB[0][0], w36s, cc0[3]);                        // 010
-                cc0[2] = pfma(padd(WB[0][0], WB[2][0]), w12, cc0[2]);         // 200
-                cc0[5] = pfma(WB[0][0], w36, cc0[5]);                         // 020
-                cc0[4] = pfma(WB[1][0], pmuls(w12s, (T)-1), cc0[4]);          // 110
-                // moments with c_z: carried to the next iteration, where this plane is the target
-                kw_new[0] = pmul(WB[0][1], pmuls(w12, (T)-1));                // 001
-                kw_new[1] = pmul(padd(WB[0][0], WB[0][2]), w12);              // 002
-                kw_new[2] = pmul(WB[1][1], pmuls(wm, (T)4));                  // 101
-                kw_new[3] = pmul(WB[0][1], pmuls(w12s, (T)-1));               // 011
-            }
-            // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
-            //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
-            const int zt = zs - 1;
-            if (zt >= z0 && st_ok) {
-                P m[TSLB_NF];
-                {
-                    m[0] = pfmas(Dz[2], (T)-108, padd(tt1[0], vm0[0]));          // 000
-                    m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));         // 001
-                    m[6] = pfmas(Dz[2], (T)-108, padd(vp2[0], vm0[0]));         // 002
-                    m[1] = pfmas(Lz[0], (T)36, padd(tt1[1], vm0[1]));           // 100
-                    m[8] = pfmas(Dz[0], (T)-36, psub(vp2[1], vm0[1]));          // 101
-                    m[2] = pfmas(Lz[1], (T)36, padd(tt1[3], vm0[3]));           // 010
-                    m[9] = pfmas(Dz[1], (T)-36, psub(vp2[3], vm0[3]));          // 011
-                    m[4] = pfmas(Dz[2], (T)-36, padd(tt1[2], vm0[2]));           // 200
-                    m[7] = padd(tt1[4], vm0[4]);                               // 110
-                    m[5] = pfmas(Dz[2], (T)-36, padd(tt1[5], vm0[5]));           // 020
-                }
-                const long long i0 = lay_idx(L, col, r0, zt);
-                if (WALLY) { m[3] = padd(m[3], kw[0]); m[6] = padd(m[6], kw[1]); m[8] = padd(m[8], kw[2]); m[9] = padd(m[9], kw[3]); }
-                const int eflags = eflags_xy | ((p.kind[4] == TSLB_BC_PERIODIC && (zt == 0 || zt == L.nz - 1)) ? 8 : 0);
-                finalize_store<P, T>(m, uprev, Bbuf, N, i0, i0 + L.px, row1_valid, eflags, L, col, r0, zt);
-            }
-            if (WALLY && any_ghost) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) kw[k] = kw_new[k];
-            }
-            // ---- shift the march state ---------------------------------------------------------------------------------
-#pragma unroll
-            for (int g = 0; g < 6; ++g) {
-                tt1[g] = padd(vp1[g], cc0[g]);               // Vp(zs-1) + centre(zs): used when plane zs+1 arrives
-                if (g == 0 || g == 1 || g == 3) vp2[g] = vp1[g];
-                vp1[g] = vp0[g];
-            }
-#pragma unroll
-            for (int a = 0; a < 3; ++a) uprev[a] = rc[1 + a];
+            for (int k = 0; k < 3; ++k) { hu[k] = pk(lds(al, T()), lds(ah, T())); al += stLo; ah += stHi; }
         }
-        __syncthreads();                                  // every warp is done with stage `stg`: refill it
-        if (threadIdx.x == 0 && i + TILE_NS < nplanes) issue(i + TILE_NS);
+        warp_arrive(sb + B_EMPTY + 8 * stg, lane);       // the stage can be refilled: everything needed is in registers
+
+        // ---- increment form along y: exact differences of the stored velocities,
+        //      Ly = (up - c) + (dn - c), Wy = (up - dn) * sgn with up / dn the neighbour rows (hu = (u(r0-1), u(r0+2)), the
+        //      other neighbour is the pack's other row); a node beyond a wall has u = 0 (zero-filled halo row).  They enter
+        //      the y pass of the groups that carry a first-order coefficient:  E += incE, O += incO  with
+        //      (kx,kz) = (1,0): 3 Ly_x, sg3 Wy_x;   (0,0): sg3 Wy_y, 3 Ly_y;   (0,1): 3 Ly_z, sg3 Wy_z. -------------------------
+        const P sg3 = pk((T)3, (T)-3);
+        P incE[3], incO[3];        // indexed by velocity component
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const P uc = rc[1 + a];
+            const P cs = pswap(uc);
+            const P ly3 = pmuls(pfmas(uc, (T)-2, padd(hu[a], cs)), (T)3);
+            const P wy3 = pmul(psub(hu[a], cs), sg3);
+            incE[a] = a == 1 ? wy3 : ly3;
+            incO[a] = a == 1 ? ly3 : wy3;
+        }
+
+        // ---- a2: Hermite coefficients of the own rows, all three rounds; y-pass combinations of the 8 groups -------------
+        // qs = swap(qc) = (M of row r0+1, P of row r0): what the two rows of the pack receive from each other.
+        // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)), so with qh = (P(r0-1), M(r0+2)) read from the
+        // neighbours:  E = up + dn = qh + qs,  O = up - dn = (qh - qs) * sgn = qh*sgn + qo,  qo = -qs*sgn;  G0 = E + cen.
+        P qe[NGRP], qo[NGRP], cen[NGRP];
+        {
+            const uint32_t w = aW + xo;
+#define TSLB_MAIN_GROUP(KX, KZ)                                                                   \
+            if (kvalid<ORDER>(KX, 0, KZ)) {                                                       \
+                constexpr int q = qidx(KX, KZ);                                                   \
+                constexpr int ia = (KX == 1 && KZ == 0) ? 0 : ((KX == 0 && KZ == 0) ? 1 : ((KX == 0 && KZ == 1) ? 2 : -1)); \
+                P qc, qp;                                                                         \
+                ycombos<ORDER, KX, KZ, P, T>(A, qc, qp, cen[q]);                                  \
+                const P qs = pswap(qc);                                                           \
+                if (ia >= 0) { qe[q] = padd(qs, incE[ia < 0 ? 0 : ia]); qo[q] = pfma(qs, nsg, incO[ia < 0 ? 0 : ia]); } \
+                else { qe[q] = qs; qo[q] = pmul(qs, nsg); }                                       \
+                sts(w + q * EXW * ES, qp.x);                                                      \
+                sts(w + 2 * SLOT_BYTES + q * EXW * ES, qp.y);                                     \
+            }
+#define TSLB_MAIN_ROUND(KZ)                                                                       \
+            {                                                                                     \
+                P A[3][3];                                                                        \
+                hermite_round<KZ, P, T>(rc, p.beta, p.g, A);                                      \
+                TSLB_MAIN_GROUP(0, KZ) TSLB_MAIN_GROUP(1, KZ) TSLB_MAIN_GROUP(2, KZ)              \
+            }
+            TSLB_MAIN_ROUND(0)
+            TSLB_MAIN_ROUND(1)
+            TSLB_MAIN_ROUND(2)
+#undef TSLB_MAIN_ROUND
+#undef TSLB_MAIN_GROUP
+        }
+        warp_arrive(bQown + 8 * (i & 1), lane);
+
+        // ---- the neighbours' combinations -----------------------------------------------------------------------------------
+        mbar_wait(bQdn + 8 * (i & 1), (uint32_t)((i >> 1) & 1));
+        mbar_wait(bQup + 8 * (i & 1), (uint32_t)((i >> 1) & 1));
+        const uint32_t rdn = aDn + xo, rup = aUp + xo;
+
+        // this plane's contributions to the z march, accumulated over kz where they are needed:
+        //   tt1[g] += Vm(zs)            (pz = 0 of the target plane zs-1; groups 2, 4, 5, where Vm is not needed alone)
+        //   vm0[g]  = Vm(zs)            (groups 0, 1, 3)
+        //   tn[g]   = vp1[g] + centre(zs)   (next iteration's tt1)
+        //   vp0[g]  = Vp(zs)
+        // with Vp = phi0 + phi1 + phi2, Vm = phi0 - phi1 + phi2, centre = 4 phi0 - 2 phi2 over kz.
+        P vp0[6], vm0[6], tn[6];
+#pragma unroll
+        for (int kz = 0; kz < 3; ++kz) {
+            // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 ---------------------------------------
+            P G1[3][3];
+#pragma unroll
+            for (int kx = 0; kx < 3; ++kx) {
+                if (!kvalid<ORDER>(kx, 0, kz)) continue;
+                const int q = qidx(kx, kz);
+                const P qh = pk(lds(rdn + q * EXW * ES, T()), lds(rup + q * EXW * ES, T()));
+                const P E = padd(qh, qe[q]);
+                G1[2][kx] = E;
+                G1[1][kx] = pfma(qh, sgn, qo[q]);
+                G1[0][kx] = padd(E, cen[q]);
+            }
+            // x differences of the stored velocities (increment form along x), from the neighbour lanes
+            P Lx[3], Dx[3];
+            if (kz == 0) {
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    const P xl = shfl_up1(rc[1 + a]), xr = shfl_dn1(rc[1 + a]);
+                    Lx[a] = pfmas(rc[1 + a], (T)-2, padd(xl, xr));
+                    Dx[a] = psub(xl, xr);
+                }
+            }
+            if (kz == 1) {
+                const P xl = shfl_up1(rc[3]), xr = shfl_dn1(rc[3]);
+                Lx[2] = pfmas(rc[3], (T)-2, padd(xl, xr));
+                Dx[2] = psub(xl, xr);
+            }
+            // ---- x pass (warp shuffles): G2[px][py] = sum_kx T^x_{px,kx} G1[py][kx]; then the z bookkeeping ----
+#pragma unroll
+            for (int py = 0; py < 3; ++py) {
+                // E = up(P) + dn(M), O = up(P) - dn(M): one shuffle up of P = phi0 + phi1 + phi2 and one down of
+                // M = phi0 - phi1 + phi2 instead of two per field
+                P t = G1[py][0];
+                if (kvalid<ORDER>(2, 0, kz)) t = padd(t, G1[py][2]);
+                P pp = t, mm = t;
+                if (kvalid<ORDER>(1, 0, kz)) { pp = padd(t, G1[py][1]); mm = psub(t, G1[py][1]); }
+                const P upP = shfl_up1(pp);   // from column-1  (c_x = +1 pulls from x-1)
+                const P dnM = shfl_dn1(mm);   // from column+1
+                P o[3];
+                o[2] = padd(upP, dnM);
+                o[1] = psub(upP, dnM);
+                o[0] = pfmas(G1[py][0], (T)4, o[2]);
+                if (kvalid<ORDER>(2, 0, kz)) o[0] = pfmas(G1[py][2], (T)-2, o[0]);
+                // x-stage increments: base multipliers after the y stage are 18 (py=0) and 6 (py=2) for ux (kx=1) and uz
+                // (kx=0, kz=1), 6 (py=1) for uy (kx=0)
+                if (kz == 0 && py == 0) { o[0] = pfmas(Dx[0], (T)18, o[0]); o[1] = pfmas(Lx[0], (T)18, o[1]); o[2] = pfmas(Dx[0], (T)18, o[2]); }
+                if (kz == 0 && py == 2) { o[0] = pfmas(Dx[0], (T)6, o[0]); }
+                if (kz == 0 && py == 1) { o[0] = pfmas(Lx[1], (T)6, o[0]); o[1] = pfmas(Dx[1], (T)6, o[1]); }
+                if (kz == 1 && py == 0) { o[0] = pfmas(Lx[2], (T)18, o[0]); o[1] = pfmas(Dx[2], (T)18, o[1]); o[2] = pfmas(Lx[2], (T)18, o[2]); }
+                if (kz == 1 && py == 2) { o[0] = pfmas(Lx[2], (T)6, o[0]); }
+#pragma unroll
+                for (int px = 0; px + py <= 2; ++px) {
+                    const int gi = gidx(px, py);
+                    const bool alone = gi == 0 || gi == 1 || gi == 3;      // Vm needed on its own (pz = 1, 2)
+                    const P v = o[px];
+                    if (kz == 0) { vp0[gi] = v; tn[gi] = pfmas(v, (T)4, vp1[gi]); if (alone) vm0[gi] = v; else tt1[gi] = padd(tt1[gi], v); }
+                    if (kz == 1) { vp0[gi] = padd(vp0[gi], v); if (alone) vm0[gi] = psub(vm0[gi], v); else tt1[gi] = psub(tt1[gi], v); }
+                    if (kz == 2) { vp0[gi] = padd(vp0[gi], v); tn[gi] = pfmas(v, (T)-2, tn[gi]); if (alone) vm0[gi] = padd(vm0[gi], v); else tt1[gi] = padd(tt1[gi], v); }
+                }
+            }
+        }
+
+        // ---- halfway bounce-back on a y face: for a wall-adjacent row the 9
+        //      populations arriving from beyond the wall are f*_ibar of the node itself, a local combination of its own
+        //      coefficients  B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz)  -- exactly the published combination qp of that row
+        //      (M of a row at the wall below, P of a row at the wall above) -- with the local sums L(0,0)=6, L(1,1)=-2,
+        //      L(2,0)=L(2,2)=2. ---------------------------------------------------------------------------------------------
+        // The six bounced populations with c_z = 0 go into this plane's centre terms (they reach the target plane through
+        // tt1); the four moments with c_z (001, 002, 101, 011) belong to the target plane zs-1 and are rebuilt there from
+        // that plane's combinations, which still sit in the other exchange slot (kwall below).
+        P kwall[4];
+        if (WALLY) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) kwall[k] = pbc<P, T>((T)0);
+        }
+        if (WALLY && any_ghost) {
+            const P wsp = pk(ghost_lo ? (T)-1 : (T)1, (T)1);
+            const P wm = pk(ghost_lo ? (T)1 : (T)0, ghost_hi ? (T)1 : (T)0);               // which row of the pack is at a wall
+            const P sgp = pk(ghost_lo ? (T)1 : (T)-1, (T)-1);                              // c_y of the arrival direction
+            const P w12 = pmuls(wm, (T)12), w36 = pmuls(wm, (T)36), w12s = pmul(w12, sgp), w36s = pmul(w36, sgp);
+            // (re-read from this warp's own exchange slots instead of being kept in registers across the passes; lanes 0, 1 of
+            //  the wx = 1 warp published elsewhere, but they are halo / duplicate lanes whose output is not stored)
+            auto own = [&](uint32_t w, int q) { return pk(lds(w + q * EXW * ES, T()), lds(w + 2 * SLOT_BYTES + q * EXW * ES, T())); };
+            {   // source plane zs: full first-order coefficients (the passes carry them without their base 3 u)
+                const uint32_t w = aW + xo;
+                const P WB10 = pfmas(rc[1], (T)3, own(w, qidx(1, 0)));
+                const P WB00 = pfma(rc[2], pmuls(wsp, (T)3), own(w, qidx(0, 0)));
+                const P WB20 = own(w, qidx(2, 0));
+                tn[0] = pfma(WB00, w36, tn[0]);                             // 000
+                tn[1] = pfma(WB10, pmuls(w12, (T)-1), tn[1]);               // 100
+                tn[3] = pfma(WB00, w36s, tn[3]);                            // 010
+                tn[2] = pfma(padd(WB00, WB20), w12, tn[2]);                 // 200
+                tn[5] = pfma(WB00, w36, tn[5]);                             // 020
+                tn[4] = pfma(WB10, pmuls(w12s, (T)-1), tn[4]);              // 110
+            }
+            if (i >= 2) {   // target plane zs-1 (its velocities are uprev)
+                const uint32_t w = aW + (SLOT_BYTES - xo);
+                const P WB00 = pfma(uprev[1], pmuls(wsp, (T)3), own(w, qidx(0, 0)));
+                const P WB01 = pfmas(uprev[2], (T)3, own(w, qidx(0, 1)));
+                const P WB11 = own(w, qidx(1, 1)), WB02 = own(w, qidx(0, 2));
+                kwall[0] = pmul(WB01, pmuls(w12, (T)-1));                   // 001
+                kwall[1] = pmul(padd(WB00, WB02), w12);                     // 002
+                kwall[2] = pmul(WB11, pmuls(wm, (T)4));                     // 101
+                kwall[3] = pmul(WB01, pmuls(w12s, (T)-1));                  // 011
+            }
+        }
+
+        // increment form along z: exact differences of the stored velocities at the target plane zs-1
+        P Lz[3], Dz[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const P dcur = psub(rc[1 + a], uprev[a]);    // u(zs) - u(zs-1)
+            Lz[a] = psub(dcur, dprev[a]);
+            Dz[a] = padd(dprev[a], dcur);                // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
+            dprev[a] = dcur;
+        }
+
+        // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
+        //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
+        if (i >= 2) {
+            const int zt = z0 + i - 2;
+            P m[TSLB_NF];
+            m[0] = pfmas(Dz[2], (T)-108, padd(tt1[0], vm0[0]));          // 000
+            m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));           // 001
+            m[6] = pfmas(Dz[2], (T)-108, padd(vp2[0], vm0[0]));          // 002
+            m[1] = pfmas(Lz[0], (T)36, padd(tt1[1], vm0[1]));            // 100
+            m[8] = pfmas(Dz[0], (T)-36, psub(vp2[1], vm0[1]));           // 101
+            m[2] = pfmas(Lz[1], (T)36, padd(tt1[3], vm0[3]));            // 010
+            m[9] = pfmas(Dz[1], (T)-36, psub(vp2[3], vm0[3]));           // 011
+            m[4] = pfmas(Dz[2], (T)-36, tt1[2]);                         // 200
+            m[7] = tt1[4];                                               // 110
+            m[5] = pfmas(Dz[2], (T)-36, tt1[5]);                         // 020
+            if (WALLY) { m[3] = padd(m[3], kwall[0]); m[6] = padd(m[6], kwall[1]); m[8] = padd(m[8], kwall[2]); m[9] = padd(m[9], kwall[3]); }
+
+            // ---- a8: finalise the two rows from their 216-scaled raw moments (m[1..3] lack their base 216 u), Eq. 12 ------
+            // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
+            const T hi = (T)(1.0 / 216.0);
+            const T lo = (T)(1.0 / 216.0 - (double)hi);
+            const P dR = pfmas(m[0], lo, pmuls(m[0], hi));
+            const P rho = padd(pbc<P, T>((T)1), dR);
+            const P den = padd(pbc<P, T>((T)216), m[0]);
+            const P inv = pk((T)1 / den.x, (T)1 / den.y);
+            const P nm0 = pmuls(m[0], (T)-1);
+            // u' = (216 u + J) / (216 + dR216) = u + (J - u dR216) / (216 + dR216)
+            P o[TSLB_NF];
+            o[0] = dR;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) o[1 + a] = pfma(pfma(uprev[a], nm0, m[1 + a]), inv, uprev[a]);
+            const P niso = pmuls(dR, (T)(-1.0 / 3.0));
+            const P nrho = pmuls(rho, (T)-1);
+            const P rx = pmul(nrho, o[1]), ry = pmul(nrho, o[2]), rz = pmul(nrho, o[3]);
+            // (the second moments are rebuilt from scratch every step, so a singly rounded 1/216 cannot compound there)
+            o[4] = pfma(rx, o[1], pfmas(m[4], hi, niso));
+            o[5] = pfma(ry, o[2], pfmas(m[5], hi, niso));
+            o[6] = pfma(rz, o[3], pfmas(m[6], hi, niso));
+            o[7] = pfma(rx, o[2], pmuls(m[7], hi));
+            o[8] = pfma(rx, o[3], pmuls(m[8], hi));
+            o[9] = pfma(ry, o[3], pmuls(m[9], hi));
+
+            // ---- into the output tile (the store thread has read the previous plane out of it) ------------------------------
+            mbar_wait(sb + B_OEMPTY, (uint32_t)((i - 1) & 1));
+            if (lane_out) {
+#pragma unroll
+                for (int f = 0; f < TSLB_NF; ++f) {
+                    sts(aO + f * (ROWS * COLS) * ES, o[f].x);
+                    sts(aO + (f * (ROWS * COLS) + COLS) * ES, o[f].y);
+                }
+            }
+            fence_async_smem();
+            warp_arrive(sb + B_OFULL, lane);
+            if (xedge || xtail) {
+                T *rp = Bbuf + ((long long)zt * L.plane + (long long)r0 * L.px);
+                if (xtail) {
+                    T *gp = rp + (col + TSLB_XOFF);
+#pragma unroll
+                    for (int f = 0; f < TSLB_NF; ++f) { gp[f * L.field] = o[f].x; gp[f * L.field + L.px] = o[f].y; }
+                }
+                if (xedge) {
+                    T *gp = rp + gcol;
+#pragma unroll
+                    for (int f = 0; f < TSLB_NF; ++f) { gp[f * L.field] = o[f].x; gp[f * L.field + L.px] = o[f].y; }
+                }
+            }
+        }
+        // ---- shift the march state ---------------------------------------------------------------------------------
+#pragma unroll
+        for (int g = 0; g < 6; ++g) {
+            if (g == 0 || g == 1 || g == 3) vp2[g] = vp1[g];
+            tt1[g] = tn[g];                              // Vp(zs-1) + centre(zs): used when plane zs+1 arrives
+            vp1[g] = vp0[g];
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) uprev[a] = rc[1 + a];
+        if (++stg == NS) { stg = 0; fpar ^= 1; }
     }
 }
 
@@ -576,7 +743,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
         const int zc = (c->nz + k - 1) / k;
         if (k > 1 && zc < 8) break;
         const long long ctas = cols * ((c->nz + zc - 1) / zc);
-        const long long slots = (long long)c->sm_count * TileGeom<T>::MINB;
+        const long long slots = (long long)c->sm_count;
         const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
         if (cost < best_cost) { best_cost = cost; best = k; }
@@ -601,6 +768,11 @@ bool tslb_tile_supported(const tslb_ctx *c, const char **why)
             if (why) *why = "bounce-back walls on x or z faces";
             return false;
         }
+    // every tile is full: the last tile of the y axis is shifted back, which needs at least one tile height of rows
+    if (c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float>::ROWS)) {
+        if (why) *why = "fewer rows (ny) than one tile";
+        return false;
+    }
     if (c->ws && !c->tmap_ok) {
         if (why) *why = "TMA descriptors unavailable";
         return false;
@@ -609,7 +781,12 @@ bool tslb_tile_supported(const tslb_ctx *c, const char **why)
     return true;
 }
 
-// TMA descriptors of the two moment buffers: 4-D tensor (x, y, z, field) of the padded SoA layout, box 36|32 x 10 x 1 x 10.
+// TMA descriptors of the two moment buffers: 4-D tensor (x, y, z, field) of the padded SoA layout.
+//   tm_main  box BXW x ROWS x 1 x 10: the tile rows of one source plane (with XPAD columns on each side)
+//   tm_row   box BXW x 1 x 1 x 10:    one halo row
+//   tm_store box COLS x ROWS x 1 x 10, tensor clipped at the last 16-byte boundary <= nx: the output tile (the kernel
+//            stores the nx % 4 (fp64: nx % 2) columns beyond it and the ghost columns from registers)
+// Out-of-bounds elements of a load are zero-filled: rows -1 / ny and planes -1 / nz beyond a wall or an open face.
 // cuTensorMapEncodeTiled is fetched through the runtime so that the library links against cudart only.
 cudaError_t tslb_tile_prepare(tslb_ctx *c)
 {
@@ -620,16 +797,25 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
     const Layout &L = c->L;
     const size_t es = tslb_elem(c);
-    const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)L.pz, TSLB_NF};
+    const bool f64 = c->dtype == TSLB_F64;
+    const cuuint32_t bxw = f64 ? TileDims<double>::BXW : TileDims<float>::BXW;
+    const cuuint32_t rows = f64 ? TileDims<double>::ROWS : TileDims<float>::ROWS;
+    const cuuint32_t cols = f64 ? TileDims<double>::COLS : TileDims<float>::COLS;
     const cuuint64_t strides[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
-    const cuuint32_t box[4] = {(cuuint32_t)(c->dtype == TSLB_F64 ? TileDims<double>::BXW : TileDims<float>::BXW),
-                               (cuuint32_t)(c->dtype == TSLB_F64 ? TileDims<double>::BY : TileDims<float>::BY), 1, TSLB_NF};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     for (int b = 0; b < 2; ++b) {
-        CUresult r = ((EncodeTiledFn)fn)(&c->tmap[b], c->dtype == TSLB_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
-                                         4, c->buf[b], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        const cuuint64_t dims_ld[4] = {(cuuint64_t)L.px, (cuuint64_t)L.ny, (cuuint64_t)L.nz, TSLB_NF};
+        const cuuint64_t dims_st[4] = {(cuuint64_t)((L.nx & ~(int)(16 / es - 1)) + TSLB_XOFF), (cuuint64_t)L.ny, (cuuint64_t)L.nz, TSLB_NF};
+        const cuuint32_t box_main[4] = {bxw, rows, 1, TSLB_NF}, box_row[4] = {bxw, 1, 1, TSLB_NF}, box_st[4] = {cols, rows, 1, TSLB_NF};
+        CUresult r = ((EncodeTiledFn)fn)(&c->tm_main[b], dt, 4, c->buf[b], dims_ld, strides, box_main, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r == CUDA_SUCCESS)
+            r = ((EncodeTiledFn)fn)(&c->tm_row[b], dt, 4, c->buf[b], dims_ld, strides, box_row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r == CUDA_SUCCESS)
+            r = ((EncodeTiledFn)fn)(&c->tm_store[b], dt, 4, c->buf[b], dims_st, strides, box_st, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
     const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
@@ -650,7 +836,9 @@ static void launch_tile(tslb_ctx *c, cudaStream_t st)
 {
     dim3 grid;
     TileParams<T> p = make_tile<T>(c, &grid);
-    sweep_tile_kernel<T, WALLY, ORDER><<<grid, TileDims<T>::WARPS * 32, TileDims<T>::SMEM_BYTES, st>>>(c->tmap[c->cur], (T *)c->buf[1 - c->cur], p);
+    const int a = c->cur, b = 1 - c->cur;
+    sweep_tile_kernel<T, WALLY, ORDER><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a], c->tm_store[b],
+                                                                                                   (T *)c->buf[b], p);
 }
 
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)

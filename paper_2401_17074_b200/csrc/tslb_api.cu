@@ -37,17 +37,16 @@ size_t scratch_bytes(const tslb_ctx *c)
 
 size_t buffer_bytes(const tslb_ctx *c) { return align256((size_t)TSLB_NF * (size_t)c->L.field * tslb_elem(c)); }
 
-// padded internal layout (tslb_internal.h): one ghost layer on every side, 16-byte rows, never smaller than a TMA box
+// padded internal layout (tslb_internal.h): ghost columns x = -1 and x = nx, node x = 0 on a 16-byte boundary, 16-byte rows,
+// never narrower than a TMA box
 Layout make_layout(int nx, int ny, int nz)
 {
     Layout L;
     L.nx = nx; L.ny = ny; L.nz = nz;
-    L.px = (nx + 2 + 3) & ~3;
+    L.px = (nx + 2 * TSLB_XOFF + 3) & ~3;
     if (L.px < 72) L.px = 72;
-    L.py = ny + 2 < TILE_MAX_BY ? TILE_MAX_BY : ny + 2;
-    L.pz = nz + 2;
-    L.plane = (long long)L.px * L.py;
-    L.field = L.plane * L.pz;
+    L.plane = (long long)L.px * ny;
+    L.field = L.plane * nz;
     return L;
 }
 
@@ -73,18 +72,17 @@ bool any_open(const tslb_ctx *c)
         if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT) return true;
     return false;
 }
-bool any_periodic(const tslb_ctx *c) { return c->kind[0] == TSLB_BC_PERIODIC || c->kind[2] == TSLB_BC_PERIODIC || c->kind[4] == TSLB_BC_PERIODIC; }
 
-// Boundary nodes of the open faces filled at time t (oracle step 1) and, for the tile kernel, valid ghost layers.
-// halo_valid: 0 = nothing done for (buf[cur], t); 1 = boundary nodes filled; 2 = ghost layers valid as well.
-// The tile kernel writes the periodic ghost images of every node it stores, so after a tile step the ghost layers of
-// the new buffer are already valid -- unless open faces exist next to a periodic axis (the fill changes boundary
-// nodes whose images then have to be refreshed).  Ghost cells beyond walls and open faces are never used by a node
-// that is advanced; they only have to be finite (the workspace is zeroed at bind time).
+// Boundary nodes of the open faces filled at time t (oracle step 1) and, for the tile kernel, valid ghost columns.
+// halo_valid: 0 = nothing done for (buf[cur], t); 1 = boundary nodes filled; 2 = ghost columns valid as well;
+// 3 = written by a tile step: the ghost columns are valid (the sweep stores the periodic x images of the nodes it
+// writes), the fill is pending.  Only when open faces exist next to a periodic x axis does the fill change nodes whose
+// images then have to be refreshed.  Ghost columns of a non-periodic x axis are never used by a node that is advanced;
+// they only have to be finite (the workspace is zeroed at bind time).
 cudaError_t refresh_boundary(tslb_ctx *c, bool need_halo, cudaStream_t st)
 {
     cudaError_t e = cudaSuccess;
-    const bool refill = any_open(c) && any_periodic(c);
+    const bool refill = any_open(c) && c->kind[0] == TSLB_BC_PERIODIC;
     if (c->halo_valid < 1 || (c->halo_valid == 3)) {
         e = tslb_launch_fill(c, c->buf[c->cur], st);
         if (e != cudaSuccess) return e;
@@ -198,6 +196,10 @@ int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
     // padding cells are never written by the kernels: give them a defined (zero) value once
     e = cudaMemset(dev_ptr, 0, 2 * buffer_bytes(c));
     if (e != cudaSuccess) return cuda_fail(c, "cudaMemset(workspace)", e);
+    // the memset runs on the legacy default stream; later calls enqueue on the caller's (possibly non-blocking) stream:
+    // bind is one-off, so simply wait for it
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(c, "cudaDeviceSynchronize(bind)", e);
     c->tmap_ok = 0;
     e = tslb_tile_prepare(c);            // TMA descriptors of the two buffers
     if (e != cudaSuccess) {              // not fatal: the gather kernel covers everything; TSLB_KERNEL_TILE then reports why

@@ -10,19 +10,23 @@
 #define TSLB_NF 10  // dr = rho - 1, ux, uy, uz, Pxx, Pyy, Pzz, Pxy, Pxz, Pyz
 
 // ---- internal moment-buffer layout -------------------------------------------------
-// SoA, one padded box per field: [pz = nz+2][py][px] elements, x fastest.  Node (x,y,z), -1 <= x <= nx etc.
-// (index -1 and n are the ghost layers), lives at element  (z+1)*plane + (y+1)*px + (x+1)  of its field.
-// px is a multiple of 4 (16-byte rows for TMA) and px >= 64, py >= ny+2 and py >= the TMA box height.
+// SoA, one padded box per field: [nz][ny][px] elements, x fastest.  Node (x,y,z), -1 <= x <= nx (x = -1 and x = nx are the
+// ghost columns: the periodic images along x, which the contiguous TMA rows cannot wrap), lives at element
+//     z*plane + y*px + (x + TSLB_XOFF)      of its field.
+// TSLB_XOFF = 4 puts node x = 0 on a 16-byte boundary for both dtypes (TMA box origins and the TMA store of the output
+// tile need 16-byte aligned addresses); px is a multiple of 4 with px >= nx + 8.  There are no ghost rows or planes:
+// the tile kernel wraps y and z by TMA coordinates, the gather kernel by index arithmetic.
+#define TSLB_XOFF 4
 struct Layout {
     int nx, ny, nz;
-    int px, py, pz;
-    long long plane;  // px*py
-    long long field;  // px*py*pz
+    int px;
+    long long plane;  // px*ny
+    long long field;  // px*ny*nz
 };
 
 __host__ __device__ inline long long lay_idx(const Layout &L, int x, int y, int z)
 {
-    return (long long)(z + 1) * L.plane + (long long)(y + 1) * L.px + (x + 1);
+    return (long long)z * L.plane + (long long)y * L.px + (x + TSLB_XOFF);
 }
 
 // Device-visible description of one lattice + its boundary set (passed by value).
@@ -51,7 +55,6 @@ struct FillParams {
 
 // geometry of the TMA-staged tile kernel (kernels_tile.cu): a warp owns 2 rows x 30 columns (+ 1 halo lane per side)
 #define TILE_COLS 30
-#define TILE_MAX_BY 18                  // tallest TMA box of any instantiation (rows): the padded layout is at least this high
 
 struct tslb_ctx {
     int nx, ny, nz, dtype;
@@ -66,12 +69,12 @@ struct tslb_ctx {
     size_t ws_bytes;
     void *buf[2];     // moment buffers, internal form (padded SoA, field 0 holds rho - 1)
     double *scratch;  // diagnostics partials
-    CUtensorMap tmap[2];  // TMA descriptors of buf[0], buf[1]
+    CUtensorMap tm_main[2], tm_row[2], tm_store[2];  // TMA descriptors of buf[0], buf[1]: tile rows, one halo row, output tile
     int tmap_ok;
     int cur;          // buf[cur] holds time t
     long long t;
     int have_state;
-    int halo_valid;   // ghost layers + open-face boundary nodes of buf[cur] are up to date for time t
+    int halo_valid;   // ghost columns + open-face boundary nodes of buf[cur] are up to date for time t (tslb_api.cu)
     int kernel_req;   // TSLB_KERNEL_*
     int sm_count;
     long long launches;

@@ -42,7 +42,9 @@ def with_faces(w, faces, g=(0.0, 0.0, 0.0), inlet_face=None, seed=5):
 # ---------------------------------------------------------------------------------------------
 # small cases: several tiles + ragged tails, every boundary kind, both dtypes, every kernel
 # ---------------------------------------------------------------------------------------------
-SHAPES = [(3, 3, 3), (4, 3, 5), (5, 7, 9), (33, 17, 6), (64, 12, 10), (130, 9, 7), (136, 36, 5), (260, 20, 4)]
+# (the tile kernel needs ny >= one tile height: 14 rows fp32, 8 rows fp64; smaller lattices run on the gather kernel only)
+SHAPES = [(3, 3, 3), (4, 3, 5), (5, 7, 9), (33, 17, 6), (64, 12, 10), (130, 9, 7), (136, 36, 5), (260, 20, 4),
+          (61, 14, 5), (3, 29, 3), (124, 15, 33), (60, 28, 3), (59, 43, 4)]
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -73,7 +75,7 @@ BC_SETS = {
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("bc", sorted(BC_SETS))
-@pytest.mark.parametrize("shape", [(4, 3, 5), (12, 10, 7), (136, 11, 6)])
+@pytest.mark.parametrize("shape", [(4, 3, 5), (12, 10, 7), (136, 11, 6), (70, 16, 6), (65, 31, 5)])
 def test_boundary_sets(B, oracle_mod, shape, bc, dtype):
     w = with_faces(W.random_state(*shape, seed=17, dtype=dtype, tau=0.58), **BC_SETS[bc])
     for k in kernels_for(B, w):
@@ -226,9 +228,9 @@ def test_set_moments_mid_run_and_timing_api(B, oracle_mod):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_order2_parity(B, oracle_mod, dtype):
     cases = [W.random_state(70, 21, 9, seed=12, dtype=dtype, tau=0.64),
-             with_faces(W.random_state(66, 11, 7, seed=13, dtype=dtype, tau=0.6),
+             with_faces(W.random_state(66, 15, 7, seed=13, dtype=dtype, tau=0.6),
                         {W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, g=(2e-4, 0, -1e-4)),
-             with_faces(W.random_state(12, 10, 14, seed=14, dtype=dtype, tau=0.58), **BC_SETS["jet_like"])]
+             with_faces(W.random_state(12, 17, 14, seed=14, dtype=dtype, tau=0.58), **BC_SETS["jet_like"])]
     for w in cases:
         w.order = 2
         for k in kernels_for(B, w):
