@@ -35,16 +35,20 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build_lib(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build_lib(force: bool = False, verbose: bool = False, out: str = LIB, extra_flags=()) -> str:
+    """Build the library.  `out` / `extra_flags` (e.g. -DTILE_F32_NS=2) build a variant beside the default one;
+    binding.load_library picks it up through the TSLB_LIBRARY environment variable."""
+    if out == LIB and not extra_flags and not force and not needs_build():
         return LIB
-    tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    tmp = out + ".tmp%d" % os.getpid()
+    cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":
-    print(build_lib(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    _defs = [a for a in sys.argv[1:] if a.startswith("-D")]
+    _out = [a.split("=", 1)[1] for a in sys.argv[1:] if a.startswith("--out=")]
+    print(build_lib(force="--force" in sys.argv, verbose="--verbose" in sys.argv, out=_out[0] if _out else LIB, extra_flags=_defs))

@@ -30,6 +30,9 @@
 // only the bracket (exact differences of stored velocities) is added at each stage, and the product of the tap sums,
 // 216 u_a(x), is re-attached in closed form at the end:  u' = u + (J_small - u dR) / (216 + dR).
 #include "tslb_internal.h"
+#ifdef TSLB_EXP_ZCHUNK
+#include <stdlib.h>
+#endif
 
 namespace {
 
@@ -54,6 +57,10 @@ template <typename P, typename T> __device__ __forceinline__ P pbc(T s) { return
 template <typename P, typename T> __device__ __forceinline__ P pfmas(P a, T s, P c) { return pfma(a, pbc<P, T>(s), c); }
 template <typename P, typename T> __device__ __forceinline__ P pmuls(P a, T s) { return pmul(a, pbc<P, T>(s)); }
 template <typename P> __device__ __forceinline__ P pswap(P a) { return pk(a.y, a.x); }
+// 1/x for x = 216 + dR216 (always close to 216): fp32 uses the hardware approximation (MUFU.RCP, <= 1 ulp) -- the quotient
+// only scales the per-step INCREMENT of u (increment form), so its rounding is far below the stored precision
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double rcp_fast(double x) { return 1.0 / x; }
 
 template <typename P> __device__ __forceinline__ P shfl_up1(P v)
 {
@@ -227,6 +234,9 @@ template <typename T> struct TileGeom;
 #endif
 #ifndef TILE_F32_NS
 #define TILE_F32_NS 3
+#endif
+#ifndef TILE_ZC_MAX
+#define TILE_ZC_MAX 48
 #endif
 template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS; };
 template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2; };
@@ -463,23 +473,6 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         }
         warp_arrive(sb + B_EMPTY + 8 * stg, lane);       // the stage can be refilled: everything needed is in registers
 
-        // ---- increment form along y (DESIGN.md "fp32 formulation"): exact differences of the stored velocities,
-        //      Ly = (up - c) + (dn - c), Wy = (up - dn) * sgn with up / dn the neighbour rows (hu = (u(r0-1), u(r0+2)), the
-        //      other neighbour is the pack's other row); a node beyond a wall has u = 0 (zero-filled halo row).  They enter
-        //      the y pass of the groups that carry a first-order coefficient:  E += incE, O += incO  with
-        //      (kx,kz) = (1,0): 3 Ly_x, sg3 Wy_x;   (0,0): sg3 Wy_y, 3 Ly_y;   (0,1): 3 Ly_z, sg3 Wy_z. -------------------------
-        const P sg3 = pk((T)3, (T)-3);
-        P incE[3], incO[3];        // indexed by velocity component
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const P uc = rc[1 + a];
-            const P cs = pswap(uc);
-            const P ly3 = pmuls(pfmas(uc, (T)-2, padd(hu[a], cs)), (T)3);
-            const P wy3 = pmul(psub(hu[a], cs), sg3);
-            incE[a] = a == 1 ? wy3 : ly3;
-            incO[a] = a == 1 ? ly3 : wy3;
-        }
-
         // ---- a2: Hermite coefficients of the own rows, all three rounds; y-pass combinations of the 8 groups -------------
         // qs = swap(qc) = (M of row r0+1, P of row r0): what the two rows of the pack receive from each other.
         // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)), so with qh = (P(r0-1), M(r0+2)) read from the
@@ -490,12 +483,10 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #define TSLB_MAIN_GROUP(KX, KZ)                                                                   \
             if (kvalid<ORDER>(KX, 0, KZ)) {                                                       \
                 constexpr int q = qidx(KX, KZ);                                                   \
-                constexpr int ia = (KX == 1 && KZ == 0) ? 0 : ((KX == 0 && KZ == 0) ? 1 : ((KX == 0 && KZ == 1) ? 2 : -1)); \
                 P qc, qp;                                                                         \
                 ycombos<ORDER, KX, KZ, P, T>(A, qc, qp, cen[q]);                                  \
                 const P qs = pswap(qc);                                                           \
-                if (ia >= 0) { qe[q] = padd(qs, incE[ia < 0 ? 0 : ia]); qo[q] = pfma(qs, nsg, incO[ia < 0 ? 0 : ia]); } \
-                else { qe[q] = qs; qo[q] = pmul(qs, nsg); }                                       \
+                qe[q] = qs; qo[q] = pmul(qs, nsg);                                                \
                 sts(w + q * EXW * ES, qp.x);                                                      \
                 sts(w + 2 * SLOT_BYTES + q * EXW * ES, qp.y);                                     \
             }
@@ -512,6 +503,25 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #undef TSLB_MAIN_GROUP
         }
         warp_arrive(bQown + 8 * (i & 1), lane);
+
+        // ---- increment form along y (DESIGN.md "fp32 formulation"): exact differences of the stored velocities,
+        //      Ly = (up - c) + (dn - c), Wy = (up - dn) * sgn with up / dn the neighbour rows (hu = (u(r0-1), u(r0+2)), the
+        //      other neighbour is the pack's other row); a node beyond a wall has u = 0 (zero-filled halo row).  They enter
+        //      the y pass of the groups that carry a first-order coefficient:  E += incE, O += incO  with
+        //      (kx,kz) = (1,0): 3 Ly_x, sg3 Wy_x;   (0,0): sg3 Wy_y, 3 Ly_y;   (0,1): 3 Ly_z, sg3 Wy_z. -------------------------
+        const P sg3 = pk((T)3, (T)-3);
+        // (after the publish: the neighbours do not wait for this)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const P uc = rc[1 + a];
+            const P cs = pswap(uc);
+            const P ly3 = pmuls(pfmas(uc, (T)-2, padd(hu[a], cs)), (T)3);
+            const P wy3 = pmul(psub(hu[a], cs), sg3);
+            const int q = a == 0 ? qidx(1, 0) : (a == 1 ? qidx(0, 0) : qidx(0, 1));
+            qe[q] = padd(qe[q], a == 1 ? wy3 : ly3);
+            qo[q] = padd(qo[q], a == 1 ? ly3 : wy3);
+        }
+
 
         // ---- the neighbours' combinations -----------------------------------------------------------------------------------
         mbar_wait(bQdn + 8 * (i & 1), (uint32_t)((i >> 1) & 1));
@@ -668,7 +678,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             const P dR = pfmas(m[0], lo, pmuls(m[0], hi));
             const P rho = padd(pbc<P, T>((T)1), dR);
             const P den = padd(pbc<P, T>((T)216), m[0]);
-            const P inv = pk((T)1 / den.x, (T)1 / den.y);
+            const P inv = pk(rcp_fast(den.x), rcp_fast(den.y));
             const P nm0 = pmuls(m[0], (T)-1);
             // u' = (216 u + J) / (216 + dR216) = u + (J - u dR216) / (216 + dR216)
             P o[TSLB_NF];
@@ -734,26 +744,36 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
     const int gx = (c->nx + TileDims<T>::COLS - 1) / TileDims<T>::COLS;
     const int gy = (c->ny + TileDims<T>::ROWS - 1) / TileDims<T>::ROWS;
-    // z chunks (one CTA per SM is resident): pick the chunk count whose number of waves x (chunk length + 2 halo planes)
-    // is smallest
+    // z chunks (one CTA per SM is resident): pick the chunk count whose number of waves x (chunk length + 2 halo planes +
+    // ring fill) is smallest, among chunks of at most TILE_ZC_MAX planes.  Long marches let the CTAs of a wave drift apart
+    // in z until the halo rows / columns that neighbouring tiles share have left L2 before their second reader arrives
+    // (measured at 512^3 fp32: DRAM reads 7.09 / 6.62 / 6.13 GB per step for chunks of 128 / 64 / 32 planes, 5.4 GB
+    // algorithmic; profiles/README.md).
     const long long cols = (long long)gx * gy;
     int best = 1;
     double best_cost = 1e300;
-    for (int k = 1; k <= 64 && k <= c->nz; ++k) {
+    for (int k = 1; k <= c->nz; ++k) {
         const int zc = (c->nz + k - 1) / k;
         if (k > 1 && zc < 8) break;
+        if (zc > TILE_ZC_MAX && (c->nz + k) / (k + 1) >= 8) continue;
         const long long ctas = cols * ((c->nz + zc - 1) / zc);
         const long long slots = (long long)c->sm_count;
         const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
         if (cost < best_cost) { best_cost = cost; best = k; }
     }
-    const int zc = (c->nz + best - 1) / best;
+    int zc = (c->nz + best - 1) / best;
+#ifdef TSLB_EXP_ZCHUNK
+    if (getenv("TSLB_ZCHUNK")) zc = atoi(getenv("TSLB_ZCHUNK"));
+#endif
     p.zchunk = zc;
     *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
     return p;
 }
 
+#ifndef TSLB_L2PROMO
+#define TSLB_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -809,10 +829,10 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
         const cuuint64_t dims_st[4] = {(cuuint64_t)((L.nx & ~(int)(16 / es - 1)) + TSLB_XOFF), (cuuint64_t)L.ny, (cuuint64_t)L.nz, TSLB_NF};
         const cuuint32_t box_main[4] = {bxw, rows, 1, TSLB_NF}, box_row[4] = {bxw, 1, 1, TSLB_NF}, box_st[4] = {cols, rows, 1, TSLB_NF};
         CUresult r = ((EncodeTiledFn)fn)(&c->tm_main[b], dt, 4, c->buf[b], dims_ld, strides, box_main, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                         CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r == CUDA_SUCCESS)
             r = ((EncodeTiledFn)fn)(&c->tm_row[b], dt, 4, c->buf[b], dims_ld, strides, box_row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r == CUDA_SUCCESS)
             r = ((EncodeTiledFn)fn)(&c->tm_store[b], dt, 4, c->buf[b], dims_st, strides, box_st, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

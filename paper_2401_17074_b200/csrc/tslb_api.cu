@@ -39,11 +39,14 @@ size_t buffer_bytes(const tslb_ctx *c) { return align256((size_t)TSLB_NF * (size
 
 // padded internal layout (tslb_internal.h): ghost columns x = -1 and x = nx, node x = 0 on a 16-byte boundary, 16-byte rows,
 // never narrower than a TMA box
+#ifndef TSLB_PXALIGN
+#define TSLB_PXALIGN 4
+#endif
 Layout make_layout(int nx, int ny, int nz)
 {
     Layout L;
     L.nx = nx; L.ny = ny; L.nz = nz;
-    L.px = (nx + 2 * TSLB_XOFF + 3) & ~3;
+    L.px = (nx + 2 * TSLB_XOFF + TSLB_PXALIGN - 1) & ~(TSLB_PXALIGN - 1);
     if (L.px < 72) L.px = 72;
     L.plane = (long long)L.px * ny;
     L.field = L.plane * nz;
