@@ -30,9 +30,6 @@
 // only the bracket (exact differences of stored velocities) is added at each stage, and the product of the tap sums,
 // 216 u_a(x), is re-attached in closed form at the end:  u' = u + (J_small - u dR) / (216 + dR).
 #include "tslb_internal.h"
-#ifdef TSLB_EXP_ZCHUNK
-#include <stdlib.h>
-#endif
 
 namespace {
 
@@ -233,10 +230,10 @@ template <typename T> struct TileGeom;
 #define TILE_F32_WY 7
 #endif
 #ifndef TILE_F32_NS
-#define TILE_F32_NS 3
+#define TILE_F32_NS 2
 #endif
 #ifndef TILE_ZC_MAX
-#define TILE_ZC_MAX 48
+#define TILE_ZC_MAX 64
 #endif
 template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS; };
 template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2; };
@@ -763,9 +760,6 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
         if (cost < best_cost) { best_cost = cost; best = k; }
     }
     int zc = (c->nz + best - 1) / best;
-#ifdef TSLB_EXP_ZCHUNK
-    if (getenv("TSLB_ZCHUNK")) zc = atoi(getenv("TSLB_ZCHUNK"));
-#endif
     p.zchunk = zc;
     *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
     return p;
