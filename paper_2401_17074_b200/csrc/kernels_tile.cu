@@ -235,15 +235,33 @@ template <typename T> struct TileGeom;
 #ifndef TILE_ZC_MAX
 #define TILE_ZC_MAX 64
 #endif
-template <> struct TileGeom<float> { static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS; };
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2; };
+// REG_MAIN / REG_HALO != 0: the register file is re-divided after launch with setmaxnreg (the main warps, which carry the
+// z-march state, get more than an even share; needs the main warps to be whole warpgroups of 4, and NIDLE idle warps that
+// complete the helpers' warpgroup).  fp64: 8 main warps at 208 registers + 2 halo + 2 idle at 80 (an even share of the
+// 16384 registers of an SM sub-partition among its 3 warps would be 168, which spills).  Register counts are multiples of
+// 16: a warp's allocation is rounded up to 512 registers, and a setmaxnreg.inc that cannot be satisfied blocks forever
+// (measured: 216 + 216 + 80 and 208 + 208 + 96 per sub-partition hang).  The pool is what the CTA was given at LAUNCH
+// (threads x MAXREG), not the whole register file: the re-divided total must not exceed it.
+#ifndef TILE_F32_RM
+#define TILE_F32_RM 0
+#define TILE_F32_RH 0
+#define TILE_F32_NIDLE 0
+#endif
+template <> struct TileGeom<float> {
+    static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, NIDLE = TILE_F32_NIDLE, REG_MAIN = TILE_F32_RM, REG_HALO = TILE_F32_RH;
+};
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = 208, REG_HALO = 80; };
 constexpr int rup128(int bytes) { return (bytes + 127) / 128 * 128; }
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;
     static constexpr int WX = G::WX, WY = G::WY, NS = G::NS;
-    static constexpr int NMAIN = WX * WY, NHALO = 2, WARPS = NMAIN + NHALO, THREADS = WARPS * 32;
+    static constexpr int NMAIN = WX * WY, NHALO = 2, WARPS = NMAIN + NHALO, THREADS = (WARPS + G::NIDLE) * 32;
     // one CTA per SM: the whole register file, 16384 registers per SM sub-partition, warps dealt round-robin to the four
-    static constexpr int MAXREG = (16384 / (((WARPS + 3) / 4) * 32)) / 8 * 8;     // 128 (fp32, 16 warps), 168 (fp64, 10 warps)
+    static constexpr int MAXREG = (16384 / (((WARPS + G::NIDLE + 3) / 4) * 32)) / 8 * 8;     // at launch: 128 (fp32, 16 warps), 168 (fp64, 12 warps)
+    static_assert(G::REG_MAIN == 0 || (NMAIN % 4 == 0 && (NHALO + G::NIDLE) % 4 == 0), "setmaxnreg works on warpgroups of 4 warps");
+    static_assert(G::REG_MAIN % 16 == 0 && G::REG_HALO % 16 == 0, "a warp's registers are allocated in units of 512");
+    static_assert(G::REG_MAIN == 0 || NMAIN * G::REG_MAIN + (NHALO + G::NIDLE) * G::REG_HALO <= (WARPS + G::NIDLE) * MAXREG, "setmaxnreg pool = launch allocation");
+    static_assert(G::REG_MAIN == 0 || (NMAIN / 4) * G::REG_MAIN + ((NHALO + G::NIDLE) / 4) * G::REG_HALO <= 512, "16384 registers per sub-partition");
     static constexpr int COLS = TILE_COLS * WX;                  // output columns per CTA (60)
     static constexpr int ROWS = 2 * WY;                          // output rows per CTA
     static constexpr int XPAD = 4;                               // box origin = first tile column - XPAD
@@ -308,6 +326,11 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     }
     __syncthreads();
 
+    if (TileGeom<T>::REG_MAIN != 0) {
+        if (wid >= TD::NMAIN) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_HALO ? TileGeom<T>::REG_HALO : 24));
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_MAIN ? TileGeom<T>::REG_MAIN : 24));
+    }
+    if (wid >= TD::WARPS) return;                         // idle warps (they only complete a warpgroup for setmaxnreg)
     if (wid >= TD::NMAIN) {
         // =================================================== halo warps ===================================================
         const int h = wid - TD::NMAIN;
