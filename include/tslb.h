@@ -73,15 +73,15 @@ typedef struct tslb_inlet_params {
 
 /* Create a context for an nx x ny x nz lattice with BGK relaxation time tau (omega = 1/tau,
  * nu = (tau - 1/2)/3).  Pure host call (no CUDA).  Defaults: all faces PERIODIC, g = 0.
- * TSLB_EINVAL: out == NULL, a dimension < 3 or the lattice exceeds 2^31-1 nodes, tau not finite or
+ * TSLB_EINVAL: out == NULL, a dimension < 3, the lattice exceeds 2^31-1 nodes or ny > 131070, tau not finite or
  * <= 0.5, unknown dtype.  TSLB_ENOMEM: host allocation failed. */
 int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out);
 
 /* Free the context (host memory only; the workspace and inlet planes stay the caller's). NULL is a no-op. */
 void tslb_destroy(tslb_ctx *ctx);
 
-/* Bytes of device memory the context needs: two moment buffers in the internal layout (10 fields, each padded
- * by one ghost layer per side and to 16-byte rows) plus scratch for the diagnostics reduction.  0 if ctx == NULL. */
+/* Bytes of device memory the context needs: two moment buffers in the internal layout (10 fields, rows padded by the two
+ * ghost columns to a multiple of 16 bytes) plus scratch for the diagnostics reduction.  0 if ctx == NULL. */
 size_t tslb_workspace_bytes(const tslb_ctx *ctx);
 
 /* Give the context its device memory (256-byte aligned, >= tslb_workspace_bytes, caller-owned).  First
@@ -116,7 +116,7 @@ int tslb_set_kernel(tslb_ctx *ctx, int kernel);
 /* The kernel the next tslb_step would launch (TSLB_KERNEL_GATHER or TSLB_KERNEL_TILE), or -1. */
 int tslb_active_kernel(const tslb_ctx *ctx);
 
-/* Advance n time steps (n >= 0): n x { boundary-node fill + ghost-layer refresh at time t ; fused stream-collide
+/* Advance n time steps (n >= 0): n x { boundary-node fill + ghost-column refresh at time t ; fused stream-collide
  * sweep A -> B ; swap }.  Asynchronous on `stream`; no host<->device traffic.  TSLB_ESTATE before bind/set_moments,
  * TSLB_EINVAL for n < 0 or an inconsistent boundary set, TSLB_ECUDA on a launch error. */
 int tslb_step(tslb_ctx *ctx, int n, void *stream);
@@ -126,6 +126,15 @@ int tslb_step(tslb_ctx *ctx, int n, void *stream);
 int tslb_get_moments(tslb_ctx *ctx, void *dev_dst, void *stream);
 /* Same to host memory; synchronises `stream` before returning. */
 int tslb_get_moments_host(tslb_ctx *ctx, void *host_dst, void *stream);
+
+/* Checkpoint / resume (the 10 moment arrays are the whole state).  tslb_export_state writes the state
+ * bit for bit as it is held -- the layout of tslb_get_moments, except that field 0 is rho - 1, the shifted form the buffers
+ * store (tslb_get_moments adds the 1 back, which rounds fp32 values once) -- and returns the
+ * step counter, which the seeded inlet noise depends on.  tslb_import_state loads such an array and restores the counter:
+ * run 2n  ==  run n, export, import, run n  bitwise, on the same kernel.  Device pointers, enqueued on `stream`.
+ * TSLB_EINVAL: NULL array, step_count < 0; TSLB_ESTATE: no workspace / (export) no state. */
+int tslb_export_state(tslb_ctx *ctx, void *dev_dst, long long *step_count, void *stream);
+int tslb_import_state(tslb_ctx *ctx, const void *dev_src, long long step_count, void *stream);
 
 /* Mass sum(rho), momentum sum(rho u)[3] and kinetic energy 1/2 sum(rho |u|^2) over the nodes that are not
  * on an open (inlet/outlet) face, accumulated in fp64 with warp-shuffle reductions and a fixed-order final

@@ -24,7 +24,8 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile
 SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_workspace", "tslb_set_moments",
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
-           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics")
+           "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
+           "tslb_export_state", "tslb_import_state")
 
 
 class InletParams(C.Structure):
@@ -68,6 +69,8 @@ def load_library(path: Optional[str] = None):
     lib.tslb_get_moments.argtypes = [vp, vp, vp]
     lib.tslb_get_moments_host.argtypes = [vp, vp, vp]
     lib.tslb_diagnostics.argtypes = [vp, vp, vp]
+    lib.tslb_export_state.argtypes = [vp, vp, C.POINTER(C.c_longlong), vp]
+    lib.tslb_import_state.argtypes = [vp, vp, C.c_longlong, vp]
     lib.tslb_plane_statistics.argtypes = [vp, ip, vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
@@ -205,6 +208,20 @@ class TSLB:
         ptr, keep = _host_ptr(out, self, (10,) + self.shape)
         self._chk(self._lib.tslb_get_moments_host(self._h, ptr, _stream_ptr(stream)), "tslb_get_moments_host")
         return out
+
+    def export_state(self, out=None, stream=None):
+        """(raw state [10][nz][ny][nx] with field 0 = rho - 1, step counter): the bit-exact checkpoint."""
+        import torch
+        if out is None:
+            out = torch.empty((10,) + self.shape, dtype=self.torch_dtype, device="cuda")
+        self._check_tensor(out, "out", (10,) + self.shape)
+        t = C.c_longlong(0)
+        self._chk(self._lib.tslb_export_state(self._h, C.c_void_p(out.data_ptr()), C.byref(t), _stream_ptr(stream)), "tslb_export_state")
+        return out, t.value
+
+    def import_state(self, S, step_count: int, stream=None):
+        self._check_tensor(S, "state", (10,) + self.shape)
+        self._chk(self._lib.tslb_import_state(self._h, C.c_void_p(S.data_ptr()), int(step_count), _stream_ptr(stream)), "tslb_import_state")
 
     def diagnostics(self, stream=None):
         """(mass, px, py, pz, kinetic energy) as a CUDA fp64 tensor of 5."""

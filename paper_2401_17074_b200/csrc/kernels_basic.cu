@@ -86,8 +86,8 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z;
     if (x >= p.L.nx || y >= p.L.ny) return;
+    for (int z = blockIdx.z; z < p.L.nz; z += gridDim.z) {
     const long long N = p.L.field;
     const long long ip = lay_idx(p.L, x, y, z);
     const Site<T> own = load_site(A, N, ip);
@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
         B[N + ip] = own.ux; B[2 * N + ip] = own.uy; B[3 * N + ip] = own.uz;
         B[4 * N + ip] = own.pxx; B[5 * N + ip] = own.pyy; B[6 * N + ip] = own.pzz;
         B[7 * N + ip] = own.pxy; B[8 * N + ip] = own.pxz; B[9 * N + ip] = own.pyz;
-        return;
+        continue;
     }
 
     // upstream coordinate x - c for c = -1, 0, +1 (index c+1), with periodic wrap; bounce flags
@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
     B[7 * N + ip] = fma(Sxy, lo, Sxy * hi) - rho * ux * uy;
     B[8 * N + ip] = fma(Sxz, lo, Sxz * hi) - rho * ux * uz;
     B[9 * N + ip] = fma(Syz, lo, Syz * hi) - rho * uy * uz;
+    }   // z
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -280,7 +281,9 @@ __global__ void halo_kernel(T *__restrict__ M, FillParams p)
 // ---------------------------------------------------------------------------------------------
 // API layout [10][nz][ny][nx] <-> internal padded layout (field 0: rho <-> rho - 1; exact for 0.5 <= rho <= 2)
 // ---------------------------------------------------------------------------------------------
-template <typename T, int DIR>
+// SHIFT = 1: field 0 is rho on the API side (tslb_set/get_moments); SHIFT = 0: field 0 stays rho - 1 (the raw checkpoint of
+// tslb_export_state / tslb_import_state, bit-for-bit the internal state)
+template <typename T, int DIR, int SHIFT>
 __global__ void convert_kernel(const T *__restrict__ src, T *__restrict__ dst, Layout L)
 {
     const long long N = (long long)L.nx * L.ny * L.nz;
@@ -292,8 +295,8 @@ __global__ void convert_kernel(const T *__restrict__ src, T *__restrict__ dst, L
         const long long r = s / L.nx;
         const int y = (int)(r % L.ny), z = (int)(r / L.ny);
         const long long j = k * L.field + lay_idx(L, x, y, z);
-        if (DIR > 0) { T v = src[i]; if (k == 0) v -= (T)1; dst[j] = v; }
-        else { T v = src[j]; if (k == 0) v += (T)1; dst[i] = v; }
+        if (DIR > 0) { T v = src[i]; if (SHIFT && k == 0) v -= (T)1; dst[j] = v; }
+        else { T v = src[j]; if (SHIFT && k == 0) v += (T)1; dst[i] = v; }
     }
 }
 
@@ -311,20 +314,26 @@ template <typename T>
 __global__ void __launch_bounds__(TSLB_DIAG_THREADS) diag_partial_kernel(const T *__restrict__ A, FillParams p,
                                                                           double *__restrict__ partial)
 {
-    const long long Ns = (long long)p.L.nx * p.L.ny * p.L.nz;
+    // one warp per lattice row (y, z), lanes along x: coalesced, one division per row; the row -> warp and x -> lane
+    // assignment is fixed, so the sums are bitwise reproducible
     const long long N = p.L.field;
-    const long long stride = (long long)gridDim.x * blockDim.x;
+    const int nrows = p.L.ny * p.L.nz;
+    const int wpb = blockDim.x >> 5;
+    const int lane_ = threadIdx.x & 31;
+    const bool open_x0 = is_open_kind(p.kind[0]), open_x1 = is_open_kind(p.kind[1]);
     double acc[5] = {0, 0, 0, 0, 0};
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < Ns; s += stride) {
-        const int x = (int)(s % p.L.nx);
-        const long long r = s / p.L.nx;
-        const int y = (int)(r % p.L.ny), z = (int)(r / p.L.ny);
-        if (on_open_face(p, x, y, z)) continue;
-        const long long i = lay_idx(p.L, x, y, z);
-        const double rho = 1.0 + (double)A[i];
-        const double ux = A[N + i], uy = A[2 * N + i], uz = A[3 * N + i];
-        acc[0] += rho; acc[1] += rho * ux; acc[2] += rho * uy; acc[3] += rho * uz;
-        acc[4] += 0.5 * rho * (ux * ux + uy * uy + uz * uz);
+    for (int row = blockIdx.x * wpb + (threadIdx.x >> 5); row < nrows; row += gridDim.x * wpb) {
+        const int y = row % p.L.ny, z = row / p.L.ny;
+        if ((y == 0 && is_open_kind(p.kind[2])) || (y == p.L.ny - 1 && is_open_kind(p.kind[3])) ||
+            (z == 0 && is_open_kind(p.kind[4])) || (z == p.L.nz - 1 && is_open_kind(p.kind[5]))) continue;
+        const T *r = A + lay_idx(p.L, 0, y, z);
+        const int x0 = open_x0 ? 1 : 0, x1 = open_x1 ? p.L.nx - 1 : p.L.nx;
+        for (int x = x0 + lane_; x < x1; x += 32) {
+            const double rho = 1.0 + (double)r[x];
+            const double ux = r[N + x], uy = r[2 * N + x], uz = r[3 * N + x];
+            acc[0] += rho; acc[1] += rho * ux; acc[2] += rho * uy; acc[3] += rho * uz;
+            acc[4] += 0.5 * rho * (ux * ux + uy * uy + uz * uz);
+        }
     }
     __shared__ double sh[5][TSLB_DIAG_THREADS / 32];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -429,7 +438,7 @@ FillParams make_fill(const tslb_ctx *c)
 cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st)
 {
     dim3 block(64, 2, 1);
-    dim3 grid((c->nx + block.x - 1) / block.x, (c->ny + block.y - 1) / block.y, c->nz);
+    dim3 grid((c->nx + block.x - 1) / block.x, (c->ny + block.y - 1) / block.y, c->nz < 65535 ? c->nz : 65535);
     if (c->dtype == TSLB_F32)
         sweep_gather_kernel<float><<<grid, block, 0, st>>>((const float *)c->buf[c->cur], (float *)c->buf[1 - c->cur],
                                                           make_params<float>(c));
@@ -471,19 +480,21 @@ cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st)
     return cudaGetLastError();
 }
 
-template <int DIR>
+template <int DIR, int SHIFT>
 static cudaError_t launch_convert(tslb_ctx *c, const void *src, void *dst, cudaStream_t st)
 {
     const size_t N = tslb_sites(c);
     size_t blocks = (TSLB_NF * N + 255) / 256;
     if (blocks > (size_t)c->sm_count * 16) blocks = (size_t)c->sm_count * 16;
-    if (c->dtype == TSLB_F32) convert_kernel<float, DIR><<<(unsigned)blocks, 256, 0, st>>>((const float *)src, (float *)dst, c->L);
-    else convert_kernel<double, DIR><<<(unsigned)blocks, 256, 0, st>>>((const double *)src, (double *)dst, c->L);
+    if (c->dtype == TSLB_F32) convert_kernel<float, DIR, SHIFT><<<(unsigned)blocks, 256, 0, st>>>((const float *)src, (float *)dst, c->L);
+    else convert_kernel<double, DIR, SHIFT><<<(unsigned)blocks, 256, 0, st>>>((const double *)src, (double *)dst, c->L);
     c->launches++;
     return cudaGetLastError();
 }
-cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<+1>(c, src, dst, st); }
-cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<-1>(c, src, dst, st); }
+cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<+1, 1>(c, src, dst, st); }
+cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<-1, 1>(c, src, dst, st); }
+cudaError_t tslb_launch_import_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<+1, 0>(c, src, dst, st); }
+cudaError_t tslb_launch_export_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st) { return launch_convert<-1, 0>(c, src, dst, st); }
 
 cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st)
 {

@@ -116,6 +116,7 @@ int tslb_create(int nx, int ny, int nz, double tau, int dtype, tslb_ctx **out)
     if (!out) return fail(nullptr, TSLB_EINVAL, "out == NULL");
     if (nx < 3 || ny < 3 || nz < 3) return fail(nullptr, TSLB_EINVAL, "every dimension must be >= 3");
     if ((double)nx * ny * nz > 2147483647.0) return fail(nullptr, TSLB_EINVAL, "lattice exceeds 2^31-1 nodes");
+    if (ny > 131070) return fail(nullptr, TSLB_EINVAL, "ny exceeds 131070 (grid limit of the gather kernel)");
     if (!isfinite(tau) || !(tau > 0.5)) return fail(nullptr, TSLB_EINVAL, "tau must be finite and > 0.5");
     if (dtype != TSLB_F32 && dtype != TSLB_F64) return fail(nullptr, TSLB_EINVAL, "unknown dtype");
     tslb_ctx *c = (tslb_ctx *)calloc(1, sizeof *c);
@@ -351,6 +352,32 @@ int tslb_get_moments_host(tslb_ctx *c, void *host_dst, void *stream)
     return TSLB_OK;
 }
 
+int tslb_export_state(tslb_ctx *c, void *dev_dst, long long *step_count, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (!dev_dst) return fail(c, TSLB_EINVAL, "dev_dst == NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = refresh_boundary(c, false, st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_export_raw(c, c->buf[c->cur], dev_dst, st);
+    if (e != cudaSuccess) return cuda_fail(c, "export kernel", e);
+    if (step_count) *step_count = c->t;
+    return TSLB_OK;
+}
+
+int tslb_import_state(tslb_ctx *c, const void *dev_src, long long step_count, void *stream)
+{
+    int rc = check_ready(c, false);
+    if (rc) return rc;
+    if (!dev_src) return fail(c, TSLB_EINVAL, "dev_src == NULL");
+    if (step_count < 0) return fail(c, TSLB_EINVAL, "step_count < 0");
+    cudaError_t e = tslb_launch_import_raw(c, dev_src, c->buf[0], (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
+    c->cur = 0; c->t = step_count; c->have_state = 1; c->halo_valid = 0;
+    return TSLB_OK;
+}
+
 int tslb_diagnostics(tslb_ctx *c, double *dev_out5, void *stream)
 {
     int rc = check_ready(c, true);
@@ -378,6 +405,6 @@ int tslb_plane_statistics(tslb_ctx *c, int axis, double *dev_sums, void *stream)
 long long tslb_step_count(const tslb_ctx *c) { return c && c->have_state ? c->t : -1; }
 long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
 const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err : g_create_err; }
-const char *tslb_version(void) { return "tslb-b200 0.2 (sm_100a)"; }
+const char *tslb_version(void) { return "tslb-b200 0.3 (sm_100a)"; }
 
 }  // extern "C"

@@ -100,6 +100,8 @@ cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st);          
 cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st);                    // ghost layers
 cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // API -> internal
 cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // internal -> API
+cudaError_t tslb_launch_import_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // the same without the rho <-> rho - 1 shift
+cudaError_t tslb_launch_export_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);
 cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st);
 cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st);
 

@@ -4,6 +4,7 @@ oracle on the same seeded workload and compare element by element.
 Tolerances (BASELINE.json north_star, reading A19):
   fp64: max |d rho|, max |d u|  <= 1e-12 (absolute)
   fp32: max |d rho| / max |rho_oracle|  and  max |d u| / max |u_oracle|  <= 2e-5
+  Pi_neq: <= 1e-12 absolute (fp64), <= 1e-3 of max |Pi_oracle| (fp32)
 over the nodes that are not on an open face (those are imposed, not computed).
 """
 import numpy as np
@@ -11,6 +12,9 @@ import numpy as np
 from paper_2401_17074_b200 import workloads as W
 
 TOL = {"f64": 1e-12, "f32": 2e-5}
+# Pi_neq (six of the ten stored fields; north_star names rho and u only): rebuilt from scratch every step, so its error does
+# not accumulate -- absolute for f64, relative to max|Pi_oracle| for f32
+TOL_PI = {"f64": 1e-12, "f32": 1e-3}
 
 
 def make_oracle(oracle_mod, w):
@@ -72,6 +76,8 @@ def assert_parity(w, G, R, what="", tol=None):
     e_rho, e_u, e_pi = errors(w, G, R)
     t = TOL[w.dtype] if tol is None else tol
     assert e_rho <= t and e_u <= t, "%s %s: err rho %.3e, u %.3e (Pi %.3e) > %.1e" % (w.name, what, e_rho, e_u, e_pi, t)
+    if tol is None:
+        assert e_pi <= TOL_PI[w.dtype], "%s %s: err Pi %.3e > %.1e" % (w.name, what, e_pi, TOL_PI[w.dtype])
     # boundary nodes are imposed values: they must agree to storage rounding
     m = ~interior_mask(w)
     if m.any():
