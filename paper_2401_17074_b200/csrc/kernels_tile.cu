@@ -29,6 +29,7 @@
 // passes.  A pass with taps (t-, t0, t+) applied to B*u gives (t- + t0 + t+) B u(x) + B [t- (u(x-1) - u(x)) + t+ (u(x+1) - u(x))];
 // only the bracket (exact differences of stored velocities) is added at each stage, and the product of the tap sums,
 // 216 u_a(x), is re-attached in closed form at the end:  u' = u + (J_small - u dR) / (216 + dR).
+#include <type_traits>
 #include "tslb_internal.h"
 
 namespace {
@@ -98,6 +99,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "DONE_%=:\n"
         "}" ::"r"(bar), "r"(parity) : "memory");
 }
+// 1: the generic -> async proxy fence before the TMA store of the output tile is executed once by the store thread,
+// after it has acquired the main warps' writes through the "tile full" mbarrier (release at their arrive), instead of
+// by every main warp after its own writes (fence.proxy.async = MEMBAR.ALL.CTA + FENCE.VIEW.ASYNC: ~400 cycles per warp
+// and plane with 20 shared-memory stores in flight)
+#ifndef TILE_FENCE_STORER
+#define TILE_FENCE_STORER 1
+#endif
 // one warp signals: every lane's earlier shared-memory accesses are ordered before the arrive of lane 0
 __device__ __forceinline__ void warp_arrive(uint32_t bar, int lane)
 {
@@ -199,20 +207,26 @@ __device__ __forceinline__ void hermite_round(const P (&raw)[TSLB_NF], T beta, c
 }
 
 // The y-pass combinations of one pack (rows .x, .y) for the coefficient group (kx, kz), from A[kx][ky]:
-//   t = A0 + A2,   qc = t + A1*sgn = (P of row .x, M of row .y)   -- what the pack's own rows exchange with each other
-//                  qp = t - A1*sgn = (M of row .x, P of row .y)   -- what the rows outside the pack need: PUBLISHED
+//   t = A0 + A2,   (p0, m1) = (P of row .x, M of row .y)          -- what the pack's own rows exchange with each other
+//                  (m0, p1) = (M of row .x, P of row .y)          -- what the rows outside the pack need: PUBLISHED
 //   cen = 4 A0 - 2 A2                                              -- the centre taps
-// with P = phi0 + phi1 + phi2 (goes up, c_y = +1), M = phi0 - phi1 + phi2 (goes down), sgn = (1, -1).
+// with P = phi0 + phi1 + phi2 (goes up, c_y = +1), M = phi0 - phi1 + phi2 (goes down).
+// The four combinations are formed with SCALAR adds (p0, m0 of row .x; p1, m1 of row .y): a packed instruction cannot add
+// in one half and subtract in the other, so the packed form needs multiplications by (1,-1) packs (three-register
+// FFMA2s, the most expensive instruction of the loop in register-file bandwidth), and a scalar FADD costs exactly half
+// a packed one.
 template <int ORDER, int KX, int KZ, typename P, typename T>
-__device__ __forceinline__ void ycombos(const P (&A)[3][3], P &qc, P &qp, P &cen)
+__device__ __forceinline__ void ycombos(const P (&A)[3][3], T &p0, T &m0, T &p1, T &m1, P &cen)
 {
-    const P sgn = pk((T)1, (T)-1), nsg = pk((T)-1, (T)1);
     const P a0 = A[KX][0];
     P t = a0;
     cen = pmuls(a0, (T)4);
     if (kvalid<ORDER>(KX, 2, KZ)) { t = padd(a0, A[KX][2]); cen = pfmas(A[KX][2], (T)-2, cen); }
-    qc = t; qp = t;
-    if (kvalid<ORDER>(KX, 1, KZ)) { qc = pfma(A[KX][1], sgn, t); qp = pfma(A[KX][1], nsg, t); }
+    p0 = t.x; m0 = t.x; p1 = t.y; m1 = t.y;
+    if (kvalid<ORDER>(KX, 1, KZ)) {
+        const P a1 = A[KX][1];
+        p0 = t.x + a1.x; m0 = t.x - a1.x; p1 = t.y + a1.y; m1 = t.y - a1.y;
+    }
 }
 
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
@@ -227,13 +241,18 @@ __host__ __device__ constexpr int qidx(int kx, int kz) { return kz * 3 + kx; }
 // the source box starts XPAD = 4 columns left of the tile (the layout puts node x = 0 on a 16-byte boundary).
 template <typename T> struct TileGeom;
 #ifndef TILE_F32_WY
-#define TILE_F32_WY 7
+#define TILE_F32_WY 6
 #endif
 #ifndef TILE_F32_NS
 #define TILE_F32_NS 2
 #endif
 #ifndef TILE_ZC_MAX
 #define TILE_ZC_MAX 64
+#endif
+// output tiles in shared memory: with two the main warps fill one while the TMA store drains the other (the store of a
+// 60 x 14 x 10 tile takes ~1200 cycles from issue to "source read"; with a single tile that is a CTA-wide bubble per plane)
+#ifndef TILE_F32_NOUT
+#define TILE_F32_NOUT 2
 #endif
 // REG_MAIN / REG_HALO != 0: the register file is re-divided after launch with setmaxnreg (the main warps, which carry the
 // z-march state, get more than an even share; needs the main warps to be whole warpgroups of 4, and NIDLE idle warps that
@@ -242,15 +261,18 @@ template <typename T> struct TileGeom;
 // 16: a warp's allocation is rounded up to 512 registers, and a setmaxnreg.inc that cannot be satisfied blocks forever
 // (measured: 216 + 216 + 80 and 208 + 208 + 96 per sub-partition hang).  The pool is what the CTA was given at LAUNCH
 // (threads x MAXREG), not the whole register file: the re-divided total must not exceed it.
+// fp32: 12 main warps at 144 registers + 2 halo + 2 idle at 80 (14 main warps at the even share of 128 spill ~40 values per
+// plane: 48.8 GLUPS at 512^3 against 54.5 with 12 warps and no spills)
 #ifndef TILE_F32_RM
-#define TILE_F32_RM 0
-#define TILE_F32_RH 0
-#define TILE_F32_NIDLE 0
+#define TILE_F32_RM 144
+#define TILE_F32_RH 80
+#define TILE_F32_NIDLE 2
 #endif
 template <> struct TileGeom<float> {
     static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, NIDLE = TILE_F32_NIDLE, REG_MAIN = TILE_F32_RM, REG_HALO = TILE_F32_RH;
+    static constexpr int NOUT = TILE_F32_NOUT;
 };
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = 208, REG_HALO = 80; };
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = 208, REG_HALO = 80, NOUT = 1; };
 constexpr int rup128(int bytes) { return (bytes + 127) / 128 * 128; }
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;
@@ -276,10 +298,13 @@ template <typename T> struct TileDims {
     static constexpr int EXW = 64;                               // exchange columns: tile columns -1 .. 62
     static constexpr int EX_SLOT = NPACK * NGRP * EXW;           // elements per component and slot
     static constexpr int OUT_ELEMS = TSLB_NF * ROWS * COLS;      // output tile [10][ROWS][COLS]
+    static constexpr int NOUT = G::NOUT;                         // output tiles (1 or 2)
+    static constexpr int OUT_BYTES = rup128(OUT_ELEMS * (int)sizeof(T));
     static constexpr int OFF_OUT = NS * STAGE_ELEMS * (int)sizeof(T);
-    static constexpr int OFF_EX = OFF_OUT + rup128(OUT_ELEMS * (int)sizeof(T));
+    static constexpr int OFF_EX = OFF_OUT + NOUT * OUT_BYTES;
     static constexpr int OFF_BAR = OFF_EX + 4 * EX_SLOT * (int)sizeof(T);     // 2 components x 2 slots
-    static constexpr int NBAR = 2 * NS + 2 * NPACK + 2;
+    static constexpr int NBAR = 2 * NS + 2 * (NPACK + 1) + 2 * NOUT;
+    static_assert(NOUT == 1 || NOUT == 2, "one or two output tiles");
     static constexpr int SMEM_BYTES = OFF_BAR + NBAR * 8;
 };
 static_assert(TileDims<float>::SMEM_BYTES <= 232448 && TileDims<double>::SMEM_BYTES <= 232448, "shared memory budget");
@@ -296,9 +321,17 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
     constexpr int ES = (int)sizeof(T);
     constexpr int STAGE_BYTES = TD::STAGE_ELEMS * ES, SLOT_BYTES = TD::EX_SLOT * ES;
-    constexpr int OFF_EXY = TD::OFF_EX + 2 * SLOT_BYTES;           // exX: [2][NPACK][NGRP][EXW] M of a pack's row .x; exY: P of its row .y
-    // barriers (8 bytes each): full[NS], empty[NS], q[NPACK][2], ofull, oempty
-    constexpr int B_FULL = TD::OFF_BAR, B_EMPTY = B_FULL + 8 * NS, B_Q = B_EMPTY + 8 * NS, B_OFULL = B_Q + 16 * NPACK, B_OEMPTY = B_OFULL + 8;
+    // Exchange area: exX [2 slots][NPACK][NGRP][EXW] = M of a pack's row .x, main pair wy at index wy, the halo pair at WY;
+    //                exY (2 slots further) = P of a pack's row .y, main pair wy at index wy + 1, the halo pair at 0.
+    // So the pair below pair wy (its "down" source) is exY[wy] and the pair above (its "up" source) exX[wy + 1] for every
+    // wy, the halo pair included: all three addresses of a main warp are one register plus immediates.
+    constexpr int PACK_BYTES = NGRP * EXW * ES;
+    constexpr int OFF_EXY = TD::OFF_EX + 2 * SLOT_BYTES;
+    constexpr int NOUT = TD::NOUT, OUT_BYTES = TD::OUT_BYTES;
+    // barriers (8 bytes each): full[NS], empty[NS], q[NPACK + 1][2], ofull[NOUT], oempty[NOUT].  "Published" barriers q: the
+    // halo pair has two (index 0 and WY + 1, it arrives on both), main pair wy has index wy + 1: a pair waits for its
+    // neighbours at index - 1 and index + 1.
+    constexpr int B_FULL = TD::OFF_BAR, B_EMPTY = B_FULL + 8 * NS, B_Q = B_EMPTY + 8 * NS, B_OFULL = B_Q + 16 * (NPACK + 1), B_OEMPTY = B_OFULL + 8 * NOUT;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const uint32_t sb = keep(smem_u32(smem_raw));
 
@@ -318,9 +351,9 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(sb + B_FULL + 8 * s, 1); mbar_init(sb + B_EMPTY + 8 * s, TD::WARPS); }
 #pragma unroll
-        for (int s = 0; s < 2 * NPACK; ++s) mbar_init(sb + B_Q + 8 * s, WX);
-        mbar_init(sb + B_OFULL, TD::NMAIN);
-        mbar_init(sb + B_OEMPTY, 1);
+        for (int s = 0; s < 2 * (NPACK + 1); ++s) mbar_init(sb + B_Q + 8 * s, WX);
+#pragma unroll
+        for (int s = 0; s < NOUT; ++s) { mbar_init(sb + B_OFULL + 8 * s, TD::NMAIN); mbar_init(sb + B_OEMPTY + 8 * s, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_async_smem();
     }
@@ -338,7 +371,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         const int bcol = ecol - 1 + XPAD;                  // box column
         // pack .x = tile row ROWS (above the tile), .y = tile row -1 (below): it publishes (M of .x, P of .y) like any pack
         const uint32_t aA = keep(sb + (TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol) * ES), aB = keep(sb + (TD::MAIN_ELEMS + bcol) * ES);
-        const uint32_t aW = keep(sb + TD::OFF_EX + ((NPACK - 1) * NGRP * EXW + ecol) * ES);
+        const uint32_t aW = keep(sb + TD::OFF_EX + (WY * NGRP * EXW + ecol) * ES);      // exX[WY]; exY[0] is HALO_Y further
+        constexpr int HALO_Y = 2 * SLOT_BYTES - WY * PACK_BYTES;
         // source rows of the two halo rows: wrapped on a periodic axis, out of bounds (zero fill) beyond a wall / open face
         const bool yper = p.kind[2] == TSLB_BC_PERIODIC;
         const int ylo = row0 > 0 ? row0 - 1 : (yper ? L.ny - 1 : -1);
@@ -361,12 +395,22 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         // rows beyond a bounce-back wall send nothing (their raw moments are zero-filled, but A100 = 3 g is not zero)
         const P hm = pk((WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && row0 + ROWS >= L.ny) ? (T)0 : (T)1,
                         (WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && row0 == 0) ? (T)0 : (T)1);
-        auto store_tile = [&](int m) {                     // output plane m of this chunk: z = z0 + m
-            mbar_wait(sb + B_OFULL, (uint32_t)(m & 1));
-            tma_store_4d(sb + TD::OFF_OUT, &tmStore, x0 + TSLB_XOFF, row0, z0 + m, 0);
+        // output plane m of this chunk (z = z0 + m) sits in output tile m % NOUT; its k-th use completes phase k of the
+        // tile's ofull / oempty barriers.  With two tiles the store of plane m is left in flight and the tile of plane m-1 is
+        // handed back once ITS store has read the shared memory (at most one bulk group pending).
+        auto store_tile = [&](int m) {
+            const int b = m % NOUT;
+            mbar_wait(sb + B_OFULL + 8 * b, (uint32_t)((m / NOUT) & 1));
+            if (TILE_FENCE_STORER) fence_async_smem();
+            tma_store_4d(sb + TD::OFF_OUT + b * OUT_BYTES, &tmStore, x0 + TSLB_XOFF, row0, z0 + m, 0);
             tma_store_commit();
-            tma_store_wait_read();
-            mbar_arrive(sb + B_OEMPTY);
+            if (NOUT == 1) {
+                tma_store_wait_read();
+                mbar_arrive(sb + B_OEMPTY);
+            } else if (m >= 1) {
+                asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                mbar_arrive(sb + B_OEMPTY + 8 * ((m - 1) % NOUT));
+            }
         };
         int stg = 0;
         uint32_t fpar = 0;
@@ -390,16 +434,17 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             // finished reading plane i-2 once they have published plane i-1.  (The main warps get the same guarantee from
             // waiting for the pairs they read from; the halo warps read nothing, so they wait explicitly.)
             if (i >= 2) {
-                mbar_wait(sb + B_Q + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
-                mbar_wait(sb + B_Q + 16 * (WY - 1) + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
+                mbar_wait(sb + B_Q + 16 * 1 + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
+                mbar_wait(sb + B_Q + 16 * WY + 8 * ((i - 1) & 1), (uint32_t)(((i - 1) >> 1) & 1));
             }
 #define TSLB_HALO_GROUP(KX, KZ)                                                                   \
             if (kvalid<ORDER>(KX, 0, KZ)) {                                                       \
-                P qc, qp, cen;                                                                    \
-                ycombos<ORDER, KX, KZ, P, T>(A, qc, qp, cen);                                     \
-                if (WALLY) qp = pmul(qp, hm);                                                     \
-                sts(w + qidx(KX, KZ) * EXW * ES, qp.x);                                           \
-                sts(w + 2 * SLOT_BYTES + qidx(KX, KZ) * EXW * ES, qp.y);                          \
+                T p0, m0, p1, m1;                                                                 \
+                P cen;                                                                            \
+                ycombos<ORDER, KX, KZ, P, T>(A, p0, m0, p1, m1, cen);                             \
+                if (WALLY) { m0 *= hm.x; p1 *= hm.y; }                                            \
+                sts(w + qidx(KX, KZ) * EXW * ES, m0);                                             \
+                sts(w + HALO_Y + qidx(KX, KZ) * EXW * ES, p1);                                    \
             }
 #define TSLB_HALO_ROUND(KZ)                                                                       \
             {                                                                                     \
@@ -412,7 +457,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             TSLB_HALO_ROUND(2)
 #undef TSLB_HALO_ROUND
 #undef TSLB_HALO_GROUP
-            warp_arrive(sb + B_Q + 16 * (NPACK - 1) + 8 * (i & 1), lane);
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(sb + B_Q + 8 * (i & 1)); mbar_arrive(sb + B_Q + 16 * (WY + 1) + 8 * (i & 1)); }
             // the output tile the main warps finished in their iteration i-1 (output plane i-3)
             if (storer && i >= 3) store_tile(i - 3);
             if (++stg == NS) { stg = 0; fpar ^= 1; }
@@ -441,31 +487,39 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     const int bcol = tc + XPAD;
     const uint32_t aC = keep(sb + ((2 * wy) * BXW + bcol) * ES);                 // row r0 in the main region (r0+1: + BXW)
     // u of rows r0-1 / r0+2: in the main region (field stride FS) or, at the tile edge, in a halo-row slot (field stride BXW)
-    const int fsLo = wy == 0 ? BXW : FS, fsHi = wy == WY - 1 ? BXW : FS;
-    const uint32_t aLo = keep(sb + ((wy == 0 ? TD::MAIN_ELEMS + bcol : (2 * wy - 1) * BXW + bcol) + fsLo) * ES);
-    const uint32_t aHi = keep(sb + ((wy == WY - 1 ? TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol : (2 * wy + 2) * BXW + bcol) + fsHi) * ES);
-    const uint32_t stLo = keep((uint32_t)(fsLo * ES)), stHi = keep((uint32_t)(fsHi * ES));
+    // (two code versions of the three loads, chosen by warp-uniform predicates, instead of run-time strides)
+    const bool loEdge = wy == 0, hiEdge = wy == WY - 1;
+    const uint32_t aLo = keep(sb + ((loEdge ? TD::MAIN_ELEMS + bcol + BXW : (2 * wy - 1) * BXW + bcol + FS)) * ES);   // field 1 (ux)
+    const uint32_t aHi = keep(sb + ((hiEdge ? TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol + BXW : (2 * wy + 2) * BXW + bcol + FS)) * ES);
     // exchange: own pack wy publishes at column tc+1 (columns 30, 31 belong to the wx = 0 warp: lanes 0, 1 of the wx = 1 warp
     // write into the unused columns 62, 63 instead); the halo pair is pack NPACK-1: below wy = 0 and above wy = WY-1
+    // Columns 30, 31 belong to both warps of a pair (lanes 30, 31 of wx = 0 and lanes 0, 1 of wx = 1 hold the same two nodes
+    // and publish bit-identical values of the same plane -- their readers wait for both warps).  Only the wall code re-reads
+    // a warp's OWN columns later in the iteration, when the twin warp may already have overwritten them with a later plane:
+    // there lanes 0, 1 of the wx = 1 warp publish into the unused columns 62, 63 and the read base is a second register.
     const int ecol = tc + 1;
-    const int ecol_w = (wx == 0 || lane >= 2) ? ecol : 62 + lane;
-    const uint32_t aW = keep(sb + TD::OFF_EX + (wy * NGRP * EXW + ecol_w) * ES);
-    const uint32_t aDn = keep(sb + OFF_EXY + (((wy + NPACK - 1) % NPACK) * NGRP * EXW + ecol) * ES);   // P of the row below
-    const uint32_t aUp = keep(sb + TD::OFF_EX + ((wy + 1) * NGRP * EXW + ecol) * ES);                  // M of the row above
+    const int ecol_w = (!WALLY || wx == 0 || lane >= 2) ? ecol : 62 + lane;
+    const uint32_t aW = keep(sb + TD::OFF_EX + (wy * NGRP * EXW + ecol_w) * ES);     // own: exX[wy]; exY[wy + 1] is OWN_Y further
+    const uint32_t aR = WALLY ? keep(sb + TD::OFF_EX + (wy * NGRP * EXW + ecol) * ES) : aW;
+    constexpr int OWN_Y = 2 * SLOT_BYTES + PACK_BYTES;
+    constexpr int DN_OFF = 2 * SLOT_BYTES;                                           // exY[wy]: P of the row below
+    constexpr int UP_OFF = PACK_BYTES;                                               // exX[wy + 1]: M of the row above
     const uint32_t aO = keep(sb + TD::OFF_OUT + ((2 * wy) * COLS + (tc < 0 ? 0 : tc)) * ES);           // output tile [f][row][tc]
-    const uint32_t bQown = sb + B_Q + 16 * wy, bQdn = sb + B_Q + 16 * ((wy + NPACK - 1) % NPACK), bQup = sb + B_Q + 16 * (wy + 1);
+    const uint32_t bQown = keep(sb + B_Q + 16 * (wy + 1));                           // neighbours: - 16, + 16
 
-    // z-march state per (px,py) group g: tt1 = Vp(zs-2) + centre(zs-1), vp1 = Vp(zs-1), and vp2 = Vp(zs-2) where it is needed
-    // alone (groups 0, 1, 3): 15 running pairs
-    P vp2[6], tt1[6], vp1[6];
-    // increment form along z: velocity of the previous plane and its backward difference, rows r0, r0+1
-    P uprev[3], dprev[3];
+    // z-march state per (px,py) group g, DOUBLE-BUFFERED over the parity of the source plane (the plane loop is unrolled by two
+    // with the parity as a compile-time constant, so the march shifts no registers and every stage / slot / barrier offset
+    // is an immediate):  vpb[par][g] = Vp of the source plane of parity par (Vp(zs-1) is in vpb[1-par], and vpb[par] still
+    // holds Vp(zs-2) until this plane's Vp overwrites it);  ttb[par][g] = Vp(zs-2) + centre(zs-1), which this plane completes
+    // (ttb[1-par] receives Vp(zs-1) + centre(zs) for the next one).
+    P vpb[2][6], ttb[2][6];
+    // increment form along z: velocity of the source planes and the backward difference, rows r0, r0+1
+    P ub[2][3], db[2][3];
 #pragma unroll
-    for (int i = 0; i < 6; ++i) { vp2[i] = pbc<P, T>((T)0); tt1[i] = vp2[i]; vp1[i] = vp2[i]; }
+    for (int i = 0; i < 6; ++i) { vpb[0][i] = pbc<P, T>((T)0); vpb[1][i] = vpb[0][i]; ttb[0][i] = vpb[0][i]; ttb[1][i] = vpb[0][i]; }
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { uprev[a] = pbc<P, T>((T)0); dprev[a] = uprev[a]; }
+    for (int a = 0; a < 3; ++a) { ub[0][a] = pbc<P, T>((T)0); ub[1][a] = ub[0][a]; db[0][a] = ub[0][a]; db[1][a] = ub[0][a]; }
 
-    const P sgn = pk((T)1, (T)-1), nsg = pk((T)-1, (T)1);
     const bool xper = p.kind[0] == TSLB_BC_PERIODIC;
     // periodic x: the node at x = 0 is also the ghost column x = nx, the node at x = nx-1 the ghost column x = -1
     const bool xedge = xper && lane_out && (col == 0 || col == L.nx - 1);
@@ -474,12 +528,22 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     // partly covered unit would be written whole, over the ghost column), the columns beyond it are stored from registers
     const bool xtail = lane_out && col >= (L.nx & ~(16 / ES - 1)) && col < L.nx;
 
-    int stg = 0;
-    uint32_t fpar = 0;
-    for (int i = 0; i < nplanes; ++i) {
-        const uint32_t so = stg * STAGE_BYTES;
-        const uint32_t xo = (i & 1) * SLOT_BYTES;
-        mbar_wait(sb + B_FULL + 8 * stg, fpar);
+    static_assert(NS == 2, "the plane loop is unrolled by two: stage = parity of the source plane");
+    // All barriers of the loop complete one phase every two planes (two stages, two exchange slots, two output tiles), so
+    // a single phase bit serves them all: ph = (i >> 1) & 1.
+    uint32_t ph = 0;
+    auto plane = [&](auto par_c, const int i) {
+        constexpr int PAR = decltype(par_c)::value;
+        constexpr uint32_t so = PAR * STAGE_BYTES, xo = PAR * SLOT_BYTES;
+        P (&vp1)[6] = vpb[1 - PAR];          // Vp(zs-1)
+        P (&vp0)[6] = vpb[PAR];              // Vp(zs-2) on entry (groups 0, 1, 3 read it first), Vp(zs) on exit
+        P (&tt1)[6] = ttb[PAR];
+        P (&tn)[6] = ttb[1 - PAR];
+        P (&uprev)[3] = ub[1 - PAR];
+        P (&ucur)[3] = ub[PAR];
+        P (&dprev)[3] = db[1 - PAR];
+        P (&dcur)[3] = db[PAR];
+        mbar_wait(sb + B_FULL + 8 * PAR, ph);
 
         // ---- a1: moments of the own rows r0, r0+1 and the velocities of the rows r0-1, r0+2 at this column ------------------
         P rc[TSLB_NF], hu[3];
@@ -487,28 +551,40 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             const uint32_t a = aC + so;
 #pragma unroll
             for (int f = 0; f < TSLB_NF; ++f) rc[f] = pk(lds(a + f * FS * ES, T()), lds(a + (f * FS + BXW) * ES, T()));
-            uint32_t al = aLo + so, ah = aHi + so;
+            T hl[3], hh[3];
+            if (loEdge) {
 #pragma unroll
-            for (int k = 0; k < 3; ++k) { hu[k] = pk(lds(al, T()), lds(ah, T())); al += stLo; ah += stHi; }
+                for (int k = 0; k < 3; ++k) hl[k] = lds(aLo + so + k * BXW * ES, T());
+            } else {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) hl[k] = lds(aLo + so + k * FS * ES, T());
+            }
+            if (hiEdge) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) hh[k] = lds(aHi + so + k * BXW * ES, T());
+            } else {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) hh[k] = lds(aHi + so + k * FS * ES, T());
+            }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) hu[k] = pk(hl[k], hh[k]);
         }
-        warp_arrive(sb + B_EMPTY + 8 * stg, lane);       // the stage can be refilled: everything needed is in registers
+        warp_arrive(sb + B_EMPTY + 8 * PAR, lane);       // the stage can be refilled: everything needed is in registers
 
         // ---- a2: Hermite coefficients of the own rows, all three rounds; y-pass combinations of the 8 groups -------------
-        // qs = swap(qc) = (M of row r0+1, P of row r0): what the two rows of the pack receive from each other.
-        // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)), so with qh = (P(r0-1), M(r0+2)) read from the
-        // neighbours:  E = up + dn = qh + qs,  O = up - dn = (qh - qs) * sgn = qh*sgn + qo,  qo = -qs*sgn;  G0 = E + cen.
-        P qe[NGRP], qo[NGRP], cen[NGRP];
+        // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)); P(r0-1) and M(r0+2) are read from the neighbours,
+        // P(r0) = qP0 and M(r0+1) = qM1 are the pack's own:  E = up + dn,  O = up - dn,  G0 = E + cen.
+        T qP0[NGRP], qM1[NGRP];
+        P cen[NGRP];
         {
             const uint32_t w = aW + xo;
 #define TSLB_MAIN_GROUP(KX, KZ)                                                                   \
             if (kvalid<ORDER>(KX, 0, KZ)) {                                                       \
                 constexpr int q = qidx(KX, KZ);                                                   \
-                P qc, qp;                                                                         \
-                ycombos<ORDER, KX, KZ, P, T>(A, qc, qp, cen[q]);                                  \
-                const P qs = pswap(qc);                                                           \
-                qe[q] = qs; qo[q] = pmul(qs, nsg);                                                \
-                sts(w + q * EXW * ES, qp.x);                                                      \
-                sts(w + 2 * SLOT_BYTES + q * EXW * ES, qp.y);                                     \
+                T m0, p1;                                                                         \
+                ycombos<ORDER, KX, KZ, P, T>(A, qP0[q], m0, p1, qM1[q], cen[q]);                  \
+                sts(w + q * EXW * ES, m0);                                                        \
+                sts(w + OWN_Y + q * EXW * ES, p1);                                                \
             }
 #define TSLB_MAIN_ROUND(KZ)                                                                       \
             {                                                                                     \
@@ -522,7 +598,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #undef TSLB_MAIN_ROUND
 #undef TSLB_MAIN_GROUP
         }
-        warp_arrive(bQown + 8 * (i & 1), lane);
+        warp_arrive(bQown + 8 * PAR, lane);
 
         // ---- increment form along y: exact differences of the stored velocities,
         //      Ly = (up - c) + (dn - c), Wy = (up - dn) * sgn with up / dn the neighbour rows (hu = (u(r0-1), u(r0+2)), the
@@ -531,30 +607,51 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         //      (kx,kz) = (1,0): 3 Ly_x, sg3 Wy_x;   (0,0): sg3 Wy_y, 3 Ly_y;   (0,1): 3 Ly_z, sg3 Wy_z. -------------------------
         const P sg3 = pk((T)3, (T)-3);
         // (after the publish: the neighbours do not wait for this)
+        P incE[3], incO[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             const P uc = rc[1 + a];
             const P cs = pswap(uc);
             const P ly3 = pmuls(pfmas(uc, (T)-2, padd(hu[a], cs)), (T)3);
             const P wy3 = pmul(psub(hu[a], cs), sg3);
-            const int q = a == 0 ? qidx(1, 0) : (a == 1 ? qidx(0, 0) : qidx(0, 1));
-            qe[q] = padd(qe[q], a == 1 ? wy3 : ly3);
-            qo[q] = padd(qo[q], a == 1 ? ly3 : wy3);
+            incE[a] = a == 1 ? wy3 : ly3;
+            incO[a] = a == 1 ? ly3 : wy3;
         }
 
+        // increment form along z: exact differences of the stored velocities at the target plane zs-1
+        P Lz[3], Dz[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            ucur[a] = rc[1 + a];
+            const P dc = psub(rc[1 + a], uprev[a]);      // u(zs) - u(zs-1)
+            Lz[a] = psub(dc, dprev[a]);
+            Dz[a] = padd(dprev[a], dc);                  // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
+            dcur[a] = dc;
+        }
+        // the z-pass terms that need Vp(zs-2) alone (groups 0, 1, 3), taken before this plane's Vp overwrites it; the z-stage
+        // increments (base multipliers 36 for ux, uy; 108 / 36 for uz) go into the sums now, so that no difference stays live
+        const P e3 = pfmas(Lz[2], (T)108, vp0[0]);       // 001
+        const P e6 = pfmas(Dz[2], (T)-108, vp0[0]);      // 002
+        const P e8 = pfmas(Dz[0], (T)-36, vp0[1]);       // 101
+        const P e9 = pfmas(Dz[1], (T)-36, vp0[3]);       // 011
+        tt1[0] = pfmas(Dz[2], (T)-108, tt1[0]);          // 000
+        tt1[1] = pfmas(Lz[0], (T)36, tt1[1]);            // 100
+        tt1[3] = pfmas(Lz[1], (T)36, tt1[3]);            // 010
+        tt1[2] = pfmas(Dz[2], (T)-36, tt1[2]);           // 200
+        tt1[5] = pfmas(Dz[2], (T)-36, tt1[5]);           // 020
 
         // ---- the neighbours' combinations -----------------------------------------------------------------------------------
-        mbar_wait(bQdn + 8 * (i & 1), (uint32_t)((i >> 1) & 1));
-        mbar_wait(bQup + 8 * (i & 1), (uint32_t)((i >> 1) & 1));
-        const uint32_t rdn = aDn + xo, rup = aUp + xo;
+        mbar_wait(bQown - 16 + 8 * PAR, ph);
+        mbar_wait(bQown + 16 + 8 * PAR, ph);
+        const uint32_t rdn = aR + DN_OFF + xo, rup = aR + UP_OFF + xo;
 
         // this plane's contributions to the z march, accumulated over kz where they are needed:
         //   tt1[g] += Vm(zs)            (pz = 0 of the target plane zs-1; groups 2, 4, 5, where Vm is not needed alone)
         //   vm0[g]  = Vm(zs)            (groups 0, 1, 3)
-        //   tn[g]   = vp1[g] + centre(zs)   (next iteration's tt1)
+        //   tn[g]   = vp1[g] + centre(zs)   (the next plane's tt1)
         //   vp0[g]  = Vp(zs)
         // with Vp = phi0 + phi1 + phi2, Vm = phi0 - phi1 + phi2, centre = 4 phi0 - 2 phi2 over kz.
-        P vp0[6], vm0[6], tn[6];
+        P vm0[6];
 #pragma unroll
         for (int kz = 0; kz < 3; ++kz) {
             // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 ---------------------------------------
@@ -563,10 +660,15 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             for (int kx = 0; kx < 3; ++kx) {
                 if (!kvalid<ORDER>(kx, 0, kz)) continue;
                 const int q = qidx(kx, kz);
-                const P qh = pk(lds(rdn + q * EXW * ES, T()), lds(rup + q * EXW * ES, T()));
-                const P E = padd(qh, qe[q]);
+                // (scalar adds: their operands are scalars from four different places, a packed add would need them moved
+                //  into register pairs first)
+                const T pdn = lds(rdn + q * EXW * ES, T()), mup = lds(rup + q * EXW * ES, T());
+                P E = pk(pdn + qM1[q], qP0[q] + mup), O = pk(pdn - qM1[q], qP0[q] - mup);
+                // (kx,kz) = (1,0): ux, (0,0): uy, (0,1): uz carry the y-stage increments
+                const int ia = q == qidx(1, 0) ? 0 : (q == qidx(0, 0) ? 1 : (q == qidx(0, 1) ? 2 : -1));
+                if (ia >= 0) { E = padd(E, incE[ia]); O = padd(O, incO[ia]); }
                 G1[2][kx] = E;
-                G1[1][kx] = pfma(qh, sgn, qo[q]);
+                G1[1][kx] = O;
                 G1[0][kx] = padd(E, cen[q]);
             }
             // x differences of the stored velocities (increment form along x), from the neighbour lanes
@@ -621,7 +723,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 
         // ---- halfway bounce-back on a y face: for a wall-adjacent row the 9
         //      populations arriving from beyond the wall are f*_ibar of the node itself, a local combination of its own
-        //      coefficients  B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz)  -- exactly the published combination qp of that row
+        //      coefficients  B(kx,kz) = sum_ky t_ky(-c_y) A(kx,ky,kz)  -- exactly the published combination of that row
         //      (M of a row at the wall below, P of a row at the wall above) -- with the local sums L(0,0)=6, L(1,1)=-2,
         //      L(2,0)=L(2,2)=2. ---------------------------------------------------------------------------------------------
         // The six bounced populations with c_z = 0 go into this plane's centre terms (they reach the target plane through
@@ -638,8 +740,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             const P sgp = pk(ghost_lo ? (T)1 : (T)-1, (T)-1);                              // c_y of the arrival direction
             const P w12 = pmuls(wm, (T)12), w36 = pmuls(wm, (T)36), w12s = pmul(w12, sgp), w36s = pmul(w36, sgp);
             // (re-read from this warp's own exchange slots instead of being kept in registers across the passes; lanes 0, 1 of
-            //  the wx = 1 warp published elsewhere, but they are halo / duplicate lanes whose output is not stored)
-            auto own = [&](uint32_t w, int q) { return pk(lds(w + q * EXW * ES, T()), lds(w + 2 * SLOT_BYTES + q * EXW * ES, T())); };
+            //  the wx = 1 warp published in the private columns 62, 63)
+            auto own = [&](uint32_t w, int q) { return pk(lds(w + q * EXW * ES, T()), lds(w + OWN_Y + q * EXW * ES, T())); };
             {   // source plane zs: full first-order coefficients (the passes carry them without their base 3 u)
                 const uint32_t w = aW + xo;
                 const P WB10 = pfmas(rc[1], (T)3, own(w, qidx(1, 0)));
@@ -664,31 +766,21 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             }
         }
 
-        // increment form along z: exact differences of the stored velocities at the target plane zs-1
-        P Lz[3], Dz[3];
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const P dcur = psub(rc[1 + a], uprev[a]);    // u(zs) - u(zs-1)
-            Lz[a] = psub(dcur, dprev[a]);
-            Dz[a] = padd(dprev[a], dcur);                // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
-            dprev[a] = dcur;
-        }
-
         // ---- z pass for target plane zt = zs - 1:  pz=0: Vp(zs-2) + centre(zs-1) + Vm(zs);  pz=1: Vp(zs-2) - Vm(zs);
         //      pz=2: Vp(zs-2) + Vm(zs); plus the z-stage increments (base multipliers 36 for ux, uy; 108 / 36 for uz) ----
         if (i >= 2) {
             const int zt = z0 + i - 2;
             P m[TSLB_NF];
-            m[0] = pfmas(Dz[2], (T)-108, padd(tt1[0], vm0[0]));          // 000
-            m[3] = pfmas(Lz[2], (T)108, psub(vp2[0], vm0[0]));           // 001
-            m[6] = pfmas(Dz[2], (T)-108, padd(vp2[0], vm0[0]));          // 002
-            m[1] = pfmas(Lz[0], (T)36, padd(tt1[1], vm0[1]));            // 100
-            m[8] = pfmas(Dz[0], (T)-36, psub(vp2[1], vm0[1]));           // 101
-            m[2] = pfmas(Lz[1], (T)36, padd(tt1[3], vm0[3]));            // 010
-            m[9] = pfmas(Dz[1], (T)-36, psub(vp2[3], vm0[3]));           // 011
-            m[4] = pfmas(Dz[2], (T)-36, tt1[2]);                         // 200
+            m[0] = padd(tt1[0], vm0[0]);                                 // 000
+            m[3] = psub(e3, vm0[0]);                                     // 001
+            m[6] = padd(e6, vm0[0]);                                     // 002
+            m[1] = padd(tt1[1], vm0[1]);                                 // 100
+            m[8] = psub(e8, vm0[1]);                                     // 101
+            m[2] = padd(tt1[3], vm0[3]);                                 // 010
+            m[9] = psub(e9, vm0[3]);                                     // 011
+            m[4] = tt1[2];                                               // 200
             m[7] = tt1[4];                                               // 110
-            m[5] = pfmas(Dz[2], (T)-36, tt1[5]);                         // 020
+            m[5] = tt1[5];                                               // 020
             if (WALLY) { m[3] = padd(m[3], kwall[0]); m[6] = padd(m[6], kwall[1]); m[8] = padd(m[8], kwall[2]); m[9] = padd(m[9], kwall[3]); }
 
             // ---- a8: finalise the two rows from their 216-scaled raw moments (m[1..3] lack their base 216 u), Eq. 12 ------
@@ -716,17 +808,20 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             o[8] = pfma(rx, o[3], pmuls(m[8], hi));
             o[9] = pfma(ry, o[3], pmuls(m[9], hi));
 
-            // ---- into the output tile (the store thread has read the previous plane out of it) ------------------------------
-            mbar_wait(sb + B_OEMPTY, (uint32_t)((i - 1) & 1));
+            // ---- into the output tile of this parity (the store thread has read the plane before the previous one out of it;
+            //      with a single tile: the previous one) --------------------------------------------------------------------
+            constexpr int ob = NOUT == 2 ? PAR : 0;
+            mbar_wait(sb + B_OEMPTY + 8 * ob, NOUT == 2 ? ph : (uint32_t)(PAR ^ 1));
             if (lane_out) {
+                const uint32_t ao = aO + ob * OUT_BYTES;
 #pragma unroll
                 for (int f = 0; f < TSLB_NF; ++f) {
-                    sts(aO + f * (ROWS * COLS) * ES, o[f].x);
-                    sts(aO + (f * (ROWS * COLS) + COLS) * ES, o[f].y);
+                    sts(ao + f * (ROWS * COLS) * ES, o[f].x);
+                    sts(ao + (f * (ROWS * COLS) + COLS) * ES, o[f].y);
                 }
             }
-            fence_async_smem();
-            warp_arrive(sb + B_OFULL, lane);
+            if (!TILE_FENCE_STORER) fence_async_smem();
+            warp_arrive(sb + B_OFULL + 8 * ob, lane);
             if (xedge || xtail) {
                 T *rp = Bbuf + ((long long)zt * L.plane + (long long)r0 * L.px);
                 if (xtail) {
@@ -741,16 +836,11 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                 }
             }
         }
-        // ---- shift the march state ---------------------------------------------------------------------------------
-#pragma unroll
-        for (int g = 0; g < 6; ++g) {
-            if (g == 0 || g == 1 || g == 3) vp2[g] = vp1[g];
-            tt1[g] = tn[g];                              // Vp(zs-1) + centre(zs): used when plane zs+1 arrives
-            vp1[g] = vp0[g];
-        }
-#pragma unroll
-        for (int a = 0; a < 3; ++a) uprev[a] = rc[1 + a];
-        if (++stg == NS) { stg = 0; fpar ^= 1; }
+    };
+    for (int i = 0; i < nplanes; i += 2) {
+        plane(std::integral_constant<int, 0>(), i);
+        if (i + 1 < nplanes) plane(std::integral_constant<int, 1>(), i + 1);
+        ph ^= 1;
     }
 }
 
