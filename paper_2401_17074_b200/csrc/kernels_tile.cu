@@ -363,7 +363,53 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         if (wid >= TD::NMAIN) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_HALO ? TileGeom<T>::REG_HALO : 24));
         else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_MAIN ? TileGeom<T>::REG_MAIN : 24));
     }
-    if (wid >= TD::WARPS) return;                         // idle warps (they only complete a warpgroup for setmaxnreg)
+    static_assert(TileGeom<T>::NIDLE == 2, "the two warps that complete the helpers' warpgroup are the producer and the store warp");
+    if (wid >= TD::WARPS) {
+        // ============================================ producer warp / store warp ==========================================
+        // One lane each.  They are warps of their own (not lanes of the halo warps) so that a load is issued the moment its
+        // stage has been released and a store the moment its tile is full, whatever the halo warps are doing: with the
+        // producer inside a halo warp the load of plane i+1 could not be issued before plane i-1 had LANDED and been
+        // processed there, which left the main warps waiting ~300 cycles per plane for their data.
+        if (lane != 0) return;
+        if (wid == TD::WARPS) {
+            const bool yper = p.kind[2] == TSLB_BC_PERIODIC, zper = p.kind[4] == TSLB_BC_PERIODIC;
+            // source rows of the two halo rows: wrapped on a periodic axis, out of bounds (zero fill) beyond a wall / open face
+            const int ylo = row0 > 0 ? row0 - 1 : (yper ? L.ny - 1 : -1);
+            const int yhi = row0 + ROWS < L.ny ? row0 + ROWS : (yper ? 0 : L.ny);
+            for (int j = 0; j < nplanes; ++j) {            // source plane z0-1+j into stage j % NS
+                int zs = z0 - 1 + j;
+                if (zs < 0) zs = zper ? L.nz - 1 : -1;
+                else if (zs >= L.nz) zs = zper ? 0 : L.nz;
+                const int s = j % NS;
+                if (j >= NS) mbar_wait(sb + B_EMPTY + 8 * s, (uint32_t)((j / NS - 1) & 1));
+                const uint32_t dst = sb + s * STAGE_BYTES, bar = sb + B_FULL + 8 * s;
+                mbar_expect_tx(bar, (uint32_t)TD::STAGE_TX);
+                tma_load_4d(dst, &tmMain, bar, x0, row0, zs, 0);
+                tma_load_4d(dst + TD::MAIN_ELEMS * ES, &tmRow, bar, x0, ylo, zs, 0);
+                tma_load_4d(dst + (TD::MAIN_ELEMS + TD::HALO_ELEMS) * ES, &tmRow, bar, x0, yhi, zs, 0);
+            }
+        } else {
+            // output plane m of this chunk (z = z0 + m) sits in output tile m % NOUT; its k-th use completes phase k of the
+            // tile's ofull / oempty barriers.  With two tiles the store of plane m is left in flight and the tile of plane
+            // m-1 is handed back once ITS store has read the shared memory (at most one bulk group pending).
+            for (int m = 0; m < nplanes - 2; ++m) {
+                const int b = m % NOUT;
+                mbar_wait(sb + B_OFULL + 8 * b, (uint32_t)((m / NOUT) & 1));
+                if (TILE_FENCE_STORER) fence_async_smem();
+                tma_store_4d(sb + TD::OFF_OUT + b * OUT_BYTES, &tmStore, x0 + TSLB_XOFF, row0, z0 + m, 0);
+                tma_store_commit();
+                if (NOUT == 1) {
+                    tma_store_wait_read();
+                    mbar_arrive(sb + B_OEMPTY);
+                } else if (m >= 1) {
+                    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                    mbar_arrive(sb + B_OEMPTY + 8 * ((m - 1) % NOUT));
+                }
+            }
+            tma_store_wait_all();
+        }
+        return;
+    }
     if (wid >= TD::NMAIN) {
         // =================================================== halo warps ===================================================
         const int h = wid - TD::NMAIN;
@@ -373,56 +419,12 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         const uint32_t aA = keep(sb + (TD::MAIN_ELEMS + TD::HALO_ELEMS + bcol) * ES), aB = keep(sb + (TD::MAIN_ELEMS + bcol) * ES);
         const uint32_t aW = keep(sb + TD::OFF_EX + (WY * NGRP * EXW + ecol) * ES);      // exX[WY]; exY[0] is HALO_Y further
         constexpr int HALO_Y = 2 * SLOT_BYTES - WY * PACK_BYTES;
-        // source rows of the two halo rows: wrapped on a periodic axis, out of bounds (zero fill) beyond a wall / open face
-        const bool yper = p.kind[2] == TSLB_BC_PERIODIC;
-        const int ylo = row0 > 0 ? row0 - 1 : (yper ? L.ny - 1 : -1);
-        const int yhi = row0 + ROWS < L.ny ? row0 + ROWS : (yper ? 0 : L.ny);
-        const bool zper = p.kind[4] == TSLB_BC_PERIODIC;
-        auto issue = [&](int j) {                          // source plane z0-1+j into stage j % NS
-            int zs = z0 - 1 + j;
-            if (zs < 0) zs = zper ? L.nz - 1 : -1;
-            else if (zs >= L.nz) zs = zper ? 0 : L.nz;
-            const int s = j % NS;
-            const uint32_t dst = sb + s * STAGE_BYTES, bar = sb + B_FULL + 8 * s;
-            mbar_expect_tx(bar, (uint32_t)TD::STAGE_TX);
-            tma_load_4d(dst, &tmMain, bar, x0, row0, zs, 0);
-            tma_load_4d(dst + TD::MAIN_ELEMS * ES, &tmRow, bar, x0, ylo, zs, 0);
-            tma_load_4d(dst + (TD::MAIN_ELEMS + TD::HALO_ELEMS) * ES, &tmRow, bar, x0, yhi, zs, 0);
-        };
-        const bool producer = h == 0 && lane == 0, storer = h == 1 && lane == 0;
-        if (producer)
-            for (int j = 0; j < NS - 1 && j < nplanes; ++j) issue(j);
         // rows beyond a bounce-back wall send nothing (their raw moments are zero-filled, but A100 = 3 g is not zero)
         const P hm = pk((WALLY && p.kind[3] == TSLB_BC_BOUNCE_BACK && row0 + ROWS >= L.ny) ? (T)0 : (T)1,
                         (WALLY && p.kind[2] == TSLB_BC_BOUNCE_BACK && row0 == 0) ? (T)0 : (T)1);
-        // output plane m of this chunk (z = z0 + m) sits in output tile m % NOUT; its k-th use completes phase k of the
-        // tile's ofull / oempty barriers.  With two tiles the store of plane m is left in flight and the tile of plane m-1 is
-        // handed back once ITS store has read the shared memory (at most one bulk group pending).
-        auto store_tile = [&](int m) {
-            const int b = m % NOUT;
-            mbar_wait(sb + B_OFULL + 8 * b, (uint32_t)((m / NOUT) & 1));
-            if (TILE_FENCE_STORER) fence_async_smem();
-            tma_store_4d(sb + TD::OFF_OUT + b * OUT_BYTES, &tmStore, x0 + TSLB_XOFF, row0, z0 + m, 0);
-            tma_store_commit();
-            if (NOUT == 1) {
-                tma_store_wait_read();
-                mbar_arrive(sb + B_OEMPTY);
-            } else if (m >= 1) {
-                asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-                mbar_arrive(sb + B_OEMPTY + 8 * ((m - 1) % NOUT));
-            }
-        };
         int stg = 0;
         uint32_t fpar = 0;
         for (int i = 0; i < nplanes; ++i) {
-            if (producer) {
-                const int j = i + NS - 1;                  // refill the stage of plane i-1 with plane j
-                if (j < nplanes) {
-                    if (i >= 1) mbar_wait(sb + B_EMPTY + 8 * (j % NS), (uint32_t)((j / NS - 1) & 1));
-                    issue(j);
-                }
-            }
-            __syncwarp();
             const uint32_t so = stg * STAGE_BYTES;
             mbar_wait(sb + B_FULL + 8 * stg, fpar);
             P rh[TSLB_NF];
@@ -459,13 +461,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #undef TSLB_HALO_GROUP
             __syncwarp();
             if (lane == 0) { mbar_arrive(sb + B_Q + 8 * (i & 1)); mbar_arrive(sb + B_Q + 16 * (WY + 1) + 8 * (i & 1)); }
-            // the output tile the main warps finished in their iteration i-1 (output plane i-3)
-            if (storer && i >= 3) store_tile(i - 3);
             if (++stg == NS) { stg = 0; fpar ^= 1; }
-        }
-        if (storer) {
-            if (nplanes >= 3) store_tile(nplanes - 3);
-            tma_store_wait_all();
         }
         return;
     }
