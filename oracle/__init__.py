@@ -63,6 +63,9 @@ def _load():
         lib.oracle_destroy.restype = None
         lib.oracle_set_moments.argtypes = [C.c_void_p, dp]
         lib.oracle_set_force.argtypes = [C.c_void_p, dp]
+        lib.oracle_set_sponge.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double]
+        lib.oracle_tau_of_plane.argtypes = [C.c_void_p, C.c_int]
+        lib.oracle_tau_of_plane.restype = C.c_double
         lib.oracle_set_face.argtypes = [C.c_void_p, C.c_int, C.c_int, dp, C.c_double, C.c_uint64, C.c_int]
         lib.oracle_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
         lib.oracle_get_moments.argtypes = [C.c_void_p, dp]
@@ -144,6 +147,13 @@ class Oracle:
     def set_force(self, g3):
         g = np.ascontiguousarray(g3, dtype=np.float64)
         self._chk(self._lib.oracle_set_force(self._h, _dptr(g)), "oracle_set_force")
+
+    def set_sponge(self, z_start: int, K: float, p: float = 3.0):
+        """Sponge layer towards z = nz (Eq. 26; reading A24).  K = 0 removes it."""
+        self._chk(self._lib.oracle_set_sponge(self._h, int(z_start), float(K), float(p)), "oracle_set_sponge")
+
+    def tau_of_plane(self, z: int) -> float:
+        return float(self._lib.oracle_tau_of_plane(self._h, int(z)))
 
     def set_face(self, face: int, kind: int, u_plane=None, noise_amp: float = 0.0, seed: int = 0,
                  noise_mask: int = 0):

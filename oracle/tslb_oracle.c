@@ -16,6 +16,7 @@
  *   - body force term rho w_i c_i.F / c_s^2
  *   - NEQ-extrapolation open boundaries (Dirichlet u / zero gradient)  PAPER.md:181-202 (Eq. 22-23), :258
  *   - halfway bounce-back no-slip walls  (paper only says "no-slip"; reading A12 in DESIGN.md)
+ *   - sponge layer nu(z) = nu (K ((z - z_start)/(N_z - z_start))^p + 1)  PAPER.md:264-268 (Eq. 26; reading A24 in DESIGN.md)
  *
  * Readings of garbled / ambiguous passages are listed in DESIGN.md ("Readings").  In short:
  * Eq. 18's duplicated third-order equilibrium term is taken once; w_i multiplies the whole
@@ -58,6 +59,7 @@ typedef struct {
     double tau, omega;     /* omega = 1/tau, nu = cs2 (1/omega - 1/2) */
     double g[3];           /* body acceleration */
     int order;             /* Hermite order of the expansion: 3 (Eq. 18, default) or 2 (Eq. 8) */
+    double *omega_z;       /* sponge layer: relaxation frequency of the nodes of plane z, or NULL (uniform omega) */
     int kind[6];           /* per face */
     double *uin[6];        /* inlet planes [3][n_b][n_a], owned copy, or NULL */
     double noise_amp[6];
@@ -210,6 +212,7 @@ void oracle_destroy(oracle_ctx *c)
 {
     if (!c) return;
     for (int f = 0; f < 6; ++f) free(c->uin[f]);
+    free(c->omega_z);
     free(c->M[0]); free(c->M[1]); free(c);
 }
 
@@ -228,6 +231,38 @@ int oracle_set_order(oracle_ctx *c, int order)
     if (!c || (order != 2 && order != 3)) return 1;
     c->order = order;
     return 0;
+}
+
+/* Sponge layer (Eq. 26): the kinematic viscosity grows towards the z = N_z exit,
+ *     nu_sponge(z) = nu ( K ((z - z_start) / (N_z - z_start))^p + 1 )   for z >= z_start,   nu otherwise,
+ * and with it the relaxation time of the nodes of that plane, tau(z) = 1/2 + nu_sponge(z)/cs2.
+ * Reading A24: the printed denominator "N_z - z_end" is the width of the layer, N_z - z_start, and the
+ * printed exponent "p = -3" is p = +3 (a negative exponent diverges at z = z_start); p is an argument here.
+ * The collision is local (Eq. 6): the population that leaves a node was relaxed with THAT node's omega, so the sweep
+ * takes omega of the upstream (source) node.  K = 0 removes the layer. */
+int oracle_set_sponge(oracle_ctx *c, int z_start, double K, double p)
+{
+    if (!c || !isfinite(K) || !isfinite(p) || K < 0) return 1;
+    free(c->omega_z); c->omega_z = NULL;
+    if (K == 0) return 0;
+    const int nz = c->n[2];
+    if (z_start < 0 || z_start >= nz) return 1;
+    c->omega_z = (double *)malloc(sizeof(double) * nz);
+    if (!c->omega_z) return 2;
+    const double nu = CS2 * (c->tau - 0.5);
+    for (int z = 0; z < nz; ++z) {
+        double nu_z = nu;
+        if (z >= z_start) nu_z = nu * (K * pow((double)(z - z_start) / (double)(nz - z_start), p) + 1.0);
+        c->omega_z[z] = 1.0 / (0.5 + nu_z / CS2);
+    }
+    return 0;
+}
+
+/* tau of the nodes of plane z (for tests) */
+double oracle_tau_of_plane(const oracle_ctx *c, int z)
+{
+    if (!c || z < 0 || z >= c->n[2]) return 0;
+    return c->omega_z ? 1.0 / c->omega_z[z] : c->tau;
 }
 
 int oracle_set_force(oracle_ctx *c, const double *g3)
@@ -368,12 +403,14 @@ static void sweep(oracle_ctx *c, int mode)
                             double f;
                             if (bounced) {          /* halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) */
                                 const int cb[3] = { -cx, -cy, -cz };
-                                f = oracle_fstar_order(Mx, cb, c->omega, c->g, mode, c->order);
+                                const double om = c->omega_z ? c->omega_z[z] : c->omega;
+                                f = oracle_fstar_order(Mx, cb, om, c->g, mode, c->order);
                             } else {
                                 double Ms[NF];
                                 size_t iq = lin(c, q);
                                 for (int k = 0; k < NF; ++k) Ms[k] = A[k * N + iq];
-                                f = oracle_fstar_order(Ms, ci, c->omega, c->g, mode, c->order);
+                                const double om = c->omega_z ? c->omega_z[q[2]] : c->omega;   /* omega of the source node */
+                                f = oracle_fstar_order(Ms, ci, om, c->g, mode, c->order);
                             }
                             R += f;
                             for (int a = 0; a < 3; ++a) {

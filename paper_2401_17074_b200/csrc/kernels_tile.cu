@@ -272,7 +272,11 @@ template <> struct TileGeom<float> {
     static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, NIDLE = TILE_F32_NIDLE, REG_MAIN = TILE_F32_RM, REG_HALO = TILE_F32_RH;
     static constexpr int NOUT = TILE_F32_NOUT;
 };
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = 208, REG_HALO = 80, NOUT = 1; };
+#ifndef TILE_F64_RM
+#define TILE_F64_RM 208
+#define TILE_F64_RH 80
+#endif
+template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = TILE_F64_RM, REG_HALO = TILE_F64_RH, NOUT = 1; };
 constexpr int rup128(int bytes) { return (bytes + 127) / 128 * 128; }
 template <typename T> struct TileDims {
     typedef TileGeom<T> G;
@@ -524,13 +528,17 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     // partly covered unit would be written whole, over the ghost column), the columns beyond it are stored from registers
     const bool xtail = lane_out && col >= (L.nx & ~(16 / ES - 1)) && col < L.nx;
 
-    static_assert(NS == 2, "the plane loop is unrolled by two: stage = parity of the source plane");
-    // All barriers of the loop complete one phase every two planes (two stages, two exchange slots, two output tiles), so
-    // a single phase bit serves them all: ph = (i >> 1) & 1.
+    // The barriers of the exchange slots and of the output tiles complete one phase every two planes (two slots, two tiles):
+    // one phase bit serves them all, ph = (i >> 1) & 1; with NS == 2 it serves the stage ring as well and the stage offset is
+    // an immediate, otherwise the ring position is carried (stg, fpar).
     uint32_t ph = 0;
+    int stg = 0;
+    uint32_t fpar = 0;
     auto plane = [&](auto par_c, const int i) {
         constexpr int PAR = decltype(par_c)::value;
-        constexpr uint32_t so = PAR * STAGE_BYTES, xo = PAR * SLOT_BYTES;
+        constexpr uint32_t xo = PAR * SLOT_BYTES;
+        const uint32_t so = NS == 2 ? PAR * STAGE_BYTES : stg * STAGE_BYTES;
+        const uint32_t bring = NS == 2 ? sb + 8 * PAR : sb + 8 * stg;          // + B_FULL / B_EMPTY
         P (&vp1)[6] = vpb[1 - PAR];          // Vp(zs-1)
         P (&vp0)[6] = vpb[PAR];              // Vp(zs-2) on entry (groups 0, 1, 3 read it first), Vp(zs) on exit
         P (&tt1)[6] = ttb[PAR];
@@ -539,7 +547,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         P (&ucur)[3] = ub[PAR];
         P (&dprev)[3] = db[1 - PAR];
         P (&dcur)[3] = db[PAR];
-        mbar_wait(sb + B_FULL + 8 * PAR, ph);
+        mbar_wait(bring + B_FULL, NS == 2 ? ph : fpar);
 
         // ---- a1: moments of the own rows r0, r0+1 and the velocities of the rows r0-1, r0+2 at this column ------------------
         P rc[TSLB_NF], hu[3];
@@ -565,7 +573,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #pragma unroll
             for (int k = 0; k < 3; ++k) hu[k] = pk(hl[k], hh[k]);
         }
-        warp_arrive(sb + B_EMPTY + 8 * PAR, lane);       // the stage can be refilled: everything needed is in registers
+        warp_arrive(bring + B_EMPTY, lane);              // the stage can be refilled: everything needed is in registers
+        if (NS != 2 && ++stg == NS) { stg = 0; fpar ^= 1; }
 
         // ---- a2: Hermite coefficients of the own rows, all three rounds; y-pass combinations of the 8 groups -------------
         // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)); P(r0-1) and M(r0+2) are read from the neighbours,

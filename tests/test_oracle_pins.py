@@ -692,3 +692,77 @@ def test_plane_statistics_vs_numpy_central_moments(oracle_mod):
     assert np.abs(rxy - (up[0] * up[1]).mean(axis=(0, 2))).max() < 1e-15
     m3 = S[10:13] / S[0] - 3 * mean * S[4:7] / S[0] + 2 * mean**3
     assert np.abs(m3 - (up**3).mean(axis=(1, 3))).max() < 1e-16
+
+
+# ---------------------------------------------------------------------------------------------
+# Sponge layer (Eq. 26; reading A24): SURVEY.md 8(f) rank 3
+# ---------------------------------------------------------------------------------------------
+def _sponge_nu(nu, z, nz, z_start, K, p):
+    """Eq. 26 typed from the paper, with reading A24 (layer width in the denominator)."""
+    return nu if z < z_start else nu * (K * ((z - z_start) / (nz - z_start)) ** p + 1.0)
+
+
+def test_sponge_K0_is_no_sponge(oracle_mod):
+    w = W.random_state(6, 5, 9, seed=21, tau=0.6)
+    a = _mk(oracle_mod, w); b = _mk(oracle_mod, w)
+    b.set_sponge(4, 0.0, 3.0)
+    a.step(3); b.step(3)
+    assert np.array_equal(a.get_moments(), b.get_moments())
+
+
+def test_sponge_profile_paper_numbers(oracle_mod):
+    """K = 1000, z_start = N_z - 50, p = 3 (A24): tau(z) = 1/2 + 3 nu_sponge(z).
+    Fails for an off-by-one in z - z_start (tau(z_start) must be the bulk tau), a dropped '+ 1', or 1/tau vs tau mix-ups."""
+    nz, tau = 120, 0.5004
+    o = oracle_mod.Oracle(4, 4, nz, tau)
+    o.set_sponge(nz - 50, 1000.0, 3.0)
+    nu = (tau - 0.5) / 3
+    assert o.tau_of_plane(0) == tau and o.tau_of_plane(nz - 51) == tau
+    assert abs(o.tau_of_plane(nz - 50) - tau) < 1e-15
+    for z in (nz - 49, nz - 25, nz - 1):
+        assert abs(o.tau_of_plane(z) - (0.5 + 3 * _sponge_nu(nu, z, nz, nz - 50, 1000.0, 3))) < 1e-13
+    # last plane: (49/50)^3 * 1000 + 1 = 942.192 times the bulk viscosity
+    assert abs((o.tau_of_plane(nz - 1) - 0.5) / (tau - 0.5) - 942.192) < 1e-6
+    taus = [o.tau_of_plane(z) for z in range(nz)]
+    assert all(b >= a for a, b in zip(taus, taus[1:]))
+
+
+def test_sponge_population_code_equivalence(oracle_mod):
+    """Collision is local (Eq. 1, 5): a population code that relaxes every node with ITS OWN omega(z) and then streams
+    gives the same moments as the thread-safe sweep with the sponge.  Fails if the sweep takes omega of the destination
+    node instead of the source node, or applies the profile along another axis."""
+    nx, ny, nz, tau = 6, 5, 10, 0.56
+    w = W.random_state(nx, ny, nz, seed=22, tau=tau)
+    g = (1e-4, 2e-4, -1e-4)
+    z_start, K, p = 4, 7.0, 3.0
+    o = oracle_mod.Oracle(nx, ny, nz, tau)
+    o.set_force(g); o.set_sponge(z_start, K, p); o.set_moments(w.moments)
+    pop = PopulationLB(w.moments, tau, g)
+    nu = CS2 * (tau - 0.5)
+    tau_z = np.array([0.5 + _sponge_nu(nu, z, nz, z_start, K, p) / CS2 for z in range(nz)])
+    pop.omega = (1.0 / tau_z).reshape(1, nz, 1, 1)         # broadcasts over [direction][z][y][x]
+    for s in range(5):
+        o.step(1); pop.step()
+        assert np.abs(o.get_moments() - pop.M()).max() < 5e-15, s
+    # and the layer matters: without it the result differs
+    o2 = oracle_mod.Oracle(nx, ny, nz, tau); o2.set_force(g); o2.set_moments(w.moments); o2.step(5)
+    assert np.abs(o2.get_moments() - o.get_moments()).max() > 1e-6
+
+
+def test_sponge_two_region_decay(oracle_mod):
+    """p = 0 turns Eq. 26 into a step: nu in z < z_start, (K + 1) nu above.  A shear wave u_y = U sin(kx), uniform in z,
+    decays as exp(-nu_local k^2 t) on planes far from the two interfaces (periodic z) -- the viscosity <-> tau map with
+    the factor (K + 1) applied on the right planes."""
+    nx, ny, nz, tau, K = 32, 3, 48, 0.56, 2.0
+    k = 2 * np.pi / nx
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.0
+    M[2] = 1e-3 * np.sin(k * np.arange(nx))[None, None, :]
+    o = oracle_mod.Oracle(nx, ny, nz, tau)
+    o.set_sponge(24, K, 0.0); o.set_moments(M)
+    # (measured between two times: the start from Pi_neq = 0 has an initial layer of a few steps)
+    o.step(20); R1 = o.get_moments()
+    o.step(40); R2 = o.get_moments()
+    nu = CS2 * (tau - 0.5)
+    for z, nu_loc in ((12, nu), (36, (K + 1) * nu)):
+        a1 = (R1[2, z] * M[2, z]).sum(); a2 = (R2[2, z] * M[2, z]).sum()
+        assert abs(-np.log(a2 / a1) / (k * k * 40) / nu_loc - 1) < 0.03, (z, a1, a2)
