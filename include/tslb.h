@@ -110,6 +110,16 @@ int tslb_set_boundary(tslb_ctx *ctx, int face, int kind, const void *params);
  * part, Eq. 7).  Same stored state, same traffic; only the arithmetic changes.  TSLB_EINVAL for any other value. */
 int tslb_set_order(tslb_ctx *ctx, int order);
 
+/* Sponge layer towards the z = nz exit (Eq. 26): the kinematic viscosity of the nodes of plane z is
+ *     nu(z) = nu ( K ((z - z_start) / (nz - z_start))^p + 1 )   for z >= z_start,     nu otherwise,
+ * i.e. a relaxation time tau(z) = 1/2 + 3 nu(z) per plane; the post-collision population of a node is
+ * relaxed with the tau of THAT (source) node (Eq. 6).  Reading A24: the printed denominator "N_z - z_end"
+ * is the width of the layer and the printed exponent "-3" is +3; p is an argument (paper: K = 1000, z_start = nz - 50).
+ * K == 0 removes the layer.  Host-side call, takes effect at the next tslb_step (the per-plane table lives in the
+ * workspace and is uploaded on the stream of that step).  Both sweep kernels honour it.
+ * TSLB_EINVAL: K < 0, non-finite K or p, z_start outside [0, nz). */
+int tslb_set_sponge(tslb_ctx *ctx, int z_start, double K, double p);
+
 /* Choose the sweep kernel (TSLB_KERNEL_*).  TSLB_EINVAL if TILE is forced on a configuration it does not
  * cover (reported by tslb_step). */
 int tslb_set_kernel(tslb_ctx *ctx, int kernel);

@@ -71,6 +71,7 @@ def _load():
         lib.oracle_get_moments.argtypes = [C.c_void_p, dp]
         lib.oracle_diagnostics.argtypes = [C.c_void_p, dp]
         lib.oracle_plane_statistics.argtypes = [C.c_void_p, C.c_int, dp]
+        lib.oracle_radial_statistics.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_int, dp]
         lib.oracle_step_count.argtypes = [C.c_void_p]
         lib.oracle_step_count.restype = C.c_longlong
         lib.oracle_num_threads.restype = C.c_int
@@ -183,6 +184,13 @@ class Oracle:
         n_axis = self.shape[2 - axis]
         assert sums.dtype == np.float64 and sums.shape == (13, n_axis) and sums.flags["C_CONTIGUOUS"]
         self._chk(self._lib.oracle_plane_statistics(self._h, int(axis), _dptr(sums)), "oracle_plane_statistics")
+        return sums
+
+    def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums: np.ndarray) -> np.ndarray:
+        """ADD one sample of the (r, z)-bin sums [8][nz][nr] of a jet along z (reading A27)."""
+        assert sums.dtype == np.float64 and sums.flags["C_CONTIGUOUS"] and sums.shape == (8, self.shape[0], nr)
+        self._chk(self._lib.oracle_radial_statistics(self._h, float(xc), float(yc), float(dr), int(nr), _dptr(sums)),
+                  "oracle_radial_statistics")
         return sums
 
     @property

@@ -507,6 +507,44 @@ int oracle_plane_statistics(oracle_ctx *c, int axis, double *sums)
     return 0;
 }
 
+/* Running (r, z)-bin statistics of a round jet along z (Fig. 7-8: centre-line velocity, half-width,
+ * mean axial profile, axial / radial rms and the Reynolds stress <u'_z u'_r> on sections z = const).  Reading A27
+ * (DESIGN.md): with (xc, yc) the jet axis in node coordinates, dx = x - xc, dy = y - yc, r = sqrt(dx^2 + dy^2), a node
+ * belongs to bin k = floor(r / dr) of its plane if k < nr; the cylindrical components are u_r = (u_x dx + u_y dy) / r,
+ * u_t = (u_y dx - u_x dy) / r (both 0 on the axis, r = 0).  For every plane z and bin k ADD to sums[8][nz][nr]
+ *     1 | u_z | u_r | u_t | u_z^2 | u_r^2 | u_t^2 | u_z u_r
+ * at the current time (boundary nodes refilled first); the caller zeroes the array once and calls once per sample. */
+int oracle_radial_statistics(oracle_ctx *c, double xc, double yc, double dr, int nr, double *sums)
+{
+    if (!c || !sums || nr < 1 || !(dr > 0) || !isfinite(xc) || !isfinite(yc)) return 1;
+    if (!c->have_state) return 4;
+    const size_t N = (size_t)c->n[0] * c->n[1] * c->n[2];
+    const int nz = c->n[2];
+    double *M = c->M[c->cur];
+    ghost_fill(c, M);
+    for (int z = 0; z < nz; ++z)
+        for (int y = 0; y < c->n[1]; ++y)
+            for (int x = 0; x < c->n[0]; ++x) {
+                const double dx = x - xc, dy = y - yc;
+                const double r = sqrt(dx * dx + dy * dy);
+                const double kf = floor(r / dr);
+                if (!(kf < nr)) continue;
+                const int k = (int)kf;
+                const int p[3] = { x, y, z };
+                const size_t i = lin(c, p);
+                const double ux = M[N + i], uy = M[2 * N + i], uz = M[3 * N + i];
+                double ur = 0, ut = 0;
+                if (r > 0) { ur = (ux * dx + uy * dy) / r; ut = (uy * dx - ux * dy) / r; }
+                double *s = sums + (size_t)z * nr + k;
+                const size_t row = (size_t)nz * nr;
+                s[0 * row] += 1.0;
+                s[1 * row] += uz; s[2 * row] += ur; s[3 * row] += ut;
+                s[4 * row] += uz * uz; s[5 * row] += ur * ur; s[6 * row] += ut * ut;
+                s[7 * row] += uz * ur;
+            }
+    return 0;
+}
+
 long long oracle_step_count(const oracle_ctx *c) { return c ? c->t : -1; }
 
 int oracle_num_threads(void)

@@ -25,7 +25,7 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
-           "tslb_export_state", "tslb_import_state")
+           "tslb_export_state", "tslb_import_state", "tslb_set_sponge")
 
 
 class InletParams(C.Structure):
@@ -64,6 +64,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_set_boundary.argtypes = [vp, ip, ip, vp]
     lib.tslb_set_kernel.argtypes = [vp, ip]
     lib.tslb_set_order.argtypes = [vp, ip]
+    lib.tslb_set_sponge.argtypes = [vp, ip, C.c_double, C.c_double]
     lib.tslb_active_kernel.argtypes = [vp]
     lib.tslb_step.argtypes = [vp, ip, vp]
     lib.tslb_get_moments.argtypes = [vp, vp, vp]
@@ -187,6 +188,10 @@ class TSLB:
         """Hermite order of the reconstruction: 3 (Eq. 18, default) or 2 (Eq. 8)."""
         self._chk(self._lib.tslb_set_order(self._h, int(order)), "tslb_set_order")
 
+    def set_sponge(self, z_start: int, K: float, p: float = 3.0):
+        """Sponge layer towards z = nz (Eq. 26; reading A24).  K = 0 removes it."""
+        self._chk(self._lib.tslb_set_sponge(self._h, int(z_start), float(K), float(p)), "tslb_set_sponge")
+
     def set_kernel(self, kernel: int):
         self._chk(self._lib.tslb_set_kernel(self._h, int(kernel)), "tslb_set_kernel")
 
@@ -287,5 +292,7 @@ def from_workload(w, kernel: int = KERNEL_AUTO) -> TSLB:
         sim.set_body_force(w.g)
     if getattr(w, "order", 3) != 3:
         sim.set_order(w.order)
+    if getattr(w, "sponge", None):
+        sim.set_sponge(*w.sponge)
     sim.set_kernel(kernel)
     return sim

@@ -124,6 +124,12 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
         }
     }
 
+    // 1 - omega of the source node: uniform, or per plane inside a sponge layer (Eq. 26)
+    T bsrc[3] = {p.beta, p.beta, p.beta};
+    if (p.beta_z) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) bsrc[k] = p.beta_z[sz[k]];
+    }
     T dR = 0, Jx = 0, Jy = 0, Jz = 0, Sxx = 0, Syy = 0, Szz = 0, Sxy = 0, Sxz = 0, Syz = 0;
 #pragma unroll
     for (int cz = -1; cz <= 1; ++cz)
@@ -136,7 +142,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                 const T w = (T)((cx ? 1 : 4) * (cy ? 1 : 4) * (cz ? 1 : 4));
                 T f;
                 if (cx == 0 && cy == 0 && cz == 0) {
-                    f = fstar_incr(own, 0, 0, 0, (T)1, w, p.beta, (T)0, p.o3);
+                    f = fstar_incr(own, 0, 0, 0, (T)1, w, bsrc[1], (T)0, p.o3);
                 } else {
                     // halfway bounce-back: f_i(x,t+1) = f*_ibar(x,t) from the node's own moments
                     const long long is = bounced ? ip : lay_idx(p.L, sx[cx + 1], sy[cy + 1], sz[cz + 1]);
@@ -150,7 +156,7 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
                         lin = -((T)cx * ((T)2 * own.ux + smx) + (T)cy * ((T)2 * own.uy + smy) + (T)cz * ((T)2 * own.uz + smz));
                     else
                         lin = (T)cx * ((m.ux - own.ux) + smx) + (T)cy * ((m.uy - own.uy) + smy) + (T)cz * ((m.uz - own.uz) + smz);
-                    f = fstar_incr(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, p.beta, lin, p.o3);
+                    f = fstar_incr(m, cx, cy, cz, bounced ? (T)-1 : (T)1, w, bounced ? bsrc[1] : bsrc[cz + 1], lin, p.o3);
                 }
                 dR += f;                                  // arrival direction c_i in every sum
                 if (cx) Jx += (T)cx * f;
@@ -421,6 +427,7 @@ SweepParams<T> make_params(const tslb_ctx *c)
     p.beta = (T)(1.0 - c->omega);
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
     p.o3 = c->order >= 3 ? (T)1 : (T)0;
+    p.beta_z = c->beta_z_host ? (const T *)c->beta_z : nullptr;
     return p;
 }
 

@@ -147,6 +147,7 @@ struct TileParams {
     Layout L;
     int kind[6];
     T beta, g[3];
+    const T *beta_z;   // sponge layer (Eq. 26): 1 - omega of the nodes of plane z, [nz] (SPONGE instantiations only)
     int zchunk;  // planes per z chunk
 };
 
@@ -314,7 +315,7 @@ template <typename T> struct TileDims {
 static_assert(TileDims<float>::SMEM_BYTES <= 232448 && TileDims<double>::SMEM_BYTES <= 232448, "shared memory budget");
 static_assert(TileGeom<float>::WX == 2 && TileGeom<double>::WX == 2, "two warps per row pair publish; two halo warps");
 
-template <typename T, bool WALLY, int ORDER>
+template <typename T, bool WALLY, int ORDER, bool SPONGE>
 __global__ void __maxnreg__(TileDims<T>::MAXREG)
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
                   const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p)
@@ -350,6 +351,13 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     const int z0 = blockIdx.z * p.zchunk;
     const int z1 = min(z0 + p.zchunk, L.nz);
     const int nplanes = z1 - z0 + 2;                     // source planes z0-1 .. z1
+    // z of the i-th source plane (wrapped on a periodic axis; beyond a wall / open face the plane is zero-filled and the
+    // index only has to be valid): needed for the per-plane relaxation of a sponge layer
+    auto zsrc = [&](int i) {
+        const int zs = z0 - 1 + i;
+        const bool zp = p.kind[4] == TSLB_BC_PERIODIC;
+        return zs < 0 ? (zp ? L.nz - 1 : 0) : (zs >= L.nz ? (zp ? 0 : L.nz - 1) : zs);
+    };
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -430,6 +438,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         uint32_t fpar = 0;
         for (int i = 0; i < nplanes; ++i) {
             const uint32_t so = stg * STAGE_BYTES;
+            T bz = p.beta;
+            if (SPONGE) bz = __ldg(p.beta_z + zsrc(i));
             mbar_wait(sb + B_FULL + 8 * stg, fpar);
             P rh[TSLB_NF];
 #pragma unroll
@@ -455,7 +465,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #define TSLB_HALO_ROUND(KZ)                                                                       \
             {                                                                                     \
                 P A[3][3];                                                                        \
-                hermite_round<KZ, P, T>(rh, p.beta, p.g, A);                                      \
+                hermite_round<KZ, P, T>(rh, bz, p.g, A);                                          \
                 TSLB_HALO_GROUP(0, KZ) TSLB_HALO_GROUP(1, KZ) TSLB_HALO_GROUP(2, KZ)              \
             }
             TSLB_HALO_ROUND(0)
@@ -547,6 +557,9 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         P (&ucur)[3] = ub[PAR];
         P (&dprev)[3] = db[1 - PAR];
         P (&dcur)[3] = db[PAR];
+        // 1 - omega of the source plane: uniform, or per plane inside a sponge layer (Eq. 26)
+        T bz = p.beta;
+        if (SPONGE) bz = __ldg(p.beta_z + zsrc(i));
         mbar_wait(bring + B_FULL, NS == 2 ? ph : fpar);
 
         // ---- a1: moments of the own rows r0, r0+1 and the velocities of the rows r0-1, r0+2 at this column ------------------
@@ -594,7 +607,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #define TSLB_MAIN_ROUND(KZ)                                                                       \
             {                                                                                     \
                 P A[3][3];                                                                        \
-                hermite_round<KZ, P, T>(rc, p.beta, p.g, A);                                      \
+                hermite_round<KZ, P, T>(rc, bz, p.g, A);                                          \
                 TSLB_MAIN_GROUP(0, KZ) TSLB_MAIN_GROUP(1, KZ) TSLB_MAIN_GROUP(2, KZ)              \
             }
             TSLB_MAIN_ROUND(0)
@@ -856,6 +869,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
     p.L = c->L;
     for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
     p.beta = (T)(1.0 - c->omega);
+    p.beta_z = c->beta_z_host ? (const T *)c->beta_z : nullptr;
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
     const int gx = (c->nx + TileDims<T>::COLS - 1) / TileDims<T>::COLS;
     const int gy = (c->ny + TileDims<T>::ROWS - 1) / TileDims<T>::ROWS;
@@ -952,7 +966,9 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     }
     const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
     e = cudaSuccess;
-#define TSLB_SMEM_ATTR(T, W, O, B) if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
+#define TSLB_SMEM_ATTR(T, W, O, B)                                                                                              \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
     TSLB_SMEM_ATTR(float, false, 3, smem32); TSLB_SMEM_ATTR(float, true, 3, smem32);
     TSLB_SMEM_ATTR(float, false, 2, smem32); TSLB_SMEM_ATTR(float, true, 2, smem32);
     TSLB_SMEM_ATTR(double, false, 3, smem64); TSLB_SMEM_ATTR(double, true, 3, smem64);
@@ -969,8 +985,12 @@ static void launch_tile(tslb_ctx *c, cudaStream_t st)
     dim3 grid;
     TileParams<T> p = make_tile<T>(c, &grid);
     const int a = c->cur, b = 1 - c->cur;
-    sweep_tile_kernel<T, WALLY, ORDER><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a], c->tm_store[b],
-                                                                                                   (T *)c->buf[b], p);
+    if (p.beta_z)
+        sweep_tile_kernel<T, WALLY, ORDER, true><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],
+                                                                                                             c->tm_store[b], (T *)c->buf[b], p);
+    else
+        sweep_tile_kernel<T, WALLY, ORDER, false><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],
+                                                                                                              c->tm_store[b], (T *)c->buf[b], p);
 }
 
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)

@@ -36,6 +36,7 @@ size_t scratch_bytes(const tslb_ctx *c)
 }
 
 size_t buffer_bytes(const tslb_ctx *c) { return align256((size_t)TSLB_NF * (size_t)c->L.field * tslb_elem(c)); }
+size_t sponge_bytes(const tslb_ctx *c) { return align256((size_t)c->nz * sizeof(double)); }
 
 // padded internal layout (tslb_internal.h): ghost columns x = -1 and x = nx, node x = 0 on a 16-byte boundary, 16-byte rows,
 // never narrower than a TMA box
@@ -136,6 +137,7 @@ void tslb_destroy(tslb_ctx *c)
     if (!c) return;
     for (int i = 0; i < 2 * c->ev_cap; ++i) cudaEventDestroy(c->ev[i]);
     free(c->ev);
+    free(c->beta_z_host);
     free(c);
 }
 
@@ -176,7 +178,7 @@ int tslb_get_timing(tslb_ctx *c, int *n_launches, double *total_ms)
 size_t tslb_workspace_bytes(const tslb_ctx *c)
 {
     if (!c) return 0;
-    return 2 * buffer_bytes(c) + scratch_bytes(c);
+    return 2 * buffer_bytes(c) + scratch_bytes(c) + sponge_bytes(c);
 }
 
 int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
@@ -196,6 +198,8 @@ int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
     c->buf[0] = dev_ptr;
     c->buf[1] = (char *)dev_ptr + buffer_bytes(c);
     c->scratch = (double *)((char *)dev_ptr + 2 * buffer_bytes(c));
+    c->beta_z = (char *)dev_ptr + 2 * buffer_bytes(c) + scratch_bytes(c);
+    c->sponge_dirty = c->beta_z_host != nullptr;
     c->cur = 0; c->t = 0; c->have_state = 0; c->halo_valid = 0;
     // padding cells are never written by the kernels: give them a defined (zero) value once
     e = cudaMemset(dev_ptr, 0, 2 * buffer_bytes(c));
@@ -280,6 +284,30 @@ int tslb_set_order(tslb_ctx *c, int order)
     return TSLB_OK;
 }
 
+int tslb_set_sponge(tslb_ctx *c, int z_start, double K, double p)
+{
+    if (!c) return TSLB_EINVAL;
+    if (!isfinite(K) || !isfinite(p) || K < 0) return fail(c, TSLB_EINVAL, "sponge: K must be finite and >= 0, p finite");
+    free(c->beta_z_host);
+    c->beta_z_host = nullptr;
+    c->sponge_dirty = 0;
+    if (K == 0) return TSLB_OK;
+    if (z_start < 0 || z_start >= c->nz) return fail(c, TSLB_EINVAL, "sponge: z_start outside [0, nz)");
+    c->beta_z_host = malloc((size_t)c->nz * tslb_elem(c));
+    if (!c->beta_z_host) return fail(c, TSLB_ENOMEM, "host allocation failed");
+    // Eq. 26 in double; 1 - omega(z) rounded once to the context dtype, like the uniform beta (Eq. 5)
+    const double nu = (c->tau - 0.5) / 3.0;
+    for (int z = 0; z < c->nz; ++z) {
+        double nuz = nu;
+        if (z >= z_start) nuz = nu * (K * pow((double)(z - z_start) / (double)(c->nz - z_start), p) + 1.0);
+        const double beta = 1.0 - 1.0 / (0.5 + 3.0 * nuz);
+        if (c->dtype == TSLB_F64) ((double *)c->beta_z_host)[z] = beta;
+        else ((float *)c->beta_z_host)[z] = (float)beta;
+    }
+    c->sponge_dirty = 1;
+    return TSLB_OK;
+}
+
 int tslb_set_kernel(tslb_ctx *c, int kernel)
 {
     if (!c) return TSLB_EINVAL;
@@ -306,6 +334,11 @@ int tslb_step(tslb_ctx *c, int n, void *stream)
     const int k = pick_kernel(c, &why);
     if (k < 0) return fail(c, TSLB_EINVAL, "TSLB_KERNEL_TILE does not cover this configuration: %s", why);
     cudaStream_t st = (cudaStream_t)stream;
+    if (c->sponge_dirty) {               // per-plane relaxation table of the sponge layer
+        cudaError_t e = cudaMemcpyAsync(c->beta_z, c->beta_z_host, (size_t)c->nz * tslb_elem(c), cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(c, "sponge table upload", e);
+        c->sponge_dirty = 0;
+    }
     for (int s = 0; s < n; ++s) {
         cudaError_t e = refresh_boundary(c, k == TSLB_KERNEL_TILE, st);    // step 1: boundary nodes (+ ghost layers) at time t
         if (e != cudaSuccess) return cuda_fail(c, "fill/halo kernel", e);

@@ -37,6 +37,7 @@ struct SweepParams {
     T beta;        // 1 - omega = 1 - 1/tau, formed in double and rounded once (Eq. 5)
     T g[3];        // body acceleration
     T o3;          // 1 for the third-order expansion (Eq. 18), 0 for the second-order one (Eq. 8)
+    const T *beta_z;  // sponge layer (Eq. 26): 1 - omega of the nodes of plane z, [nz]; NULL = uniform beta
 };
 
 struct InletDev {
@@ -69,6 +70,9 @@ struct tslb_ctx {
     size_t ws_bytes;
     void *buf[2];     // moment buffers, internal form (padded SoA, field 0 holds rho - 1)
     double *scratch;  // diagnostics partials
+    void *beta_z;     // sponge layer: per-plane 1 - omega in the context dtype, [nz] (in the workspace)
+    void *beta_z_host;   // the same on the host (staging for the upload), NULL = no sponge layer
+    int sponge_dirty;    // the host table has to be uploaded before the next sweep
     CUtensorMap tm_main[2], tm_row[2], tm_store[2];  // TMA descriptors of buf[0], buf[1]: tile rows, one halo row, output tile
     int tmap_ok;
     int cur;          // buf[cur] holds time t

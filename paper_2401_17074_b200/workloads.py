@@ -48,6 +48,7 @@ class Workload:
     g: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     inlet: Optional[Inlet] = None
     order: int = 3               # Hermite order of the reconstruction (3: Eq. 18, 2: Eq. 8)
+    sponge: Optional[Tuple[int, float, float]] = None     # (z_start, K, p) of the sponge layer (Eq. 26), or None
 
     @property
     def sites(self) -> int:

@@ -27,6 +27,8 @@ def make_oracle(oracle_mod, w):
     o.set_force(w.g)
     if getattr(w, "order", 3) != 3:
         o.set_order(w.order)
+    if getattr(w, "sponge", None):
+        o.set_sponge(*w.sponge)
     o.set_moments(w.moments)          # the run-dtype array, converted exactly to fp64
     return o
 

@@ -254,6 +254,31 @@ def test_order2_config1_reduced(B, oracle_mod):
 
 
 # ---------------------------------------------------------------------------------------------
+# sponge layer (Eq. 26, tslb_set_sponge): SURVEY.md 8(f) rank 3
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_sponge_parity(B, oracle_mod, dtype):
+    """Per-plane relaxation time along z in both kernels: periodic box (the layer wraps around), channel walls, and the jet
+    set (inlet at z = 0, outlets elsewhere) with the paper's K = 1000, p = 3 on a layer of 10 planes; several z chunks and
+    tiles.  Also: K = 0 is bit-identical to no layer."""
+    cases = [W.random_state(70, 27, 40, seed=41, dtype=dtype, tau=0.56),
+             with_faces(W.random_state(66, 15, 21, seed=42, dtype=dtype, tau=0.6),
+                        {W.FACE_YLO: W.BC_BOUNCE_BACK, W.FACE_YHI: W.BC_BOUNCE_BACK}, g=(2e-4, 0, -1e-4)),
+             with_faces(W.random_state(24, 17, 30, seed=43, dtype=dtype, tau=0.52), **BC_SETS["jet_like"])]
+    for w, sp in zip(cases, [(25, 40.0, 3.0), (9, 1000.0, 3.0), (20, 1000.0, 3.0)]):
+        w.sponge = sp
+        for k in kernels_for(B, w):
+            G, R, _ = run_both(oracle_mod, w, 5, k)
+            assert_parity(w, G, R, "sponge, kernel %d" % k)
+            w0 = W.Workload(**{**w.__dict__, "sponge": None})
+            G0, _, _ = run_both(oracle_mod, w0, 5, k)
+            assert np.abs(G0 - G).max() > 1e-7                 # the layer changes the result
+            wk0 = W.Workload(**{**w.__dict__, "sponge": (sp[0], 0.0, 3.0)})
+            Gk0, _, _ = run_both(oracle_mod, wk0, 5, k)
+            assert np.array_equal(Gk0, G0)
+
+
+# ---------------------------------------------------------------------------------------------
 # plane statistics (Eq. 24-25 raw sums, tslb_plane_statistics): SURVEY.md 8(f) rank 1
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])

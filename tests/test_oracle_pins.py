@@ -766,3 +766,57 @@ def test_sponge_two_region_decay(oracle_mod):
     for z, nu_loc in ((12, nu), (36, (K + 1) * nu)):
         a1 = (R1[2, z] * M[2, z]).sum(); a2 = (R2[2, z] * M[2, z]).sum()
         assert abs(-np.log(a2 / a1) / (k * k * 40) / nu_loc - 1) < 0.03, (z, a1, a2)
+
+
+# ---------------------------------------------------------------------------------------------
+# (r, z)-bin statistics of the jet (Fig. 7-8; reading A27): SURVEY.md 8(f) rank 1
+# ---------------------------------------------------------------------------------------------
+def test_radial_statistics_analytic_swirling_jet(oracle_mod):
+    """u_z = exp(-r^2/s^2), u_r = a r, u_t = b r written in Cartesian components: every bin sum is then a sum of known
+    functions of the node radii, evaluated here with numpy's hypot / bincount (library routines, no shared code).
+    Fails for swapped u_r / u_t projections, a wrong sign of u_t, bins along the wrong axis or a missing z index."""
+    nx, ny, nz, nr, dr = 21, 19, 4, 6, 1.5
+    xc, yc, s2, a, b = 9.25, 8.5, 30.0, 2e-3, -1e-3
+    X, Y = np.meshgrid(np.arange(nx) - xc, np.arange(ny) - yc)          # [ny][nx]
+    r = np.hypot(X, Y)
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.0
+    for z in range(nz):
+        M[3, z] = (1 + 0.1 * z) * np.exp(-r * r / s2)
+        M[1, z] = a * X - b * Y                                          # u_r e_r + u_t e_t, e_r = (X, Y)/r, e_t = (-Y, X)/r
+        M[2, z] = a * Y + b * X
+    o = oracle_mod.Oracle(nx, ny, nz, 0.7); o.set_moments(M)
+    S = np.zeros((8, nz, nr)); o.radial_statistics(xc, yc, dr, nr, S)
+    k = np.floor(r / dr).astype(int)
+    sel = k < nr
+    cnt = np.bincount(k[sel], minlength=nr)
+    for z in range(nz):
+        uz = M[3, z]
+        exp = [cnt, np.bincount(k[sel], uz[sel], nr), np.bincount(k[sel], (a * r)[sel], nr), np.bincount(k[sel], (b * r)[sel], nr),
+               np.bincount(k[sel], (uz * uz)[sel], nr), np.bincount(k[sel], (a * r)[sel] ** 2, nr),
+               np.bincount(k[sel], (b * r)[sel] ** 2, nr), np.bincount(k[sel], (uz * a * r)[sel], nr)]
+        for row in range(8):
+            assert np.abs(S[row, z] - exp[row]).max() < 1e-13, (row, z)
+    # a second sample adds
+    o.radial_statistics(xc, yc, dr, nr, S)
+    assert np.abs(S[0, 0] - 2 * cnt).max() == 0
+
+
+def test_radial_statistics_axis_node_and_rotation(oracle_mod):
+    """A node exactly on the axis has no radial direction: it counts in bin 0 with u_r = u_t = 0.  Rotating the field
+    by 90 degrees about a centred axis leaves every sum unchanged (the bins are rings)."""
+    n, nz, nr, dr = 11, 3, 5, 1.0
+    w = W.random_state(n, n, nz, seed=8)
+    M = w.moments.astype(np.float64)
+    o = oracle_mod.Oracle(n, n, nz, 0.7); o.set_moments(M)
+    S = np.zeros((8, nz, nr)); o.radial_statistics(5.0, 5.0, dr, nr, S)
+    assert np.all(S[0, :, 0] == 1.0)                                    # only the axis node has r < 1
+    assert np.abs(S[1, :, 0] - M[3, :, 5, 5]).max() == 0 and np.all(S[2, :, 0] == 0) and np.all(S[3, :, 0] == 0)
+    # rotate by +90 degrees about z: (x, y) -> (-y, x); u_x' = -u_y, u_y' = u_x on the rotated nodes
+    Mr = np.empty_like(M)
+    rot = lambda F: np.rot90(F, k=1, axes=(2, 1))                       # value at (x, y) moves to (-y, x) (centred grid)
+    for f in range(10):
+        Mr[f] = rot(M[f])
+    Mr[1], Mr[2] = -rot(M[2]), rot(M[1])
+    o2 = oracle_mod.Oracle(n, n, nz, 0.7); o2.set_moments(Mr)
+    S2 = np.zeros((8, nz, nr)); o2.radial_statistics(5.0, 5.0, dr, nr, S2)
+    assert np.abs(S2 - S).max() < 1e-13
