@@ -168,6 +168,18 @@ int tslb_get_timing(tslb_ctx *ctx, int *n_launches, double *total_ms);
  * fixed-order final pass (bitwise reproducible).  TSLB_EINVAL: bad axis or NULL; TSLB_ESTATE: no state. */
 int tslb_plane_statistics(tslb_ctx *ctx, int axis, double *dev_sums, void *stream);
 
+/* Running (r, z)-bin statistics of a round jet along z (Fig. 7-8: centre-line velocity and Eq. 27,
+ * half-width, mean axial profile, axial / radial rms, Reynolds stress <u'_z u'_r> on sections z = const).  Reading A27
+ * (DESIGN.md): with (xc, yc) the jet axis in node coordinates, dx = x - xc, dy = y - yc, r = sqrt(dx^2 + dy^2), a node
+ * belongs to ring k = floor(r / dr) of its plane if k < nr; u_r = (u_x dx + u_y dy) / r, u_t = (u_y dx - u_x dy) / r
+ * (both 0 on the axis).  For every plane z and ring k the sums of
+ *     1 | u_z | u_r | u_t | u_z^2 | u_r^2 | u_t^2 | u_z u_r
+ * at the current time (open-face boundary nodes refilled first) are ADDED to dev_sums, [8][nz][nr] doubles in device
+ * memory.  The caller zeroes the array once and calls once per sample.  fp64 throughout; the ring index is decided in
+ * fp64 without fused multiply-adds (identical on every IEEE machine); the additions use atomics, so repeated runs agree
+ * to rounding, not bitwise.  TSLB_EINVAL: NULL, dr <= 0, non-finite arguments, nr outside [1, 512]; TSLB_ESTATE: no state. */
+int tslb_radial_statistics(tslb_ctx *ctx, double xc, double yc, double dr, int nr, double *dev_sums, void *stream);
+
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);
 /* Number of kernels this context has launched so far (all kinds), for bench.py's gpu_launches. */

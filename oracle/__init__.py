@@ -26,6 +26,8 @@ _lib = None
 FIELDS = ("rho", "ux", "uy", "uz", "Pxx", "Pyy", "Pzz", "Pxy", "Pxz", "Pyz")
 FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
 BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT = range(4)
+BC_OUTLET_PRESSURE = 5
+NOISE_GAUSSIAN = 0x100
 MODE_BRUTE, MODE_CLOSED = 0, 1
 
 
@@ -58,6 +60,9 @@ def _load():
         lib.oracle_noise_r24.argtypes = [C.c_uint64, C.c_longlong, C.c_longlong]
         lib.oracle_noise_xi.restype = C.c_double
         lib.oracle_noise_xi.argtypes = [C.c_uint64, C.c_longlong, C.c_longlong]
+        lib.oracle_noise_gauss.restype = C.c_double
+        lib.oracle_noise_gauss.argtypes = [C.c_uint64, C.c_longlong, C.c_longlong]
+        lib.oracle_set_pressure_outlet.argtypes = [C.c_void_p, C.c_int, C.c_double]
         lib.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(C.c_void_p)]
         lib.oracle_destroy.argtypes = [C.c_void_p]
         lib.oracle_destroy.restype = None
@@ -104,6 +109,10 @@ def noise_xi(seed: int, t: int, idx: int) -> float:
     return float(_load().oracle_noise_xi(C.c_uint64(seed), t, idx))
 
 
+def noise_gauss(seed: int, t: int, idx: int) -> float:
+    return float(_load().oracle_noise_gauss(C.c_uint64(seed), int(t), int(idx)))
+
+
 def num_threads() -> int:
     return int(_load().oracle_num_threads())
 
@@ -148,6 +157,10 @@ class Oracle:
     def set_force(self, g3):
         g = np.ascontiguousarray(g3, dtype=np.float64)
         self._chk(self._lib.oracle_set_force(self._h, _dptr(g)), "oracle_set_force")
+
+    def set_pressure_outlet(self, face: int, rho: float):
+        """Density-imposed outlet: u and Pi_neq from x_F, rho imposed."""
+        self._chk(self._lib.oracle_set_pressure_outlet(self._h, int(face), float(rho)), "oracle_set_pressure_outlet")
 
     def set_sponge(self, z_start: int, K: float, p: float = 3.0):
         """Sponge layer towards z = nz (Eq. 26; reading A24).  K = 0 removes it."""

@@ -52,7 +52,8 @@
 #define NF 10
 
 enum { FACE_XLO = 0, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI };
-enum { BC_PERIODIC = 0, BC_BOUNCE_BACK = 1, BC_VELOCITY_INLET = 2, BC_OUTLET_ZERO_GRADIENT = 3 };
+enum { BC_PERIODIC = 0, BC_BOUNCE_BACK = 1, BC_VELOCITY_INLET = 2, BC_OUTLET_ZERO_GRADIENT = 3, BC_OUTLET_PRESSURE = 5 };
+#define NOISE_GAUSSIAN 0x100   /* bit 8 of the noise mask: Gaussian law instead of the uniform one */
 
 typedef struct {
     int n[3];              /* nx, ny, nz */
@@ -65,6 +66,7 @@ typedef struct {
     double noise_amp[6];
     uint64_t seed[6];
     int noise_mask[6];
+    double rho_out[6];     /* imposed density of a pressure outlet */
     double *M[2];          /* ping-pong ("AB flip-flop") moment buffers */
     int cur;
     long long t;
@@ -186,6 +188,19 @@ uint32_t oracle_noise_r24(uint64_t seed, long long t, long long idx)
     k = mix64(k + (uint64_t)idx);
     return (uint32_t)(k >> 40);
 }
+/* Gaussian variant ("time-varying Gaussian noise"; reading A14b in DESIGN.md): Box-Muller on two uniforms of
+ * the same counter-based stream, u1 = (r24 + 1) / 2^24 in (0, 1] from the first hash, u2 = r24' / 2^24 in [0, 1) from the
+ * hash of that hash:  xi = sqrt(-2 ln u1) cos(2 pi u2)  -- zero mean, unit variance. */
+double oracle_noise_gauss(uint64_t seed, long long t, long long idx)
+{
+    uint64_t k = mix64(seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(t + 1)));
+    uint64_t a = mix64(k + (uint64_t)idx);
+    uint64_t b = mix64(a);
+    double u1 = ((double)(uint32_t)(a >> 40) + 1.0) / 16777216.0;
+    double u2 = (double)(uint32_t)(b >> 40) / 16777216.0;
+    return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
+}
+
 double oracle_noise_xi(uint64_t seed, long long t, long long idx)
 {
     return (double)oracle_noise_r24(seed, t, idx) / 8388608.0 - 1.0;   /* 2 r / 2^24 - 1 */
@@ -298,7 +313,18 @@ int oracle_set_face(oracle_ctx *c, int face, int kind, const double *u_plane, do
     return 0;
 }
 
-static int is_open(int kind) { return kind == BC_VELOCITY_INLET || kind == BC_OUTLET_ZERO_GRADIENT; }
+static int is_open(int kind) { return kind == BC_VELOCITY_INLET || kind == BC_OUTLET_ZERO_GRADIENT || kind == BC_OUTLET_PRESSURE; }
+
+/* Pressure (density-imposed) outlet, PAPER.md:187 ("imposing the hydrodynamic variables at the boundary (either momentum
+ * or density/pressure)") and :202: the boundary node takes u and Pi_neq of x_F and the imposed rho. */
+int oracle_set_pressure_outlet(oracle_ctx *c, int face, double rho)
+{
+    if (!c || face < 0 || face > 5 || !(rho > 0) || !isfinite(rho)) return 1;
+    free(c->uin[face]); c->uin[face] = NULL;
+    c->kind[face] = BC_OUTLET_PRESSURE;
+    c->rho_out[face] = rho;
+    return 0;
+}
 
 /* A node is a boundary node if it lies on a face of kind INLET/OUTLET (step 1 of the update). */
 static int on_open_face(const oracle_ctx *c, const int p[3])
@@ -340,6 +366,13 @@ static void ghost_fill(oracle_ctx *c, double *M)
                 }
                 size_t ib = lin(c, p), iF = lin(c, q);
                 for (int k = 0; k < NF; ++k) M[k * N + ib] = M[k * N + iF];
+                for (int f = 0; f < 6; ++f) {        /* imposed density (lowest pressure face that holds the node) */
+                    if (c->kind[f] != BC_OUTLET_PRESSURE) continue;
+                    int on = (f % 2 == 0) ? (p[f / 2] == 0) : (p[f / 2] == c->n[f / 2] - 1);
+                    if (!on) continue;
+                    M[ib] = c->rho_out[f];
+                    break;
+                }
                 for (int f = 0; f < 6; ++f) {
                     if (c->kind[f] != BC_VELOCITY_INLET) continue;
                     int ax, a, b; face_axes(f, &ax, &a, &b);
@@ -347,7 +380,8 @@ static void ghost_fill(oracle_ctx *c, double *M)
                     if (!on) continue;
                     size_t pl = (size_t)c->n[a] * c->n[b];
                     size_t j = (size_t)p[b] * c->n[a] + p[a];
-                    double xi = oracle_noise_xi(c->seed[f], c->t, (long long)ib);
+                    double xi = (c->noise_mask[f] & NOISE_GAUSSIAN) ? oracle_noise_gauss(c->seed[f], c->t, (long long)ib)
+                                                                    : oracle_noise_xi(c->seed[f], c->t, (long long)ib);
                     for (int k = 0; k < 3; ++k) {
                         double v = c->uin[f][k * pl + j];
                         if (c->noise_mask[f] & (1 << k)) v *= 1.0 + c->noise_amp[f] * xi;

@@ -25,7 +25,7 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
-           "tslb_export_state", "tslb_import_state", "tslb_set_sponge")
+           "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics")
 
 
 class InletParams(C.Structure):
@@ -73,6 +73,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_export_state.argtypes = [vp, vp, C.POINTER(C.c_longlong), vp]
     lib.tslb_import_state.argtypes = [vp, vp, C.c_longlong, vp]
     lib.tslb_plane_statistics.argtypes = [vp, ip, vp, vp]
+    lib.tslb_radial_statistics.argtypes = [vp, C.c_double, C.c_double, C.c_double, ip, vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
@@ -245,6 +246,18 @@ class TSLB:
             raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
         self._chk(self._lib.tslb_plane_statistics(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
                   "tslb_plane_statistics")
+        return sums
+
+    def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums=None, stream=None):
+        """Add one sample of the (r, z)-bin sums of a jet along z to sums[8][nz][nr] (CUDA fp64)."""
+        import torch
+        shape = (8, self.shape[0], int(nr))
+        if sums is None:
+            sums = torch.zeros(shape, dtype=torch.float64, device="cuda")
+        if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == shape):
+            raise ValueError("sums must be a contiguous CUDA float64 tensor of shape %s" % (shape,))
+        self._chk(self._lib.tslb_radial_statistics(self._h, float(xc), float(yc), float(dr), int(nr),
+                                                   C.c_void_p(sums.data_ptr()), _stream_ptr(stream)), "tslb_radial_statistics")
         return sums
 
     def set_timing(self, max_launches: int):

@@ -418,6 +418,54 @@ __global__ void stats_final_kernel(const double *__restrict__ partial, int n_axi
     sums[i] += v;
 }
 
+// ---------------------------------------------------------------------------------------------
+// (r, z)-bin statistics of a round jet along z (Fig. 7-8; reading A27 in DESIGN.md): a node of plane z
+// at distance r = sqrt(dx^2 + dy^2) from the axis (xc, yc) belongs to ring k = floor(r / dr) if k < nr; per plane and
+// ring the sums of 1 | u_z | u_r | u_t | u_z^2 | u_r^2 | u_t^2 | u_z u_r are ADDED to sums[8][nz][nr].
+// The ring index is an integer decided by floating point: it is taken in fp64 with the oracle's operation order and no
+// fused multiply-add (sqrt and the division are correctly rounded on both sides), so both sides bin identically.
+// One CTA per (plane, slab of rows): ring sums in shared memory (fp64 atomics), then one global atomic per ring and row
+// -- the order of the additions is not fixed, so repeated runs agree to rounding (~1e-16 relative), not bitwise.
+// ---------------------------------------------------------------------------------------------
+#define TSLB_RSTAT_ROWS 8
+#define TSLB_RSTAT_MAXBINS 512
+template <typename T>
+__global__ void __launch_bounds__(256) radial_stats_kernel(const T *__restrict__ A, Layout L, double xc, double yc, double dr, int nr,
+                                                           double *__restrict__ sums)
+{
+    __shared__ double sh[TSLB_RSTAT_ROWS][TSLB_RSTAT_MAXBINS];
+    const int z = blockIdx.x;
+    for (int i = threadIdx.x; i < TSLB_RSTAT_ROWS * nr; i += blockDim.x) sh[i / nr][i % nr] = 0.0;
+    __syncthreads();
+    const int rows_per = (L.ny + gridDim.y - 1) / gridDim.y;
+    const int y0 = blockIdx.y * rows_per, y1 = min(y0 + rows_per, L.ny);
+    for (int y = y0 + (threadIdx.x >> 5); y < y1; y += blockDim.x >> 5) {
+        const double dy = (double)y - yc;
+        const double dy2 = __dmul_rn(dy, dy);
+        for (int x = threadIdx.x & 31; x < L.nx; x += 32) {
+            const double dx = (double)x - xc;
+            const double r = sqrt(__dadd_rn(__dmul_rn(dx, dx), dy2));
+            const double kf = floor(r / dr);
+            if (!(kf < (double)nr)) continue;
+            const int k = (int)kf;
+            const long long idx = lay_idx(L, x, y, z);
+            const double ux = A[L.field + idx], uy = A[2 * L.field + idx], uz = A[3 * L.field + idx];
+            double ur = 0.0, ut = 0.0;
+            if (r > 0.0) { ur = (ux * dx + uy * dy) / r; ut = (uy * dx - ux * dy) / r; }
+            atomicAdd(&sh[0][k], 1.0);
+            atomicAdd(&sh[1][k], uz); atomicAdd(&sh[2][k], ur); atomicAdd(&sh[3][k], ut);
+            atomicAdd(&sh[4][k], uz * uz); atomicAdd(&sh[5][k], ur * ur); atomicAdd(&sh[6][k], ut * ut);
+            atomicAdd(&sh[7][k], uz * ur);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < TSLB_RSTAT_ROWS * nr; i += blockDim.x) {
+        const int row = i / nr, k = i % nr;
+        const double v = sh[row][k];
+        if (v != 0.0) atomicAdd(&sums[((long long)row * L.nz + z) * nr + k], v);
+    }
+}
+
 template <typename T>
 SweepParams<T> make_params(const tslb_ctx *c)
 {
@@ -511,6 +559,17 @@ cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st)
         diag_partial_kernel<double><<<TSLB_DIAG_BLOCKS, TSLB_DIAG_THREADS, 0, st>>>((const double *)c->buf[c->cur], make_fill(c), c->scratch);
     diag_final_kernel<<<1, 160, 0, st>>>(c->scratch, TSLB_DIAG_BLOCKS, dev_out5);
     c->launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t tslb_launch_radial_stats(tslb_ctx *c, double xc, double yc, double dr, int nr, double *dev_sums, cudaStream_t st)
+{
+    int parts = (c->ny + 63) / 64;          // slabs of ~64 rows: enough CTAs for small nz, few global atomics per ring
+    if (parts < 1) parts = 1;
+    dim3 grid(c->nz, parts);
+    if (c->dtype == TSLB_F32) radial_stats_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, xc, yc, dr, nr, dev_sums);
+    else radial_stats_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, xc, yc, dr, nr, dev_sums);
+    c->launches += 1;
     return cudaGetLastError();
 }
 

@@ -435,6 +435,21 @@ int tslb_plane_statistics(tslb_ctx *c, int axis, double *dev_sums, void *stream)
     return TSLB_OK;
 }
 
+int tslb_radial_statistics(tslb_ctx *c, double xc, double yc, double dr, int nr, double *dev_sums, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (!dev_sums) return fail(c, TSLB_EINVAL, "dev_sums == NULL");
+    if (!isfinite(xc) || !isfinite(yc) || !isfinite(dr) || !(dr > 0)) return fail(c, TSLB_EINVAL, "radial statistics: axis and dr must be finite, dr > 0");
+    if (nr < 1 || nr > 512) return fail(c, TSLB_EINVAL, "radial statistics: nr must be in [1, 512]");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = refresh_boundary(c, false, st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_radial_stats(c, xc, yc, dr, nr, dev_sums, st);
+    if (e != cudaSuccess) return cuda_fail(c, "radial statistics kernel", e);
+    return TSLB_OK;
+}
+
 long long tslb_step_count(const tslb_ctx *c) { return c && c->have_state ? c->t : -1; }
 long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
 const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err : g_create_err; }

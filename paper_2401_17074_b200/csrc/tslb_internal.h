@@ -108,6 +108,7 @@ cudaError_t tslb_launch_import_raw(tslb_ctx *c, const void *src, void *dst, cuda
 cudaError_t tslb_launch_export_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);
 cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st);
 cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st);
+cudaError_t tslb_launch_radial_stats(tslb_ctx *c, double xc, double yc, double dr, int nr, double *dev_sums, cudaStream_t st);
 
 #define TSLB_STAT_ROWS 13   // 1, u (3), uu (6), uuu (3)
 #define TSLB_STAT_PARTS 8   // CTAs per plane in the statistics reduction

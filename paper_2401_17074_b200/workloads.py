@@ -21,6 +21,8 @@ import numpy as np
 
 FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
 BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT = range(4)
+BC_OUTLET_PRESSURE = 5       # rho imposed (Workload.rho_out[face]), u and Pi_neq from the interior neighbour
+NOISE_GAUSSIAN = 0x100       # bit 8 of Inlet.noise_mask: Gaussian instead of uniform inlet noise
 
 _NP_DTYPE = {"f32": np.float32, "f64": np.float64}
 
@@ -49,6 +51,7 @@ class Workload:
     inlet: Optional[Inlet] = None
     order: int = 3               # Hermite order of the reconstruction (3: Eq. 18, 2: Eq. 8)
     sponge: Optional[Tuple[int, float, float]] = None     # (z_start, K, p) of the sponge layer (Eq. 26), or None
+    rho_out: Dict[int, float] = field(default_factory=dict)   # face -> imposed density of a BC_OUTLET_PRESSURE face
 
     @property
     def sites(self) -> int:

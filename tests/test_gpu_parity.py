@@ -253,6 +253,31 @@ def test_order2_config1_reduced(B, oracle_mod):
         assert_parity(w, G, R, "order 2 kernel %d" % k)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_radial_statistics_match_oracle(B, oracle_mod, dtype):
+    """(r, z)-bin sums of the jet (tslb_radial_statistics) against the oracle after a few steps of the jet boundary set:
+    ring counts bit-exact (the ring index is an integer both sides decide in fp64), sums to 1e-12 relative in fp64 /
+    to the state's own parity in fp32; off-centre axis, rings that leave the box, two samples accumulate."""
+    w = with_faces(W.random_state(45, 38, 12, seed=51, dtype=dtype, tau=0.6), **BC_SETS["jet_like"])
+    nr, dr, xc, yc = 9, 2.5, 21.3, 18.0
+    o = make_oracle(oracle_mod, w)
+    S = np.zeros((8, w.nz, nr))
+    for k in kernels_for(B, w)[-1:]:
+        sim = make_gpu(w, k)
+        G = None
+        for n in (0, 3):
+            sim.step(n); o.step(n)
+            G = sim.radial_statistics(xc, yc, dr, nr, G)
+            o.radial_statistics(xc, yc, dr, nr, S)
+        Gh = G.cpu().numpy()
+        assert np.array_equal(Gh[0], S[0])
+        assert S[0].sum() > 0 and S[0, :, -1].min() > 0
+        tol = 1e-12 if dtype == "f64" else 2e-5
+        scale = np.abs(S).max(axis=(1, 2), keepdims=True)
+        assert (np.abs(Gh - S) / scale).max() < tol, (np.abs(Gh - S) / scale).max()
+        sim.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # sponge layer (Eq. 26, tslb_set_sponge): SURVEY.md 8(f) rank 3
 # ---------------------------------------------------------------------------------------------

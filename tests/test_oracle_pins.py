@@ -820,3 +820,105 @@ def test_radial_statistics_axis_node_and_rotation(oracle_mod):
     o2 = oracle_mod.Oracle(n, n, nz, 0.7); o2.set_moments(Mr)
     S2 = np.zeros((8, nz, nr)); o2.radial_statistics(5.0, 5.0, dr, nr, S2)
     assert np.abs(S2 - S).max() < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# Boundary variants of section II.C: pressure outlet, NEQ no-slip wall, Gaussian inlet noise
+# ---------------------------------------------------------------------------------------------
+def test_pressure_outlet_populations_are_eq23_with_imposed_density(oracle_mod):
+    """'the equilibrium distribution is computed by imposing the hydrodynamic variables at the boundary
+    (either momentum or density/pressure), while the non-equilibrium part is extrapolated'.  The population pulled from a
+    pressure-outlet node is f_eq(rho_out, u(x_F)) + (1 - omega) f_neq(Pi(x_F), u(x_F)), built with the independent numpy
+    tensors.  Fails if rho is copied instead of imposed, or u is zeroed."""
+    nx, ny, nz, tau, rho_out = 6, 5, 7, 0.63, 0.97
+    w = W.random_state(nx, ny, nz, seed=43, tau=tau)
+    up = np.random.default_rng(9).uniform(-0.03, 0.03, (3, ny, nx))
+    o = oracle_mod.Oracle(nx, ny, nz, tau)
+    o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.0, 3, 0)
+    o.set_pressure_outlet(W.FACE_ZHI, rho_out)
+    o.set_moments(w.moments)
+    p = PopulationLB(w.moments, tau, (0.0, 0.0, 0.0))
+    M = w.moments.copy()
+    Pi_at = lambda M, z: np.array([[M[4, z], M[7, z], M[8, z]], [M[7, z], M[5, z], M[9, z]], [M[8, z], M[9, z], M[6, z]]])
+    for step in range(2):
+        post = _fstar_all(p, M)
+        uF = M[1:4, nz - 2]
+        fB = p.feq(np.full((ny, nx), rho_out), uF) + (1 - p.omega) * p.fneq_reg(Pi_at(M, nz - 2), uF)
+        want = _pull_plane(p, {1: post[:, nz - 3], 0: post[:, nz - 2], -1: fB})
+        o.step(1)
+        R = o.get_moments()
+        assert np.abs(R[:, nz - 2] - want).max() < 2e-15, step
+        f_copy = post[:, nz - 2]                                          # zero-gradient outlet instead
+        assert np.abs(_pull_plane(p, {1: post[:, nz - 3], 0: post[:, nz - 2], -1: f_copy}) - R[:, nz - 2]).max() > 1e-4
+        assert np.all(R[0, nz - 1] == rho_out) and np.array_equal(R[1:, nz - 1], R[1:, nz - 2])
+        M = R
+
+
+def test_pressure_outlet_uniform_through_flow(oracle_mod):
+    """Uniform flow leaving through a pressure outlet with rho_out = rho0 is a fixed point; a lower rho_out is not."""
+    nx, ny, nz = 5, 6, 8
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.02; M[3] = 0.03
+    up = np.zeros((3, ny, nx)); up[2] = 0.03
+    def run(rho_out):
+        o = oracle_mod.Oracle(nx, ny, nz, 0.58)
+        o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.0, 1, 0)
+        o.set_pressure_outlet(W.FACE_ZHI, rho_out)
+        o.set_moments(M); o.step(6)
+        return o.get_moments()
+    assert np.abs(run(1.02) - M).max() < 1e-15
+    assert np.abs(run(1.00)[:, nz - 2] - M[:, nz - 2]).max() > 1e-3
+
+
+def test_neq_no_slip_wall_poiseuille(oracle_mod):
+    """The Dirichlet member of section II.C with u_B = 0 is the paper's thread-safe no-slip wall:
+    wall nodes ON the faces y = 0, ny-1 with imposed zero velocity.  Steady forced flow between them is the parabola
+    u_x'' = -g/nu through u = 0 AT the wall nodes (halfway bounce-back puts the zero half a cell outside, P7)."""
+    nx, ny, nz, tau, g = 3, 25, 3, 0.9, 1e-6
+    nu = CS2 * (tau - 0.5)
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.0
+    zero = np.zeros((3, nz, nx))
+    o = oracle_mod.Oracle(nx, ny, nz, tau)
+    o.set_face(W.FACE_YLO, W.BC_VELOCITY_INLET, zero, 0.0, 1, 0)
+    o.set_face(W.FACE_YHI, W.BC_VELOCITY_INLET, zero, 0.0, 1, 0)
+    o.set_force((g, 0.0, 0.0)); o.set_moments(M)
+    o.step(6000)
+    u = o.get_moments()[1, 1, :, 1]
+    y = np.arange(ny)
+    exact = g / (2 * nu) * y * (ny - 1 - y)
+    assert np.all(u[[0, -1]] == 0.0)
+    assert np.abs(u - exact).max() / exact.max() < 0.02
+    assert abs(np.diff(u, 2)[3:-3].mean() / (-g / nu) - 1) < 0.01
+
+
+def test_gaussian_noise_is_box_muller_of_the_counter_stream(oracle_mod):
+    """xi = sqrt(-2 ln u1) cos(2 pi u2) with u1 = (r24 + 1)/2^24, u2 = r24'/2^24 from the pinned SplitMix64 mixer
+    (recomputed here through oracle.mix64, itself pinned to the published stream), and the sample moments of 2e5 draws
+    are those of a unit normal (mean 0, variance 1, kurtosis 3)."""
+    GOLD, mask = 0x9E3779B97F4A7C15, (1 << 64) - 1
+    seed, t = 77, 5
+    k = oracle_mod.mix64((seed ^ (GOLD * (t + 1))) & mask)
+    for idx in (0, 1, 12345, 2**31 + 7):
+        a = oracle_mod.mix64((k + idx) & mask); b = oracle_mod.mix64(a)
+        u1 = ((a >> 40) + 1) / 2.0**24; u2 = (b >> 40) / 2.0**24
+        assert abs(oracle_mod.noise_gauss(seed, t, idx) - np.sqrt(-2 * np.log(u1)) * np.cos(2 * np.pi * u2)) < 1e-14
+    x = np.array([oracle_mod.noise_gauss(3, 0, i) for i in range(200000)])
+    assert abs(x.mean()) < 0.01 and abs(x.var() - 1) < 0.02 and abs((x**4).mean() / x.var()**2 - 3) < 0.1
+    # consecutive steps and neighbouring nodes are uncorrelated
+    y = np.array([oracle_mod.noise_gauss(3, 1, i) for i in range(200000)])
+    assert abs(np.corrcoef(x, y)[0, 1]) < 0.01 and abs(np.corrcoef(x[:-1], x[1:])[0, 1]) < 0.01
+
+
+def test_gaussian_inlet_noise_enters_relatively(oracle_mod):
+    """Bit 8 of the noise mask switches the inlet to the Gaussian law: u_k = u_in,k (1 + amp xi_gauss) on masked components."""
+    nx, ny, nz = 4, 5, 6
+    M = np.zeros((10, nz, ny, nx)); M[0] = 1.0
+    up = np.zeros((3, ny, nx)); up[2] = 0.05; up[0] = 0.01
+    o = oracle_mod.Oracle(nx, ny, nz, 0.6)
+    o.set_face(W.FACE_ZLO, W.BC_VELOCITY_INLET, up, 0.1, 11, 0b100 | W.NOISE_GAUSSIAN)
+    o.set_face(W.FACE_ZHI, W.BC_OUTLET_ZERO_GRADIENT)
+    o.set_moments(M)
+    R = o.get_moments()
+    for y in range(ny):
+        for x in range(nx):
+            xi = oracle_mod.noise_gauss(11, 0, y * nx + x)
+            assert abs(R[3, 0, y, x] - 0.05 * (1 + 0.1 * xi)) < 1e-16 and R[1, 0, y, x] == 0.01
