@@ -51,8 +51,11 @@ enum {
     TSLB_BC_BOUNCE_BACK = 1,          /* halfway bounce-back no-slip wall half a cell outside the face */
     TSLB_BC_VELOCITY_INLET = 2,       /* nodes ON the face: u imposed, rho and Pi_neq from x_F          */
     TSLB_BC_OUTLET_ZERO_GRADIENT = 3, /* nodes ON the face: all 10 moments copied from x_F              */
-    TSLB_BC_BODY_FORCE = 4            /* not a face kind: sets the body acceleration g (face ignored)   */
+    TSLB_BC_BODY_FORCE = 4,           /* not a face kind: sets the body acceleration g (face ignored)   */
+    TSLB_BC_OUTLET_PRESSURE = 5       /* nodes ON the face: rho imposed, u and Pi_neq copied from x_F    */
 };
+/* Bit 8 of tslb_inlet_params.noise_component_mask: Gaussian noise law instead of the uniform one (below). */
+#define TSLB_NOISE_GAUSSIAN 0x100
 /* Which sweep kernel tslb_step uses. AUTO picks the TMA-staged register-marching tile kernel when the
  * boundary set allows it and the per-direction gather kernel otherwise. */
 enum { TSLB_KERNEL_AUTO = 0, TSLB_KERNEL_GATHER = 1, TSLB_KERNEL_TILE = 2 };
@@ -63,7 +66,10 @@ enum { TSLB_KERNEL_AUTO = 0, TSLB_KERNEL_GATHER = 1, TSLB_KERNEL_TILE = 2 };
  * Component k of node x_B at step t is  u_in,k * (1 + noise_amp * xi(seed, t, lin(x_B)))  when bit k of
  * noise_component_mask is set, else u_in,k;  xi in [-1,1) = 2 r24 / 2^24 - 1 with r24 the top 24 bits
  * of mix64(mix64(seed ^ (0x9E3779B97F4A7C15 * (t+1))) + lin), mix64 = SplitMix64's finaliser and
- * lin = (z*ny + y)*nx + x. */
+ * lin = (z*ny + y)*nx + x.  With TSLB_NOISE_GAUSSIAN set in the mask xi is instead the unit normal
+ * sqrt(-2 ln u1) cos(2 pi u2), u1 = (r24 + 1)/2^24, u2 = r24'/2^24 with r24' the top 24 bits of mix64 applied once
+ * more ("time-varying Gaussian noise"; evaluated in fp64).
+ * A zero u_in with no noise is the thread-safe NEQ no-slip wall of PAPER.md:161-187 (wall nodes ON the face). */
 typedef struct tslb_inlet_params {
     const void *dev_u_plane;
     double noise_amp;
@@ -99,6 +105,8 @@ int tslb_set_moments_host(tslb_ctx *ctx, const void *host_src, void *stream);
 /* Set the kind of one face, or the body force.
  *   PERIODIC / BOUNCE_BACK / OUTLET_ZERO_GRADIENT : params == NULL.
  *   VELOCITY_INLET : params -> tslb_inlet_params.
+ *   OUTLET_PRESSURE: params -> const double rho_out (> 0): density imposed on the face nodes, u and Pi_neq from x_F
+ *                    (PAPER.md:187 "either momentum or density/pressure", :202).
  *   BODY_FORCE     : params -> const double g[3] (acceleration; adds w_i rho c_i.g / cs^2 to the
  *                    post-collision population of the SOURCE node, reading A11); face ignored.
  * TSLB_EINVAL: unknown face/kind, missing params, non-finite g or noise_amp.  Consistency of the whole

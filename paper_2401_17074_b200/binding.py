@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(HERE, "libtslb.so")
 TSLB_F32, TSLB_F64 = 0, 1
 TSLB_OK, TSLB_EINVAL, TSLB_ENOMEM, TSLB_ECUDA, TSLB_ESTATE = range(5)
 FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
-BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE = range(5)
+BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE, BC_OUTLET_PRESSURE = range(6)
+NOISE_GAUSSIAN = 0x100
 KERNEL_AUTO, KERNEL_GATHER, KERNEL_TILE = range(3)
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile"}
 
@@ -169,8 +170,11 @@ class TSLB:
         self._chk(self._lib.tslb_set_moments_host(self._h, ptr, _stream_ptr(stream)), "tslb_set_moments_host")
 
     def set_boundary(self, face: int, kind: int, u_plane=None, noise_amp: float = 0.0, seed: int = 0,
-                     noise_mask: int = 0):
-        if kind == BC_VELOCITY_INLET:
+                     noise_mask: int = 0, rho_out: float = 1.0):
+        if kind == BC_OUTLET_PRESSURE:
+            rho = C.c_double(float(rho_out))
+            self._chk(self._lib.tslb_set_boundary(self._h, face, kind, C.cast(C.byref(rho), C.c_void_p)), "tslb_set_boundary")
+        elif kind == BC_VELOCITY_INLET:
             if u_plane is None:
                 raise ValueError("VELOCITY_INLET needs u_plane")
             self._check_tensor(u_plane, "u_plane")
@@ -299,6 +303,8 @@ def from_workload(w, kernel: int = KERNEL_AUTO) -> TSLB:
         if w.inlet is not None and face == w.inlet.face:
             up = torch.from_numpy(w.inlet.u_plane).to("cuda")
             sim.set_boundary(face, kind, up, w.inlet.noise_amp, w.inlet.seed, w.inlet.noise_mask)
+        elif kind == BC_OUTLET_PRESSURE:
+            sim.set_boundary(face, kind, rho_out=w.rho_out[face])
         else:
             sim.set_boundary(face, kind)
     if any(w.g):

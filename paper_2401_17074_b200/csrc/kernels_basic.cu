@@ -64,7 +64,7 @@ __device__ __forceinline__ T fstar_incr(const Site<T> &m, int cx, int cy, int cz
 
 __device__ __forceinline__ bool is_open_kind(int k)
 {
-    return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT;
+    return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT || k == TSLB_BC_OUTLET_PRESSURE;
 }
 
 template <typename P>
@@ -238,6 +238,13 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
     const long long iF = lay_idx(p.L, r[0], r[1], r[2]);
 #pragma unroll
     for (int k = 0; k < TSLB_NF; ++k) M[k * N + ib] = M[k * N + iF];
+    for (int f2 = 0; f2 < 6; ++f2) {     // imposed density (field 0 holds rho - 1): lowest pressure face that holds the node
+        if (p.kind[f2] != TSLB_BC_OUTLET_PRESSURE) continue;
+        const int ax2 = f2 >> 1;
+        if (q[ax2] != ((f2 & 1) ? n[ax2] - 1 : 0)) continue;
+        M[ib] = (T)(p.rho_out[f2] - 1.0);
+        break;
+    }
     for (int f2 = 0; f2 < 6; ++f2) {
         if (p.kind[f2] != TSLB_BC_VELOCITY_INLET) continue;
         const int ax2 = f2 >> 1;
@@ -248,7 +255,13 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
         const uint64_t lin = ((uint64_t)q[2] * p.L.ny + q[1]) * p.L.nx + q[0];   // API linear index of the node
         uint64_t k64 = mix64(p.inlet[f2].seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(p.t + 1)));
         k64 = mix64(k64 + lin);
-        const double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
+        double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
+        if (p.inlet[f2].mask & TSLB_NOISE_GAUSSIAN) {   // Box-Muller on two uniforms of the same stream, fp64
+            const uint64_t k2 = mix64(k64);
+            const double u1 = ((double)(uint32_t)(k64 >> 40) + 1.0) / 16777216.0;
+            const double u2 = (double)(uint32_t)(k2 >> 40) / 16777216.0;
+            xi = sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
+        }
         const T *up = (const T *)p.inlet[f2].u_plane;
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -483,7 +496,7 @@ FillParams make_fill(const tslb_ctx *c)
 {
     FillParams p;
     p.L = c->L;
-    for (int f = 0; f < 6; ++f) { p.kind[f] = c->kind[f]; p.inlet[f] = c->inlet[f]; }
+    for (int f = 0; f < 6; ++f) { p.kind[f] = c->kind[f]; p.inlet[f] = c->inlet[f]; p.rho_out[f] = c->rho_out[f]; }
     p.t = c->t;
     return p;
 }
@@ -504,10 +517,15 @@ cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st)
     return cudaGetLastError();
 }
 
+static bool is_open_kind_host(int k)
+{
+    return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT || k == TSLB_BC_OUTLET_PRESSURE;
+}
+
 static bool any_open(const tslb_ctx *c)
 {
     for (int f = 0; f < 6; ++f)
-        if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT) return true;
+        if (is_open_kind_host(c->kind[f])) return true;
     return false;
 }
 

@@ -73,7 +73,7 @@ int check_boundary_set(tslb_ctx *c)
 bool any_open(const tslb_ctx *c)
 {
     for (int f = 0; f < 6; ++f)
-        if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT) return true;
+        if (c->kind[f] == TSLB_BC_VELOCITY_INLET || c->kind[f] == TSLB_BC_OUTLET_ZERO_GRADIENT || c->kind[f] == TSLB_BC_OUTLET_PRESSURE) return true;
     return false;
 }
 
@@ -258,7 +258,13 @@ int tslb_set_boundary(tslb_ctx *c, int face, int kind, const void *params)
         return TSLB_OK;
     }
     if (face < 0 || face > 5) return fail(c, TSLB_EINVAL, "unknown face");
-    if (kind < 0 || kind > TSLB_BC_OUTLET_ZERO_GRADIENT) return fail(c, TSLB_EINVAL, "unknown boundary kind");
+    if (kind < 0 || kind > TSLB_BC_OUTLET_PRESSURE) return fail(c, TSLB_EINVAL, "unknown boundary kind");
+    if (kind == TSLB_BC_OUTLET_PRESSURE) {
+        if (!params) return fail(c, TSLB_EINVAL, "OUTLET_PRESSURE needs params -> double rho_out");
+        const double rho = *(const double *)params;
+        if (!isfinite(rho) || !(rho > 0)) return fail(c, TSLB_EINVAL, "rho_out must be finite and > 0");
+        c->rho_out[face] = rho;
+    }
     if (kind == TSLB_BC_VELOCITY_INLET) {
         if (!params) return fail(c, TSLB_EINVAL, "VELOCITY_INLET needs params -> tslb_inlet_params");
         const tslb_inlet_params *ip = (const tslb_inlet_params *)params;

@@ -51,6 +51,7 @@ struct FillParams {
     Layout L;
     int kind[6];
     InletDev inlet[6];
+    double rho_out[6];   // imposed density of the TSLB_BC_OUTLET_PRESSURE faces
     long long t;  // step index the fill belongs to (noise counter)
 };
 
@@ -64,6 +65,7 @@ struct tslb_ctx {
     double g[3];
     int kind[6];
     InletDev inlet[6];
+    double rho_out[6];
     Layout L;
     // device memory (caller-owned workspace)
     void *ws;

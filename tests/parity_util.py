@@ -22,6 +22,8 @@ def make_oracle(oracle_mod, w):
     for f, k in w.faces.items():
         if w.inlet is not None and f == w.inlet.face:
             o.set_face(f, k, w.inlet.u_plane, w.inlet.noise_amp, w.inlet.seed, w.inlet.noise_mask)
+        elif k == 5:                       # BC_OUTLET_PRESSURE
+            o.set_pressure_outlet(f, w.rho_out[f])
         else:
             o.set_face(f, k)
     o.set_force(w.g)

@@ -254,6 +254,34 @@ def test_order2_config1_reduced(B, oracle_mod):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_boundary_variants_of_section_IIC(B, oracle_mod, dtype):
+    """pressure (density-imposed) outlet, NEQ no-slip walls (zero-velocity Dirichlet nodes on the
+    faces) and the Gaussian inlet noise, on lattices that span several tiles, both kernels."""
+    def jet_pressure(shape, seed):
+        w = with_faces(W.random_state(*shape, seed=seed, dtype=dtype, tau=0.56), **BC_SETS["jet_like"])
+        w.faces[W.FACE_ZHI] = W.BC_OUTLET_PRESSURE
+        w.rho_out = {W.FACE_ZHI: 0.98}
+        w.inlet.noise_mask |= W.NOISE_GAUSSIAN
+        return w
+    def neq_walls(shape, seed):
+        w = W.random_state(*shape, seed=seed, dtype=dtype, tau=0.6)
+        w.faces = {W.FACE_YLO: W.BC_VELOCITY_INLET, W.FACE_YHI: W.BC_OUTLET_PRESSURE}
+        w.rho_out = {W.FACE_YHI: 1.01}
+        w.g = (1e-4, 0.0, 0.0)
+        w.inlet = W.Inlet(W.FACE_YLO, np.zeros((3, w.nz, w.nx), dtype=w.np_dtype), 0.0, 0, 0)
+        return w
+    for w in (jet_pressure((24, 17, 12), 61), jet_pressure((70, 30, 9), 62), neq_walls((66, 15, 7), 63)):
+        for k in kernels_for(B, w):
+            G, R, _ = run_both(oracle_mod, w, 5, k)
+            assert_parity(w, G, R, "%s kernel %d" % (w.name, k))
+            # boundary nodes themselves (get_moments refills them): imposed density / zero wall velocity, exactly
+            for f, rho in w.rho_out.items():
+                sl = [slice(None)] * 3
+                sl[2 - f // 2] = -1 if f % 2 else 0
+                assert np.abs(G[(0,) + tuple(sl)] - rho).max() <= (2e-7 if dtype == "f32" else 3e-16)   # one rounding of rho - 1
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_radial_statistics_match_oracle(B, oracle_mod, dtype):
     """(r, z)-bin sums of the jet (tslb_radial_statistics) against the oracle after a few steps of the jet boundary set:
     ring counts bit-exact (the ring index is an integer both sides decide in fp64), sums to 1e-12 relative in fp64 /
