@@ -200,12 +200,6 @@ __global__ void __launch_bounds__(128) sweep_gather_kernel(const T *__restrict__
 // One thread per (face, in-plane position); a node on several open faces is handled by the
 // lowest-index one.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint64_t mix64(uint64_t z)  // SplitMix64 finaliser (Vigna, public domain)
-{
-    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
-    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
-    return z ^ (z >> 31);
-}
 
 template <typename T>
 __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
@@ -252,23 +246,9 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
         const int a2 = (ax2 == 0) ? 1 : 0, b2 = (ax2 == 2) ? 1 : 2;
         const size_t pl = (size_t)n[a2] * n[b2];
         const size_t jj = (size_t)q[b2] * n[a2] + q[a2];
-        const uint64_t lin = ((uint64_t)q[2] * p.L.ny + q[1]) * p.L.nx + q[0];   // API linear index of the node
-        uint64_t k64 = mix64(p.inlet[f2].seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(p.t + 1)));
-        k64 = mix64(k64 + lin);
-        double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
-        if (p.inlet[f2].mask & TSLB_NOISE_GAUSSIAN) {   // Box-Muller on two uniforms of the same stream, fp64
-            const uint64_t k2 = mix64(k64);
-            const double u1 = ((double)(uint32_t)(k64 >> 40) + 1.0) / 16777216.0;
-            const double u2 = (double)(uint32_t)(k2 >> 40) / 16777216.0;
-            xi = sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
-        }
-        const T *up = (const T *)p.inlet[f2].u_plane;
+        const double xi = tslb_inlet_xi(p.inlet[f2], p.L, q[0], q[1], q[2], p.t);
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            double v = (double)up[k * pl + jj];
-            if (p.inlet[f2].mask & (1 << k)) v *= 1.0 + p.inlet[f2].noise_amp * xi;
-            M[(1 + k) * N + ib] = (T)v;
-        }
+        for (int k = 0; k < 3; ++k) M[(1 + k) * N + ib] = tslb_inlet_u<T>(p.inlet[f2], pl, jj, k, xi);
         break;
     }
 }

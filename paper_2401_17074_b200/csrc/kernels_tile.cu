@@ -149,6 +149,15 @@ struct TileParams {
     T beta, g[3];
     const T *beta_z;   // sponge layer (Eq. 26): 1 - omega of the nodes of plane z, [nz] (SPONGE instantiations only)
     int zchunk;  // planes per z chunk
+    int fuse;    // the store warp writes the open-face boundary nodes of time t+1 itself (FUSE instantiations)
+};
+// fused boundary fill (a6): what the store warp needs to impose inlet velocities / outlet densities
+struct FuseParams {
+    Layout L;
+    int kind[6];
+    long long tnext;           // step index the written boundary values belong to (noise counter)
+    InletDev inlet[6];
+    double rho_out[6];
 };
 
 // valid Hermite index: each <= 2, sum <= ORDER (3: Eq. 18, H3_aaa == 0 on this lattice; 2: the second-order TSLB of Eq. 8)
@@ -315,10 +324,43 @@ template <typename T> struct TileDims {
 static_assert(TileDims<float>::SMEM_BYTES <= 232448 && TileDims<double>::SMEM_BYTES <= 232448, "shared memory budget");
 static_assert(TileGeom<float>::WX == 2 && TileGeom<double>::WX == 2, "two warps per row pair publish; two halo warps");
 
-template <typename T, bool WALLY, int ORDER, bool SPONGE>
+// values imposed on the open-face boundary node (x, y, z) into its slot `a` of an output tile (field stride fs bytes):
+// lowest-index pressure face -> rho, lowest-index inlet face -> u (the rule of fill_boundary_kernel).  Out of line: it
+// is used from five places of the store warp and is not on the hot path.
+template <typename T>
+__device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32_t fs, int x, int y, int z)
+{
+    const Layout &L = p.L;
+    const int n3[3] = {L.nx, L.ny, L.nz};
+    const int q[3] = {x, y, z};
+    bool done = false;
+#pragma unroll
+    for (int f2 = 0; f2 < 6; ++f2) {
+        if (done || p.kind[f2] != TSLB_BC_OUTLET_PRESSURE) continue;
+        if (q[f2 >> 1] != ((f2 & 1) ? n3[f2 >> 1] - 1 : 0)) continue;
+        sts(a, (T)(p.rho_out[f2] - 1.0));
+        done = true;
+    }
+    done = false;
+#pragma unroll
+    for (int f2 = 0; f2 < 6; ++f2) {
+        if (done || p.kind[f2] != TSLB_BC_VELOCITY_INLET) continue;
+        const int ax2 = f2 >> 1;
+        if (q[ax2] != ((f2 & 1) ? n3[ax2] - 1 : 0)) continue;
+        const int a2 = (ax2 == 0) ? 1 : 0, b2 = (ax2 == 2) ? 1 : 2;
+        const size_t pl = (size_t)n3[a2] * n3[b2];
+        const size_t jj = (size_t)q[b2] * n3[a2] + q[a2];
+        const double xi = tslb_inlet_xi(p.inlet[f2], L, x, y, z, p.tnext);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) sts(a + (1 + k) * fs, tslb_inlet_u<T>(p.inlet[f2], pl, jj, k, xi));
+        done = true;
+    }
+}
+
+template <typename T, bool WALLY, int ORDER, bool SPONGE, bool FUSE>
 __global__ void __maxnreg__(TileDims<T>::MAXREG)
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
-                  const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p)
+                  const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p, const __grid_constant__ FuseParams fp)
 {
     typedef typename PackOf<T>::type P;
     typedef TileDims<T> TD;
@@ -382,6 +424,102 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         // stage has been released and a store the moment its tile is full, whatever the halo warps are doing: with the
         // producer inside a halo warp the load of plane i+1 could not be issued before plane i-1 had LANDED and been
         // processed there, which left the main warps waiting ~300 cycles per plane for their data.
+        if (FUSE && wid == TD::WARPS + 1) {
+            // ================================== store warp with the fused boundary fill (a6) ==================================
+            // Open faces (PAPER.md:181-196 Eq. 22-23, :202, :258): a boundary node of time t+1 takes the 10 moments of the
+            // interior node x_F its coordinates clamp to -- moments this very sweep produces -- and then the imposed velocity
+            // (inlet) or density (pressure outlet).  The whole warp patches the finished output tile in shared memory before
+            // the TMA store: boundary nodes on lateral faces copy from their x_F inside the tile; a boundary PLANE (z = 0 or
+            // nz-1) is the patched tile of its neighbour plane stored a second time, with the imposed values written over it.
+            // The host selects this path only when every boundary node shares a tile and a chunk with its x_F
+            // (tile_fusable), so no separate fill launch is needed between steps.  The main warps' own results for boundary
+            // nodes (nodes that are not advanced) are never stored.
+            auto open_k = [&](int f) { const int k = p.kind[f]; return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT || k == TSLB_BC_OUTLET_PRESSURE; };
+            const bool oxl = open_k(0), oxh = open_k(1), oyl = open_k(2), oyh = open_k(3), ozl = open_k(4), ozh = open_k(5);
+            // which boundary rows / columns this tile holds (tile coordinates, -1 = none)
+            const int bcol_lo = (oxl && x0 == 0) ? 0 : -1, bcol_hi = (oxh && x0 < L.nx && x0 + COLS >= L.nx) ? L.nx - 1 - x0 : -1;
+            const int brow_lo = (oyl && row0 == 0) ? 0 : -1, brow_hi = (oyh && row0 + ROWS >= L.ny) ? L.ny - 1 - row0 : -1;
+            const bool lateral = bcol_lo >= 0 || bcol_hi >= 0 || brow_lo >= 0 || brow_hi >= 0;
+            // does any lateral face impose a value (inlet velocity, outlet density)?  plain zero-gradient outlets only copy
+            auto imposes = [&](int f) { return p.kind[f] == TSLB_BC_VELOCITY_INLET || p.kind[f] == TSLB_BC_OUTLET_PRESSURE; };
+            const bool imp_lateral = imposes(0) || imposes(1) || imposes(2) || imposes(3);
+            auto impose = [&](uint32_t a, int x, int y, int z) { tile_impose<T>(fp, a, (uint32_t)(ROWS * COLS * ES), x, y, z); };
+            // one boundary node of a lateral face, tile coordinates (r, cx): copy the 10 moments of its x_F, impose
+            auto patch_node = [&](uint32_t tile, int r, int cx, int z) {
+                const int x = x0 + cx, y = row0 + r;
+                if (x >= L.nx) return;
+                int xf = x, yf = y;
+                if (x == 0 && oxl) xf = 1;
+                if (x == L.nx - 1 && oxh) xf = L.nx - 2;
+                if (y == 0 && oyl) yf = 1;
+                if (y == L.ny - 1 && oyh) yf = L.ny - 2;
+                const uint32_t src = tile + ((yf - row0) * COLS + (xf - x0)) * ES, dst = tile + (r * COLS + cx) * ES;
+                T v[TSLB_NF];
+#pragma unroll
+                for (int f = 0; f < TSLB_NF; ++f) v[f] = lds(src + f * (ROWS * COLS) * ES, T());
+#pragma unroll
+                for (int f = 0; f < TSLB_NF; ++f) sts(dst + f * (ROWS * COLS) * ES, v[f]);
+                if (imp_lateral) impose(dst, x, y, z);
+            };
+            int pending = -1;                                  // tile whose last store may still be reading it
+            for (int m = 0; m < nplanes - 2; ++m) {
+                const int b = m % NOUT, z = z0 + m;
+                const uint32_t tile = sb + TD::OFF_OUT + b * OUT_BYTES;
+                mbar_wait(sb + B_OFULL + 8 * b, (uint32_t)((m / NOUT) & 1));
+                const bool zplane = (z == 0 && ozl) || (z == L.nz - 1 && ozh);   // a boundary plane: not advanced
+                int groups = 0;
+                if (!zplane) {
+                    if (lateral) {
+                        // (a corner node is patched by its row and by its column, with the same values; x_F is never a
+                        //  boundary node, so the order of the copies does not matter)
+                        if (brow_lo >= 0) for (int cx = lane; cx < COLS; cx += 32) patch_node(tile, brow_lo, cx, z);
+                        if (brow_hi >= 0) for (int cx = lane; cx < COLS; cx += 32) patch_node(tile, brow_hi, cx, z);
+                        if (lane < ROWS) {
+                            if (bcol_lo >= 0) patch_node(tile, lane, bcol_lo, z);
+                            if (bcol_hi >= 0) patch_node(tile, lane, bcol_hi, z);
+                        }
+                        __syncwarp();
+                    }
+                    if (lane == 0) {
+                        fence_async_smem();
+                        tma_store_4d(tile, &tmStore, x0 + TSLB_XOFF, row0, z, 0);
+                        tma_store_commit();
+                    }
+                    ++groups;
+                    const int zb = (z == 1 && ozl) ? 0 : ((z == L.nz - 2 && ozh) ? L.nz - 1 : -1);
+                    if (zb >= 0) {                             // the boundary plane next to this one
+                        if (lane == 0) tma_store_wait_read();  // the store above has read the tile
+                        __syncwarp();
+                        if (imp_lateral || imposes(zb == 0 ? 4 : 5)) {
+                            for (int idx = lane; idx < ROWS * COLS; idx += 32) {
+                                const int r = idx / COLS, cx = idx - r * COLS, x = x0 + cx, y = row0 + r;
+                                if (x < L.nx) impose(tile + idx * ES, x, y, zb);
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) {
+                            fence_async_smem();
+                            tma_store_4d(tile, &tmStore, x0 + TSLB_XOFF, row0, zb, 0);
+                            tma_store_commit();
+                        }
+                        ++groups;
+                    }
+                }
+                if (lane == 0) {
+                    if (NOUT == 1 || groups != 1) {            // nothing or two groups from this tile: drain, hand back everything
+                        tma_store_wait_read();
+                        if (pending >= 0) mbar_arrive(sb + B_OEMPTY + 8 * pending);
+                        mbar_arrive(sb + B_OEMPTY + 8 * b);
+                    } else if (pending >= 0) {
+                        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                        mbar_arrive(sb + B_OEMPTY + 8 * pending);
+                    }
+                }
+                pending = (NOUT == 1 || groups != 1) ? -1 : b;
+            }
+            if (lane == 0) tma_store_wait_all();
+            return;
+        }
         if (lane != 0) return;
         if (wid == TD::WARPS) {
             const bool yper = p.kind[2] == TSLB_BC_PERIODIC, zper = p.kind[4] == TSLB_BC_PERIODIC;
@@ -894,6 +1032,28 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
     int zc = (c->nz + best - 1) / best;
     p.zchunk = zc;
     *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
+    // Fused boundary fill: possible when every open-face boundary node shares a tile and a z chunk with the interior node
+    // x_F it copies (the store warp patches the output tile in shared memory), the row tail and the periodic ghost
+    // columns -- stored from the main warps' registers, unpatched -- do not hold boundary values, and open axes are
+    // long enough for x_F to be an interior node.
+    auto open_k = [&](int f) {
+        const int k = c->kind[f];
+        return k == TSLB_BC_VELOCITY_INLET || k == TSLB_BC_OUTLET_ZERO_GRADIENT || k == TSLB_BC_OUTLET_PRESSURE;
+    };
+    bool any = false, ok = true;
+    for (int f = 0; f < 6; ++f) any = any || open_k(f);
+    const int n3[3] = {c->nx, c->ny, c->nz};
+    for (int ax = 0; ax < 3; ++ax)
+        if ((open_k(2 * ax) || open_k(2 * ax + 1)) && n3[ax] < 4) ok = false;
+    if (c->kind[0] == TSLB_BC_PERIODIC) ok = false;                               // ghost-column images of boundary rows
+    if (c->nx % (int)(16 / sizeof(T)) != 0) ok = false;                           // row tail stored from registers
+    if (open_k(1) && (c->nx - 1) % TileDims<T>::COLS == 0) ok = false;            // x = nx-1 alone in the last tile column
+    if (open_k(5) && c->nz - (int)(grid->z - 1) * zc < 2) ok = false;             // z = nz-1 alone in the last chunk
+    if (zc < 2) ok = false;
+#ifdef TILE_NO_FUSE
+    ok = false;
+#endif
+    p.fuse = (any && ok) ? 1 : 0;
     return p;
 }
 
@@ -967,8 +1127,10 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
     e = cudaSuccess;
 #define TSLB_SMEM_ATTR(T, W, O, B)                                                                                              \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
     TSLB_SMEM_ATTR(float, false, 3, smem32); TSLB_SMEM_ATTR(float, true, 3, smem32);
     TSLB_SMEM_ATTR(float, false, 2, smem32); TSLB_SMEM_ATTR(float, true, 2, smem32);
     TSLB_SMEM_ATTR(double, false, 3, smem64); TSLB_SMEM_ATTR(double, true, 3, smem64);
@@ -985,12 +1147,17 @@ static void launch_tile(tslb_ctx *c, cudaStream_t st)
     dim3 grid;
     TileParams<T> p = make_tile<T>(c, &grid);
     const int a = c->cur, b = 1 - c->cur;
-    if (p.beta_z)
-        sweep_tile_kernel<T, WALLY, ORDER, true><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],
-                                                                                                             c->tm_store[b], (T *)c->buf[b], p);
-    else
-        sweep_tile_kernel<T, WALLY, ORDER, false><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],
-                                                                                                              c->tm_store[b], (T *)c->buf[b], p);
+    c->last_fused = p.fuse;
+    FuseParams fp;
+    fp.L = c->L;
+    fp.tnext = c->t + 1;
+    for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
+#define TSLB_TILE_LAUNCH(S, F)                                                                                                            \
+    sweep_tile_kernel<T, WALLY, ORDER, S, F><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],       \
+                                                                                                         c->tm_store[b], (T *)c->buf[b], p, fp)
+    if (p.beta_z) { if (p.fuse) TSLB_TILE_LAUNCH(true, true); else TSLB_TILE_LAUNCH(true, false); }
+    else { if (p.fuse) TSLB_TILE_LAUNCH(false, true); else TSLB_TILE_LAUNCH(false, false); }
+#undef TSLB_TILE_LAUNCH
 }
 
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)

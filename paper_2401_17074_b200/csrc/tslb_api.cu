@@ -355,7 +355,9 @@ int tslb_step(tslb_ctx *c, int n, void *stream)
         if (e != cudaSuccess) return cuda_fail(c, "sweep kernel", e);
         c->cur = 1 - c->cur;                                               // step 5: AB flip-flop
         c->t += 1;
-        c->halo_valid = (k == TSLB_KERNEL_TILE) ? 3 : 0;   // 3: periodic ghost images written by the sweep, fill pending
+        // 3: periodic ghost images written by the sweep, fill pending; 2: the sweep also wrote the open-face boundary nodes
+        // of time t+1 (fused fill; x is not periodic there, so the ghost columns are not used)
+        c->halo_valid = (k == TSLB_KERNEL_TILE) ? (c->last_fused ? 2 : 3) : 0;
     }
     return TSLB_OK;
 }

@@ -55,6 +55,40 @@ struct FillParams {
     long long t;  // step index the fill belongs to (noise counter)
 };
 
+#ifdef __CUDACC__
+// ---- values imposed on open-face boundary nodes: shared by the boundary-fill kernel and by the store warp of the tile
+//      kernel (which writes the boundary nodes of time t+1 itself), so that both give the same bits ------------------------
+__device__ __forceinline__ uint64_t tslb_mix64(uint64_t z)  // SplitMix64 finaliser (Vigna, public domain)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+// noise variate of the inlet node (x, y, z) at step t (include/tslb.h, tslb_inlet_params; readings A14, A14b)
+__device__ __forceinline__ double tslb_inlet_xi(const InletDev &in, const Layout &L, int x, int y, int z, long long t)
+{
+    const uint64_t lin = ((uint64_t)z * L.ny + y) * L.nx + x;   // API linear index of the node
+    uint64_t k64 = tslb_mix64(in.seed ^ (0x9E3779B97F4A7C15ULL * (uint64_t)(t + 1)));
+    k64 = tslb_mix64(k64 + lin);
+    double xi = (double)(uint32_t)(k64 >> 40) / 8388608.0 - 1.0;  // exact: 24-bit integer
+    if (in.mask & TSLB_NOISE_GAUSSIAN) {   // Box-Muller on two uniforms of the same stream, fp64
+        const uint64_t k2 = tslb_mix64(k64);
+        const double u1 = ((double)(uint32_t)(k64 >> 40) + 1.0) / 16777216.0;
+        const double u2 = (double)(uint32_t)(k2 >> 40) / 16777216.0;
+        xi = sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
+    }
+    return xi;
+}
+// imposed velocity component k of an inlet node: u_in,k (1 + amp xi) on the masked components (fp64, rounded once)
+template <typename T>
+__device__ __forceinline__ T tslb_inlet_u(const InletDev &in, size_t plane_elems, size_t j, int k, double xi)
+{
+    double v = (double)((const T *)in.u_plane)[k * plane_elems + j];
+    if (in.mask & (1 << k)) v = __dmul_rn(v, __dadd_rn(1.0, __dmul_rn(in.noise_amp, xi)));
+    return (T)v;
+}
+#endif
+
 // geometry of the TMA-staged tile kernel (kernels_tile.cu): a warp owns 2 rows x 30 columns (+ 1 halo lane per side)
 #define TILE_COLS 30
 
@@ -75,6 +109,7 @@ struct tslb_ctx {
     void *beta_z;     // sponge layer: per-plane 1 - omega in the context dtype, [nz] (in the workspace)
     void *beta_z_host;   // the same on the host (staging for the upload), NULL = no sponge layer
     int sponge_dirty;    // the host table has to be uploaded before the next sweep
+    int last_fused;      // the last tile launch wrote the open-face boundary nodes of its output itself (fused fill)
     CUtensorMap tm_main[2], tm_row[2], tm_store[2];  // TMA descriptors of buf[0], buf[1]: tile rows, one halo row, output tile
     int tmap_ok;
     int cur;          // buf[cur] holds time t

@@ -253,6 +253,28 @@ def test_order2_config1_reduced(B, oracle_mod):
         assert_parity(w, G, R, "order 2 kernel %d" % k)
 
 
+def test_open_faces_are_filled_inside_the_sweep(B, oracle_mod):
+    """north_star: 'boundary and forcing kernels fused into the same sweep'.  On the jet boundary set the tile kernel's
+    store warp writes the boundary nodes of time t+1 itself: one launch per step once the first fill has run, and the
+    boundary nodes it wrote are exactly what the oracle's fill gives (inlet with noise, outlets, edges and corners)."""
+    w = W.jet(64, 48, 40, steps=6, D=12.0)
+    sim = make_gpu(w, TILE)
+    assert sim.active_kernel() == TILE
+    sim.step(1)
+    n0 = sim.launch_count
+    sim.step(5)
+    assert sim.launch_count - n0 == 5, "open faces cost extra launches: %d for 5 steps" % (sim.launch_count - n0)
+    G = gpu_state(sim)
+    o = make_oracle(oracle_mod, w); o.step(6)
+    R = o.get_moments()
+    assert_parity(w, G, R, "fused fill")
+    # boundary nodes (get_moments does not have to refill them: the sweep's own fill is current)
+    for ax, idx in ((1, 0), (1, -1), (2, 0), (2, -1), (3, 0), (3, -1)):
+        g = np.take(G, idx, axis=ax).astype(np.float64); r = np.take(R, idx, axis=ax)
+        assert np.abs(g[0] - r[0]).max() < 1e-6 and np.abs(g[1:4] - r[1:4]).max() < 1e-6 * max(1e-30, np.abs(R[1:4]).max()) + 1e-8
+    sim.close()
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_boundary_variants_of_section_IIC(B, oracle_mod, dtype):
     """pressure (density-imposed) outlet, NEQ no-slip walls (zero-velocity Dirichlet nodes on the
