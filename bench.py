@@ -86,7 +86,7 @@ class ClockSampler:
         except subprocess.TimeoutExpired:
             self.proc.kill()
         self.thr.join(timeout=5)
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for l in self.lines:
             p = [x.strip() for x in l.split(",")]
@@ -94,6 +94,10 @@ class ClockSampler:
                 continue
             try:
                 sm.append(float(p[0])); mx.append(float(p[1]))
+                try:
+                    pw.append(float(p[2]))
+                except ValueError:
+                    pass
             except ValueError:
                 continue
             for nme, v in zip(names, p[3:7]):
@@ -102,7 +106,8 @@ class ClockSampler:
         if not sm:
             return None
         sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "samples": len(sm), "reasons": sorted(reasons)}
+        return {"sm_mhz": sm[len(sm) // 2], "sm_min_mhz": sm[0], "sm_max_mhz": max(mx), "power_w_max": max(pw) if pw else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
 
 
 # ------------------------------------------------------------------------------------------------

@@ -106,10 +106,11 @@ def taylor_green_2d(n: int = 32, nz: int = 4, tau: float = 0.8, U0: float = 0.01
     return Workload("tg2d_%d" % n, n, n, nz, "f64", tau, steps, M)
 
 
-def config1(n: int = 128, steps: int = 1000, dtype: str = "f32") -> Workload:
-    """configs[1]: fp32 periodic cube, TG U0 = 0.02 + uniform(+-1e-3) noise (seed 1), tau = 0.5 + 3e-5."""
+def config1(n: int = 128, steps: int = 1000, dtype: str = "f32", U0: float = 0.02) -> Workload:
+    """configs[1]: fp32 periodic cube, TG U0 = 0.02 + uniform(+-1e-3) noise (seed 1), tau = 0.5 + 3e-5.
+    (U0 is an argument for the stability-margin scan of tests/test_gpu_stability.py.)"""
     M = _empty_moments(n, n, n)
-    _taylor_green(M, 0.02)
+    _taylor_green(M, U0)
     _add_uniform_noise(M, 1e-3, seed=1)
     return Workload("cfg1_tgnoise%d_%s" % (n, dtype), n, n, n, dtype, 0.5 + 3e-5, steps,
                     M.astype(_NP_DTYPE[dtype]))
