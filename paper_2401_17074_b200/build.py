@@ -16,7 +16,7 @@ LIB = os.path.join(HERE, "libtslb.so")
 SOURCES = ["tslb_api.cu", "kernels_basic.cu", "kernels_tile.cu"]
 HEADERS = [os.path.join(CSRC, "tslb_internal.h"), os.path.join(HERE, "..", "include", "tslb.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "4"]
 
 
 def _nvcc() -> str:

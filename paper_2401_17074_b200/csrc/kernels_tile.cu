@@ -249,12 +249,22 @@ __host__ __device__ constexpr int qidx(int kx, int kz) { return kz * 3 + kx; }
 // lock-step, which keeps the halo re-reads of neighbouring tiles inside L2).  TMA needs the byte offset of a box origin
 // along x to be a multiple of 16 (measured on B200: an origin at a multiple of 2 floats raises "illegal instruction"):
 // the source box starts XPAD = 4 columns left of the tile (the layout puts node x = 0 on a 16-byte boundary).
-template <typename T> struct TileGeom;
+// Geometry index G: 0 = the large tile (one CTA per SM), 1 = the small tile for lattices that cannot fill 148 large CTAs
+// (fp32 only: 60 columns x 4 rows, 4 main warps + the 4 helpers, two CTAs per SM).
+template <typename T, int G> struct TileGeom;
 #ifndef TILE_F32_WY
 #define TILE_F32_WY 6
 #endif
 #ifndef TILE_F32_NS
 #define TILE_F32_NS 2
+#endif
+// duration of one plane of a small-geometry CTA relative to a large one (measured, profiles/README.md)
+#ifndef TILE_SMALL_PLANE
+#define TILE_SMALL_PLANE 0.8
+#endif
+// -1: choose the geometry by estimated cost; 0 / 1: force it (experiments)
+#ifndef TILE_FORCE_GEOM
+#define TILE_FORCE_GEOM -1
 #endif
 #ifndef TILE_ZC_MAX
 #define TILE_ZC_MAX 64
@@ -278,26 +288,30 @@ template <typename T> struct TileGeom;
 #define TILE_F32_RH 80
 #define TILE_F32_NIDLE 2
 #endif
-template <> struct TileGeom<float> {
+template <> struct TileGeom<float, 0> {
     static constexpr int WX = 2, WY = TILE_F32_WY, NS = TILE_F32_NS, NIDLE = TILE_F32_NIDLE, REG_MAIN = TILE_F32_RM, REG_HALO = TILE_F32_RH;
-    static constexpr int NOUT = TILE_F32_NOUT;
+    static constexpr int NOUT = TILE_F32_NOUT, CTAS = 1;
+};
+template <> struct TileGeom<float, 1> {
+    static constexpr int WX = 2, WY = 2, NS = 2, NIDLE = 2, REG_MAIN = 144, REG_HALO = 80, NOUT = 2, CTAS = 2;
 };
 #ifndef TILE_F64_RM
 #define TILE_F64_RM 208
 #define TILE_F64_RH 80
 #endif
-template <> struct TileGeom<double> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = TILE_F64_RM, REG_HALO = TILE_F64_RH, NOUT = 1; };
+template <> struct TileGeom<double, 0> { static constexpr int WX = 2, WY = 4, NS = 2, NIDLE = 2, REG_MAIN = TILE_F64_RM, REG_HALO = TILE_F64_RH, NOUT = 1, CTAS = 1; };
+template <> struct TileGeom<double, 1> : TileGeom<double, 0> {};     // fp64 has the large geometry only
 constexpr int rup128(int bytes) { return (bytes + 127) / 128 * 128; }
-template <typename T> struct TileDims {
-    typedef TileGeom<T> G;
+template <typename T, int GI = 0> struct TileDims {
+    typedef TileGeom<T, GI> G;
     static constexpr int WX = G::WX, WY = G::WY, NS = G::NS;
     static constexpr int NMAIN = WX * WY, NHALO = 2, WARPS = NMAIN + NHALO, THREADS = (WARPS + G::NIDLE) * 32;
-    // one CTA per SM: the whole register file, 16384 registers per SM sub-partition, warps dealt round-robin to the four
-    static constexpr int MAXREG = (16384 / (((WARPS + G::NIDLE + 3) / 4) * 32)) / 8 * 8;     // at launch: 128 (fp32, 16 warps), 168 (fp64, 12 warps)
+    // CTAS CTAs per SM share the register file: 16384 registers per SM sub-partition, warps dealt round-robin to the four
+    static constexpr int MAXREG = (16384 / (((WARPS + G::NIDLE + 3) / 4) * 32 * G::CTAS)) / 8 * 8;   // at launch: 128 (fp32), 168 (fp64, 12 warps)
     static_assert(G::REG_MAIN == 0 || (NMAIN % 4 == 0 && (NHALO + G::NIDLE) % 4 == 0), "setmaxnreg works on warpgroups of 4 warps");
     static_assert(G::REG_MAIN % 16 == 0 && G::REG_HALO % 16 == 0, "a warp's registers are allocated in units of 512");
     static_assert(G::REG_MAIN == 0 || NMAIN * G::REG_MAIN + (NHALO + G::NIDLE) * G::REG_HALO <= (WARPS + G::NIDLE) * MAXREG, "setmaxnreg pool = launch allocation");
-    static_assert(G::REG_MAIN == 0 || (NMAIN / 4) * G::REG_MAIN + ((NHALO + G::NIDLE) / 4) * G::REG_HALO <= 512, "16384 registers per sub-partition");
+    static_assert(G::REG_MAIN == 0 || (NMAIN / 4) * G::REG_MAIN + ((NHALO + G::NIDLE) / 4) * G::REG_HALO <= 512 / G::CTAS, "16384 registers per sub-partition");
     static constexpr int COLS = TILE_COLS * WX;                  // output columns per CTA (60)
     static constexpr int ROWS = 2 * WY;                          // output rows per CTA
     static constexpr int XPAD = 4;                               // box origin = first tile column - XPAD
@@ -322,7 +336,8 @@ template <typename T> struct TileDims {
     static constexpr int SMEM_BYTES = OFF_BAR + NBAR * 8;
 };
 static_assert(TileDims<float>::SMEM_BYTES <= 232448 && TileDims<double>::SMEM_BYTES <= 232448, "shared memory budget");
-static_assert(TileGeom<float>::WX == 2 && TileGeom<double>::WX == 2, "two warps per row pair publish; two halo warps");
+static_assert(2 * (TileDims<float, 1>::SMEM_BYTES + 1024) <= 233472, "two small CTAs per SM");
+static_assert(TileGeom<float, 0>::WX == 2 && TileGeom<float, 1>::WX == 2 && TileGeom<double, 0>::WX == 2, "two warps per row pair publish; two halo warps");
 
 // values imposed on the open-face boundary node (x, y, z) into its slot `a` of an output tile (field stride fs bytes):
 // lowest-index pressure face -> rho, lowest-index inlet face -> u (the rule of fill_boundary_kernel).  Out of line: it
@@ -357,13 +372,13 @@ __device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32
     }
 }
 
-template <typename T, bool WALLY, int ORDER, bool SPONGE, bool FUSE>
-__global__ void __maxnreg__(TileDims<T>::MAXREG)
+template <typename T, bool WALLY, int ORDER, bool SPONGE, bool FUSE, int GEO>
+__global__ void __maxnreg__((TileDims<T, GEO>::MAXREG))
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
                   const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p, const __grid_constant__ FuseParams fp)
 {
     typedef typename PackOf<T>::type P;
-    typedef TileDims<T> TD;
+    typedef TileDims<T, GEO> TD;
     constexpr int NS = TD::NS, BXW = TD::BXW, FS = TD::FS, ROWS = TD::ROWS, COLS = TD::COLS, WY = TD::WY, WX = TD::WX;
     constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
     constexpr int ES = (int)sizeof(T);
@@ -413,11 +428,12 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     }
     __syncthreads();
 
-    if (TileGeom<T>::REG_MAIN != 0) {
-        if (wid >= TD::NMAIN) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_HALO ? TileGeom<T>::REG_HALO : 24));
-        else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(TileGeom<T>::REG_MAIN ? TileGeom<T>::REG_MAIN : 24));
+    typedef TileGeom<T, GEO> GE;
+    if (GE::REG_MAIN != 0) {
+        if (wid >= TD::NMAIN) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(GE::REG_HALO ? GE::REG_HALO : 24));
+        else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(GE::REG_MAIN ? GE::REG_MAIN : 24));
     }
-    static_assert(TileGeom<T>::NIDLE == 2, "the two warps that complete the helpers' warpgroup are the producer and the store warp");
+    static_assert(GE::NIDLE == 2, "the two warps that complete the helpers' warpgroup are the producer and the store warp");
     if (wid >= TD::WARPS) {
         // ============================================ producer warp / store warp ==========================================
         // One lane each.  They are warps of their own (not lanes of the halo warps) so that a load is issued the moment its
@@ -1000,17 +1016,20 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     }
 }
 
-template <typename T>
-TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
+// Launch geometry for tile geometry GEO.  *cost = estimated duration in units of one plane of a LARGE CTA (for the choice
+// between the geometries), or a huge value if the lattice has fewer rows than one tile.
+template <typename T, int GEO>
+TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
 {
+    typedef TileDims<T, GEO> TDH;
     TileParams<T> p;
     p.L = c->L;
     for (int f = 0; f < 6; ++f) p.kind[f] = c->kind[f];
     p.beta = (T)(1.0 - c->omega);
     p.beta_z = c->beta_z_host ? (const T *)c->beta_z : nullptr;
     for (int a = 0; a < 3; ++a) p.g[a] = (T)c->g[a];
-    const int gx = (c->nx + TileDims<T>::COLS - 1) / TileDims<T>::COLS;
-    const int gy = (c->ny + TileDims<T>::ROWS - 1) / TileDims<T>::ROWS;
+    const int gx = (c->nx + TDH::COLS - 1) / TDH::COLS;
+    const int gy = (c->ny + TDH::ROWS - 1) / TDH::ROWS;
     // z chunks (one CTA per SM is resident): pick the chunk count whose number of waves x (chunk length + 2 halo planes +
     // ring fill) is smallest, among chunks of at most TILE_ZC_MAX planes.  Long marches let the CTAs of a wave drift apart
     // in z until the halo rows / columns that neighbouring tiles share have left L2 before their second reader arrives
@@ -1024,11 +1043,13 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
         if (k > 1 && zc < 8) break;
         if (zc > TILE_ZC_MAX && (c->nz + k) / (k + 1) >= 8) continue;
         const long long ctas = cols * ((c->nz + zc - 1) / zc);
-        const long long slots = (long long)c->sm_count;
+        const long long slots = (long long)c->sm_count * TDH::G::CTAS;
         const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
         if (cost < best_cost) { best_cost = cost; best = k; }
     }
+    // a plane of a small CTA (4 rows, two CTAs per SM) takes about TILE_SMALL_PLANE of a large one's (12 rows)
+    if (cost_out) *cost_out = (c->ny < TDH::ROWS) ? 1e300 : best_cost * (GEO == 1 ? TILE_SMALL_PLANE : 1.0);
     int zc = (c->nz + best - 1) / best;
     p.zchunk = zc;
     *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
@@ -1047,7 +1068,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid)
         if ((open_k(2 * ax) || open_k(2 * ax + 1)) && n3[ax] < 4) ok = false;
     if (c->kind[0] == TSLB_BC_PERIODIC) ok = false;                               // ghost-column images of boundary rows
     if (c->nx % (int)(16 / sizeof(T)) != 0) ok = false;                           // row tail stored from registers
-    if (open_k(1) && (c->nx - 1) % TileDims<T>::COLS == 0) ok = false;            // x = nx-1 alone in the last tile column
+    if (open_k(1) && (c->nx - 1) % TDH::COLS == 0) ok = false;            // x = nx-1 alone in the last tile column
     if (open_k(5) && c->nz - (int)(grid->z - 1) * zc < 2) ok = false;             // z = nz-1 alone in the last chunk
     if (zc < 2) ok = false;
 #ifdef TILE_NO_FUSE
@@ -1075,7 +1096,7 @@ bool tslb_tile_supported(const tslb_ctx *c, const char **why)
             return false;
         }
     // every tile is full: the last tile of the y axis is shifted back, which needs at least one tile height of rows
-    if (c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float>::ROWS)) {
+    if (c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 1>::ROWS)) {
         if (why) *why = "fewer rows (ny) than one tile";
         return false;
     }
@@ -1105,47 +1126,52 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     const size_t es = tslb_elem(c);
     const bool f64 = c->dtype == TSLB_F64;
     const cuuint32_t bxw = f64 ? TileDims<double>::BXW : TileDims<float>::BXW;
-    const cuuint32_t rows = f64 ? TileDims<double>::ROWS : TileDims<float>::ROWS;
+    const cuuint32_t rows_g[2] = {(cuuint32_t)(f64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS),
+                                  (cuuint32_t)(f64 ? TileDims<double>::ROWS : TileDims<float, 1>::ROWS)};
     const cuuint32_t cols = f64 ? TileDims<double>::COLS : TileDims<float>::COLS;
+    static_assert(TileDims<float, 0>::BXW == TileDims<float, 1>::BXW && TileDims<float, 0>::COLS == TileDims<float, 1>::COLS, "same tile width");
     const cuuint64_t strides[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.field * es};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUtensorMapDataType dt = f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    for (int g = 0; g < 2; ++g)
     for (int b = 0; b < 2; ++b) {
+        const cuuint32_t rows = rows_g[g];
         const cuuint64_t dims_ld[4] = {(cuuint64_t)L.px, (cuuint64_t)L.ny, (cuuint64_t)L.nz, TSLB_NF};
         const cuuint64_t dims_st[4] = {(cuuint64_t)((L.nx & ~(int)(16 / es - 1)) + TSLB_XOFF), (cuuint64_t)L.ny, (cuuint64_t)L.nz, TSLB_NF};
         const cuuint32_t box_main[4] = {bxw, rows, 1, TSLB_NF}, box_row[4] = {bxw, 1, 1, TSLB_NF}, box_st[4] = {cols, rows, 1, TSLB_NF};
-        CUresult r = ((EncodeTiledFn)fn)(&c->tm_main[b], dt, 4, c->buf[b], dims_ld, strides, box_main, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        CUresult r = ((EncodeTiledFn)fn)(&c->tm_main[g][b], dt, 4, c->buf[b], dims_ld, strides, box_main, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                          CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r == CUDA_SUCCESS)
-            r = ((EncodeTiledFn)fn)(&c->tm_row[b], dt, 4, c->buf[b], dims_ld, strides, box_row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            r = ((EncodeTiledFn)fn)(&c->tm_row[g][b], dt, 4, c->buf[b], dims_ld, strides, box_row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                     CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r == CUDA_SUCCESS)
-            r = ((EncodeTiledFn)fn)(&c->tm_store[b], dt, 4, c->buf[b], dims_st, strides, box_st, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            r = ((EncodeTiledFn)fn)(&c->tm_store[g][b], dt, 4, c->buf[b], dims_st, strides, box_st, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
-    const int smem32 = TileDims<float>::SMEM_BYTES, smem64 = TileDims<double>::SMEM_BYTES;
     e = cudaSuccess;
-#define TSLB_SMEM_ATTR(T, W, O, B)                                                                                              \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, B);  \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B);  \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
-    TSLB_SMEM_ATTR(float, false, 3, smem32); TSLB_SMEM_ATTR(float, true, 3, smem32);
-    TSLB_SMEM_ATTR(float, false, 2, smem32); TSLB_SMEM_ATTR(float, true, 2, smem32);
-    TSLB_SMEM_ATTR(double, false, 3, smem64); TSLB_SMEM_ATTR(double, true, 3, smem64);
-    TSLB_SMEM_ATTR(double, false, 2, smem64); TSLB_SMEM_ATTR(double, true, 2, smem64);
+#define TSLB_SMEM_ATTR(T, W, O, G)                                                                                              \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES)
+    TSLB_SMEM_ATTR(float, false, 3, 0); TSLB_SMEM_ATTR(float, true, 3, 0);
+    TSLB_SMEM_ATTR(float, false, 2, 0); TSLB_SMEM_ATTR(float, true, 2, 0);
+    TSLB_SMEM_ATTR(float, false, 3, 1); TSLB_SMEM_ATTR(float, true, 3, 1);
+    TSLB_SMEM_ATTR(float, false, 2, 1); TSLB_SMEM_ATTR(float, true, 2, 1);
+    TSLB_SMEM_ATTR(double, false, 3, 0); TSLB_SMEM_ATTR(double, true, 3, 0);
+    TSLB_SMEM_ATTR(double, false, 2, 0); TSLB_SMEM_ATTR(double, true, 2, 0);
 #undef TSLB_SMEM_ATTR
     if (e != cudaSuccess) return e;
     c->tmap_ok = 1;
     return cudaSuccess;
 }
 
-template <typename T, bool WALLY, int ORDER>
-static void launch_tile(tslb_ctx *c, cudaStream_t st)
+template <typename T, bool WALLY, int ORDER, int GEO>
+static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 {
     dim3 grid;
-    TileParams<T> p = make_tile<T>(c, &grid);
+    TileParams<T> p = make_tile<T, GEO>(c, &grid, nullptr);
     const int a = c->cur, b = 1 - c->cur;
     c->last_fused = p.fuse;
     FuseParams fp;
@@ -1153,11 +1179,27 @@ static void launch_tile(tslb_ctx *c, cudaStream_t st)
     fp.tnext = c->t + 1;
     for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
 #define TSLB_TILE_LAUNCH(S, F)                                                                                                            \
-    sweep_tile_kernel<T, WALLY, ORDER, S, F><<<grid, TileDims<T>::THREADS, TileDims<T>::SMEM_BYTES, st>>>(c->tm_main[a], c->tm_row[a],       \
-                                                                                                         c->tm_store[b], (T *)c->buf[b], p, fp)
+    sweep_tile_kernel<T, WALLY, ORDER, S, F, GEO><<<grid, TileDims<T, GEO>::THREADS, TileDims<T, GEO>::SMEM_BYTES, st>>>(                    \
+        c->tm_main[GEO][a], c->tm_row[GEO][a], c->tm_store[GEO][b], (T *)c->buf[b], p, fp)
     if (p.beta_z) { if (p.fuse) TSLB_TILE_LAUNCH(true, true); else TSLB_TILE_LAUNCH(true, false); }
     else { if (p.fuse) TSLB_TILE_LAUNCH(false, true); else TSLB_TILE_LAUNCH(false, false); }
 #undef TSLB_TILE_LAUNCH
+}
+
+// fp32 has two tile geometries: the one with the smaller estimated duration is taken (a lattice that cannot fill 148
+// large CTAs, or whose width / height the large tile pads badly, runs on the small one)
+template <typename T, bool WALLY, int ORDER>
+static void launch_tile(tslb_ctx *c, cudaStream_t st)
+{
+    if (sizeof(T) == 8) { launch_tile_geo<T, WALLY, ORDER, 0>(c, st); return; }
+    dim3 g0, g1;
+    double c0 = 0, c1 = 0;
+    make_tile<T, 0>(c, &g0, &c0);
+    make_tile<T, 1>(c, &g1, &c1);
+    int geo = c1 < c0 ? 1 : 0;
+    if (TILE_FORCE_GEOM >= 0 && (TILE_FORCE_GEOM == 1 ? c1 : c0) < 1e299) geo = TILE_FORCE_GEOM;
+    if (geo == 1) launch_tile_geo<T, WALLY, ORDER, 1>(c, st);
+    else launch_tile_geo<T, WALLY, ORDER, 0>(c, st);
 }
 
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)

@@ -110,7 +110,7 @@ struct tslb_ctx {
     void *beta_z_host;   // the same on the host (staging for the upload), NULL = no sponge layer
     int sponge_dirty;    // the host table has to be uploaded before the next sweep
     int last_fused;      // the last tile launch wrote the open-face boundary nodes of its output itself (fused fill)
-    CUtensorMap tm_main[2], tm_row[2], tm_store[2];  // TMA descriptors of buf[0], buf[1]: tile rows, one halo row, output tile
+    CUtensorMap tm_main[2][2], tm_row[2][2], tm_store[2][2];  // TMA descriptors [tile geometry][buffer]: tile rows, one halo row, output tile
     int tmap_ok;
     int cur;          // buf[cur] holds time t
     long long t;
