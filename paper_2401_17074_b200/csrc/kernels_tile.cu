@@ -395,13 +395,15 @@ __device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32
     }
 }
 
-template <typename T, bool WALLY, int ORDER, bool SPONGE, bool FUSE, int GEO>
+// WALL: 0 = no bounce-back wall, 1 = walls on y faces, 2 = walls on z faces (walls on two axes, or on x: gather kernel)
+template <typename T, int WALL, int ORDER, bool SPONGE, bool FUSE, int GEO>
 __global__ void __maxnreg__((TileDims<T, GEO>::MAXREG))
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
                   const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p, const __grid_constant__ FuseParams fp)
 {
     typedef typename PackOf<T>::type P;
     typedef TileDims<T, GEO> TD;
+    constexpr bool WALLY = WALL == 1, WALLZ = WALL == 2;
     constexpr int NS = TD::NS, BXW = TD::BXW, FS = TD::FS, ROWS = TD::ROWS, COLS = TD::COLS, WY = TD::WY, WX = TD::WX;
     constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
     constexpr int ES = (int)sizeof(T);
@@ -571,9 +573,11 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             const int ylo = row0 > 0 ? row0 - 1 : (yper ? L.ny - 1 : -1);
             const int yhi = row0 + ROWS < L.ny ? row0 + ROWS : (yper ? 0 : L.ny);
             for (int j = 0; j < nplanes; ++j) {            // source plane z0-1+j into stage j % NS
+                // (beyond a z wall the plane NEXT to the wall is loaded once more: its own coefficients give the bounced
+                //  populations, see "halfway bounce-back on a z face" in the main warps)
                 int zs = z0 - 1 + j;
-                if (zs < 0) zs = zper ? L.nz - 1 : -1;
-                else if (zs >= L.nz) zs = zper ? 0 : L.nz;
+                if (zs < 0) zs = zper ? L.nz - 1 : ((WALLZ && p.kind[4] == TSLB_BC_BOUNCE_BACK) ? 0 : -1);
+                else if (zs >= L.nz) zs = zper ? 0 : ((WALLZ && p.kind[5] == TSLB_BC_BOUNCE_BACK) ? L.nz - 1 : L.nz);
                 const int s = j % NS;
                 if (j >= NS) mbar_wait(sb + B_EMPTY + 8 * s, (uint32_t)((j / NS - 1) & 1));
                 const uint32_t dst = sb + s * STAGE_BYTES, bar = sb + B_FULL + 8 * s;
@@ -786,6 +790,20 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         // ---- a2: Hermite coefficients of the own rows, all three rounds; y-pass combinations of the 8 groups -------------
         // For the output pack: up = (P(r0-1), P(r0)), dn = (M(r0+1), M(r0+2)); P(r0-1) and M(r0+2) are read from the neighbours,
         // P(r0) = qP0 and M(r0+1) = qM1 are the pack's own:  E = up + dn,  O = up - dn,  G0 = E + cen.
+        // ---- halfway bounce-back on a z face: the source "plane" beyond the wall (zs = -1 / nz) holds the moments of the
+        //      wall-adjacent plane once more (producer).  What that plane would send across the wall -- Vp(-1) into plane 0,
+        //      Vm(nz) into plane nz-1 -- is replaced by the bounced populations f*_ibar of the nodes themselves: with
+        //      Bz(kx,ky) = sum_kz t_kz(-c_z) A(kx,ky,kz) (M combination below, P above) and the local sums L(0,0) = 6,
+        //      L(1,1) = -2, L(2,0) = L(2,2) = 2 over x and y,
+        //        V(0,0) = 36 Bz00, V(1,0) = -12 Bz10, V(2,0) = 12 (Bz00 + Bz20), V(0,1) = -12 Bz01, V(1,1) = 4 Bz11,
+        //        V(0,2) = 12 (Bz00 + Bz02);
+        //      the z march then applies c_z^pz by itself.  The y / x passes of such a plane are skipped (CTA-uniform). ----------
+        const int zsrc_raw = z0 - 1 + i;
+        const bool wsrc_lo = WALLZ && zsrc_raw < 0 && p.kind[4] == TSLB_BC_BOUNCE_BACK;
+        const bool wsrc_hi = WALLZ && zsrc_raw >= L.nz && p.kind[5] == TSLB_BC_BOUNCE_BACK;
+        const bool wsrc = wsrc_lo || wsrc_hi;
+        P Bz[6];                                          // (kx,ky) = 00, 10, 20, 01, 11, 02
+        const T sz = wsrc_lo ? (T)-1 : (T)1;
         T qP0[NGRP], qM1[NGRP];
         P cen[NGRP];
         {
@@ -798,10 +816,20 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                 sts(w + q * EXW * ES, m0);                                                        \
                 sts(w + OWN_Y + q * EXW * ES, p1);                                                \
             }
+#define TSLB_BZ(G, KX, KY, KZ)                                                                    \
+            if (kvalid<ORDER>(KX, KY, KZ)) {                                                      \
+                if (KZ == 0) Bz[G] = A[KX][KY];                                                   \
+                else if (KZ == 1) Bz[G] = pfmas(A[KX][KY], sz, Bz[G]);                            \
+                else Bz[G] = padd(Bz[G], A[KX][KY]);                                              \
+            }
 #define TSLB_MAIN_ROUND(KZ)                                                                       \
             {                                                                                     \
                 P A[3][3];                                                                        \
                 hermite_round<KZ, P, T>(rc, bz, p.g, A);                                          \
+                if (WALLZ && wsrc) {                                                              \
+                    TSLB_BZ(0, 0, 0, KZ) TSLB_BZ(1, 1, 0, KZ) TSLB_BZ(2, 2, 0, KZ)                \
+                    TSLB_BZ(3, 0, 1, KZ) TSLB_BZ(4, 1, 1, KZ) TSLB_BZ(5, 0, 2, KZ)                \
+                }                                                                                 \
                 TSLB_MAIN_GROUP(0, KZ) TSLB_MAIN_GROUP(1, KZ) TSLB_MAIN_GROUP(2, KZ)              \
             }
             TSLB_MAIN_ROUND(0)
@@ -809,6 +837,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             TSLB_MAIN_ROUND(2)
 #undef TSLB_MAIN_ROUND
 #undef TSLB_MAIN_GROUP
+#undef TSLB_BZ
         }
         if (GE::QFLAGS) flag_set(bQown, (uint32_t)(i + 1), lane);
         else warp_arrive(bQown + 8 * PAR, lane);
@@ -835,8 +864,10 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         P Lz[3], Dz[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            ucur[a] = rc[1 + a];
-            const P dc = psub(rc[1 + a], uprev[a]);      // u(zs) - u(zs-1)
+            // (a plane beyond a z wall enters the differences with u = 0, like the ghost rows of a y wall)
+            const P uz = (WALLZ && wsrc) ? pbc<P, T>((T)0) : rc[1 + a];
+            ucur[a] = uz;
+            const P dc = psub(uz, uprev[a]);             // u(zs) - u(zs-1)
             Lz[a] = psub(dc, dprev[a]);
             Dz[a] = padd(dprev[a], dc);                  // u(zs) - u(zs-2) = -(D along z); used with negated multipliers
             dcur[a] = dc;
@@ -870,6 +901,26 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         //   vp0[g]  = Vp(zs)
         // with Vp = phi0 + phi1 + phi2, Vm = phi0 - phi1 + phi2, centre = 4 phi0 - 2 phi2 over kz.
         P vm0[6];
+        if (WALLZ && wsrc) {
+            // full first-order coefficients (the passes carry them without their base 3 u)
+            const P b00 = pfmas(rc[3], (T)3 * sz, Bz[0]);
+            const P b10 = pfmas(rc[1], (T)3, Bz[1]);
+            const P b01 = pfmas(rc[2], (T)3, Bz[3]);
+            P V[6];
+            V[0] = pmuls(b00, (T)36);
+            V[1] = pmuls(b10, (T)-12);
+            V[2] = pmuls(padd(b00, Bz[2]), (T)12);
+            V[3] = pmuls(b01, (T)-12);
+            V[4] = kvalid<ORDER>(1, 1, 0) ? pmuls(Bz[4], (T)4) : pbc<P, T>((T)0);
+            V[5] = pmuls(padd(b00, Bz[5]), (T)12);
+#pragma unroll
+            for (int g = 0; g < 6; ++g) {
+                const bool alone = g == 0 || g == 1 || g == 3;
+                if (wsrc_lo) { vp0[g] = V[g]; tn[g] = pbc<P, T>((T)0); if (alone) vm0[g] = pbc<P, T>((T)0); }   // Vp(-1) into plane 0
+                else if (alone) vm0[g] = V[g];                                                              // Vm(nz) into plane nz-1
+                else tt1[g] = padd(tt1[g], V[g]);
+            }
+        } else
 #pragma unroll
         for (int kz = 0; kz < 3; ++kz) {
             // ---- y pass: G1[py][kx] = sum_ky T^y_{py,ky} A(kx,ky,kz) at rows r0, r0+1 ---------------------------------------
@@ -1117,6 +1168,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
     if (open_k(1) && (c->nx - 1) % TDH::COLS == 0) ok = false;            // x = nx-1 alone in the last tile column
     if (open_k(5) && c->nz - (int)(grid->z - 1) * zc < 2) ok = false;             // z = nz-1 alone in the last chunk
     if (zc < 2) ok = false;
+    if (c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK) ok = false;   // z-wall kernels: plain store warp only
 #ifdef TILE_NO_FUSE
     ok = false;
 #endif
@@ -1135,12 +1187,19 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 bool tslb_tile_supported(const tslb_ctx *c, const char **why)
 {
-    // bounce-back walls are handled on the y faces only (x or z walls: gather kernel)
+    // bounce-back walls are handled on the y faces or on the z faces (walls on x, or on two axes: gather kernel); the z-wall
+    // instantiations exist for the plain case only (no sponge layer)
+    bool wall_ax[3] = {false, false, false};
     for (int f = 0; f < 6; ++f)
-        if (c->kind[f] == TSLB_BC_BOUNCE_BACK && (f >> 1) != 1) {
-            if (why) *why = "bounce-back walls on x or z faces";
-            return false;
-        }
+        if (c->kind[f] == TSLB_BC_BOUNCE_BACK) wall_ax[f >> 1] = true;
+    if (wall_ax[0] || (wall_ax[1] && wall_ax[2])) {
+        if (why) *why = "bounce-back walls on x faces or on two axes";
+        return false;
+    }
+    if (wall_ax[2] && (c->beta_z_host || c->nz < 4 || c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS))) {
+        if (why) *why = "z walls together with a sponge layer, or fewer rows than one large tile";
+        return false;
+    }
     // every tile is full: the last tile of the y axis is shifted back, which needs at least one tile height of rows
     if (c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 1>::ROWS)) {
         if (why) *why = "fewer rows (ny) than one tile";
@@ -1196,24 +1255,28 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
     e = cudaSuccess;
+#define TSLB_SMEM_ATTR_Z(T, O)                                                                                                  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 2, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES)
+    TSLB_SMEM_ATTR_Z(float, 3); TSLB_SMEM_ATTR_Z(float, 2); TSLB_SMEM_ATTR_Z(double, 3); TSLB_SMEM_ATTR_Z(double, 2);
+#undef TSLB_SMEM_ATTR_Z
 #define TSLB_SMEM_ATTR(T, W, O, G)                                                                                              \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES); \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES);  \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, false, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES);  \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, W, O, true, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, G>::SMEM_BYTES)
-    TSLB_SMEM_ATTR(float, false, 3, 0); TSLB_SMEM_ATTR(float, true, 3, 0);
-    TSLB_SMEM_ATTR(float, false, 2, 0); TSLB_SMEM_ATTR(float, true, 2, 0);
-    TSLB_SMEM_ATTR(float, false, 3, 1); TSLB_SMEM_ATTR(float, true, 3, 1);
-    TSLB_SMEM_ATTR(float, false, 2, 1); TSLB_SMEM_ATTR(float, true, 2, 1);
-    TSLB_SMEM_ATTR(double, false, 3, 0); TSLB_SMEM_ATTR(double, true, 3, 0);
-    TSLB_SMEM_ATTR(double, false, 2, 0); TSLB_SMEM_ATTR(double, true, 2, 0);
+    TSLB_SMEM_ATTR(float, 0, 3, 0); TSLB_SMEM_ATTR(float, 1, 3, 0);
+    TSLB_SMEM_ATTR(float, 0, 2, 0); TSLB_SMEM_ATTR(float, 1, 2, 0);
+    TSLB_SMEM_ATTR(float, 0, 3, 1); TSLB_SMEM_ATTR(float, 1, 3, 1);
+    TSLB_SMEM_ATTR(float, 0, 2, 1); TSLB_SMEM_ATTR(float, 1, 2, 1);
+    TSLB_SMEM_ATTR(double, 0, 3, 0); TSLB_SMEM_ATTR(double, 1, 3, 0);
+    TSLB_SMEM_ATTR(double, 0, 2, 0); TSLB_SMEM_ATTR(double, 1, 2, 0);
 #undef TSLB_SMEM_ATTR
     if (e != cudaSuccess) return e;
     c->tmap_ok = 1;
     return cudaSuccess;
 }
 
-template <typename T, bool WALLY, int ORDER, int GEO>
+template <typename T, int WALLY, int ORDER, int GEO>
 static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 {
     dim3 grid;
@@ -1234,7 +1297,23 @@ static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 
 // fp32 has two tile geometries: the one with the smaller estimated duration is taken (a lattice that cannot fill 148
 // large CTAs, or whose width / height the large tile pads badly, runs on the small one)
-template <typename T, bool WALLY, int ORDER>
+// z walls: the large geometry, plain store warp, no sponge (tslb_tile_supported / make_tile see to it)
+template <typename T, int ORDER>
+static void launch_tile_zwall(tslb_ctx *c, cudaStream_t st)
+{
+    dim3 grid;
+    TileParams<T> p = make_tile<T, 0>(c, &grid, nullptr);
+    const int a = c->cur, b = 1 - c->cur;
+    c->last_fused = 0;
+    FuseParams fp;
+    fp.L = c->L;
+    fp.tnext = c->t + 1;
+    for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
+    sweep_tile_kernel<T, 2, ORDER, false, false, 0><<<grid, TileDims<T, 0>::THREADS, TileDims<T, 0>::SMEM_BYTES, st>>>(
+        c->tm_main[0][a], c->tm_row[0][a], c->tm_store[0][b], (T *)c->buf[b], p, fp);
+}
+
+template <typename T, int WALLY, int ORDER>
 static void launch_tile(tslb_ctx *c, cudaStream_t st)
 {
     if (sizeof(T) == 8) { launch_tile_geo<T, WALLY, ORDER, 0>(c, st); return; }
@@ -1251,13 +1330,16 @@ static void launch_tile(tslb_ctx *c, cudaStream_t st)
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
 {
     const bool wally = c->kind[2] == TSLB_BC_BOUNCE_BACK || c->kind[3] == TSLB_BC_BOUNCE_BACK;
+    const bool wallz = c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK;
     const bool o3 = c->order >= 3;
     if (c->dtype == TSLB_F32) {
-        if (wally) { if (o3) launch_tile<float, true, 3>(c, st); else launch_tile<float, true, 2>(c, st); }
-        else { if (o3) launch_tile<float, false, 3>(c, st); else launch_tile<float, false, 2>(c, st); }
+        if (wallz) { if (o3) launch_tile_zwall<float, 3>(c, st); else launch_tile_zwall<float, 2>(c, st); }
+        else if (wally) { if (o3) launch_tile<float, 1, 3>(c, st); else launch_tile<float, 1, 2>(c, st); }
+        else { if (o3) launch_tile<float, 0, 3>(c, st); else launch_tile<float, 0, 2>(c, st); }
     } else {
-        if (wally) { if (o3) launch_tile<double, true, 3>(c, st); else launch_tile<double, true, 2>(c, st); }
-        else { if (o3) launch_tile<double, false, 3>(c, st); else launch_tile<double, false, 2>(c, st); }
+        if (wallz) { if (o3) launch_tile_zwall<double, 3>(c, st); else launch_tile_zwall<double, 2>(c, st); }
+        else if (wally) { if (o3) launch_tile<double, 1, 3>(c, st); else launch_tile<double, 1, 2>(c, st); }
+        else { if (o3) launch_tile<double, 0, 3>(c, st); else launch_tile<double, 0, 2>(c, st); }
     }
     c->launches++;
     return cudaGetLastError();

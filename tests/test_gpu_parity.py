@@ -42,7 +42,8 @@ def with_faces(w, faces, g=(0.0, 0.0, 0.0), inlet_face=None, seed=5):
 # ---------------------------------------------------------------------------------------------
 # small cases: several tiles + ragged tails, every boundary kind, both dtypes, every kernel
 # ---------------------------------------------------------------------------------------------
-# (the tile kernel needs ny >= one tile height: 14 rows fp32, 8 rows fp64; smaller lattices run on the gather kernel only)
+# (the tile kernel needs ny >= one tile height: 4 rows fp32 (small geometry), 8 rows fp64; smaller lattices run on the gather
+#  kernel only)
 SHAPES = [(3, 3, 3), (4, 3, 5), (5, 7, 9), (33, 17, 6), (64, 12, 10), (130, 9, 7), (136, 36, 5), (260, 20, 4),
           (61, 14, 5), (3, 29, 3), (124, 15, 33), (60, 28, 3), (59, 43, 4)]
 
@@ -251,6 +252,18 @@ def test_order2_config1_reduced(B, oracle_mod):
         G, R, curve = run_both(oracle_mod, w, w.steps, k, checkpoints=[1, 100])
         print("config1@32 order 2 kernel %d curve: %s" % (k, curve))
         assert_parity(w, G, R, "order 2 kernel %d" % k)
+
+
+def test_which_boundary_sets_run_on_the_tile_kernel(B):
+    """Bounce-back walls on the y faces or on the z faces (also next to open faces) run on the tile kernel; walls on x or on
+    two axes fall back to the gather kernel."""
+    want = {"walls_y+force": TILE, "walls_z": TILE, "walls_x": GATHER, "walls_xyz": GATHER, "jet_like": TILE,
+            "inlet_x_walls_y": TILE, "outlet_y_walls_z": TILE, "mixed_wall_outlet_same_axis": TILE}
+    for name, k in want.items():
+        w = with_faces(W.random_state(70, 31, 12, seed=3, dtype="f32", tau=0.6), **BC_SETS[name])
+        sim = B.from_workload(w, B.KERNEL_AUTO)
+        assert sim.active_kernel() == k, name
+        sim.close()
 
 
 def test_open_faces_are_filled_inside_the_sweep(B, oracle_mod):
