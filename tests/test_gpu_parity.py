@@ -254,6 +254,34 @@ def test_order2_config1_reduced(B, oracle_mod):
         assert_parity(w, G, R, "order 2 kernel %d" % k)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_tile_kernel_is_bitwise_repeatable(B, dtype):
+    """The sweep has no atomics and a fixed operation order: repeated runs from the same state must agree bit for bit.
+    A run-to-run difference means a race between the warp roles (exchange slots, stage ring, output tiles, the store
+    warp's boundary patches): 12 repetitions of 6 steps on lattices that exercise every instantiation family."""
+    import torch
+    cases = {"periodic": W.random_state(130, 38, 70, seed=71, dtype=dtype, tau=0.6),
+             "small_geometry": W.random_state(64, 9, 24, seed=72, dtype=dtype, tau=0.6),
+             "walls_y": with_faces(W.random_state(124, 37, 30, seed=73, dtype=dtype, tau=0.6), **BC_SETS["walls_y+force"]),
+             "walls_z": with_faces(W.random_state(124, 37, 30, seed=74, dtype=dtype, tau=0.6), **BC_SETS["walls_z"]),
+             "jet_fused": with_faces(W.random_state(124, 38, 30, seed=75, dtype=dtype, tau=0.6), **BC_SETS["jet_like"]),
+             "inlet_x_walls_y": with_faces(W.random_state(124, 37, 30, seed=76, dtype=dtype, tau=0.6), **BC_SETS["inlet_x_walls_y"])}
+    for name, w in cases.items():
+        ref = None
+        for rep in range(12):
+            sim = make_gpu(w, TILE)
+            assert sim.active_kernel() == TILE, name
+            sim.step(6)
+            G = sim.get_moments()
+            torch.cuda.synchronize()
+            if ref is None:
+                ref = G.clone()
+                assert torch.isfinite(ref).all(), name
+            else:
+                assert torch.equal(G, ref), "%s: run %d differs from run 0 in %d values" % (name, rep, int((G != ref).sum()))
+            sim.close()
+
+
 def test_which_boundary_sets_run_on_the_tile_kernel(B):
     """Bounce-back walls on the y faces or on the z faces (also next to open faces) run on the tile kernel; walls on x or on
     two axes fall back to the gather kernel."""
