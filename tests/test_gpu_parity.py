@@ -282,6 +282,23 @@ def test_tile_kernel_is_bitwise_repeatable(B, dtype):
             sim.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_z_walls_and_sponge_across_z_chunks(B, oracle_mod, dtype):
+    """Lattices longer than one z chunk (64 planes): the wall planes sit in the first and the last chunk only, the sponge
+    table is indexed with the source plane of every chunk; z walls also next to open faces and with a body force."""
+    wz = with_faces(W.random_state(70, 26, 150, seed=81, dtype=dtype, tau=0.6), **BC_SETS["walls_z"])
+    wz.g = (1e-4, -1e-4, 2e-4)
+    wo = with_faces(W.random_state(66, 25, 140, seed=82, dtype=dtype, tau=0.58), **BC_SETS["outlet_y_walls_z"])
+    wm = with_faces(W.random_state(30, 13, 135, seed=83, dtype=dtype, tau=0.58), **BC_SETS["mixed_wall_outlet_same_axis"])
+    ws = W.random_state(40, 20, 150, seed=84, dtype=dtype, tau=0.54)
+    ws.sponge = (100, 1000.0, 3.0)
+    for w in (wz, wo, wm, ws):
+        ks = kernels_for(B, w)
+        assert TILE in ks, w.name
+        G, R, _ = run_both(oracle_mod, w, 4, TILE)
+        assert_parity(w, G, R, "%s tile" % w.name)
+
+
 def test_which_boundary_sets_run_on_the_tile_kernel(B):
     """Bounce-back walls on the y faces or on the z faces (also next to open faces) run on the tile kernel; walls on x or on
     two axes fall back to the gather kernel."""
