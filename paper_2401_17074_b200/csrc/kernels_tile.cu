@@ -395,7 +395,7 @@ __device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32
     }
 }
 
-// WALL: 0 = no bounce-back wall, 1 = walls on y faces, 2 = walls on z faces (walls on two axes, or on x: gather kernel)
+// WALL: 0 = no bounce-back wall, 1 = walls on y faces, 2 = walls on z faces, 3 = both (a duct); walls on x: gather kernel
 template <typename T, int WALL, int ORDER, bool SPONGE, bool FUSE, int GEO>
 __global__ void __maxnreg__((TileDims<T, GEO>::MAXREG))
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
@@ -403,7 +403,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 {
     typedef typename PackOf<T>::type P;
     typedef TileDims<T, GEO> TD;
-    constexpr bool WALLY = WALL == 1, WALLZ = WALL == 2;
+    constexpr bool WALLY = (WALL & 1) != 0, WALLZ = (WALL & 2) != 0;
     constexpr int NS = TD::NS, BXW = TD::BXW, FS = TD::FS, ROWS = TD::ROWS, COLS = TD::COLS, WY = TD::WY, WX = TD::WX;
     constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
     constexpr int ES = (int)sizeof(T);
@@ -1003,6 +1003,12 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #pragma unroll
             for (int k = 0; k < 4; ++k) kwall[k] = pbc<P, T>((T)0);
         }
+        // Duct (walls on y AND z): on a row next to a y wall of a plane next to a z wall the three populations that arrive
+        // across the edge (c_y and c_z both pointing out of the walls) are in the y correction (9 populations, all c_z)
+        // and in the z replacement V (9 populations, all c_y): they are taken out once.  With
+        // Bm(kx) = sum_kz t_kz(-c_z) B(kx,kz) and the local sums over x:  e(px,py,pz) = c_y^py c_z^pz (6 Bm0 | -2 Bm1 | 2 (Bm0 + Bm2)).
+        P ewall[TSLB_NF];
+        bool edge = false;
         if (WALLY && any_ghost) {
             const P wsp = pk(ghost_lo ? (T)-1 : (T)1, (T)1);
             const P wm = pk(ghost_lo ? (T)1 : (T)0, ghost_hi ? (T)1 : (T)0);               // which row of the pack is at a wall
@@ -1032,6 +1038,24 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                 kwall[1] = pmul(padd(WB00, WB02), w12);                     // 002
                 kwall[2] = pmul(WB11, pmuls(wm, (T)4));                     // 101
                 kwall[3] = pmul(WB01, pmuls(w12s, (T)-1));                  // 011
+                if (WALLZ) {
+                    const int ztw = z0 + i - 2;
+                    const bool e_lo = ztw == 0 && p.kind[4] == TSLB_BC_BOUNCE_BACK, e_hi = ztw == L.nz - 1 && p.kind[5] == TSLB_BC_BOUNCE_BACK;
+                    if (e_lo || e_hi) {
+                        edge = true;
+                        const T cz = e_lo ? (T)1 : (T)-1;
+                        const P F10 = pfmas(uprev[0], (T)3, own(w, qidx(1, 0)));
+                        P Bm0 = padd(pfmas(WB01, -cz, WB00), WB02);
+                        P Bm1 = pfmas(WB11, -cz, F10);
+                        if (kvalid<ORDER>(1, 0, 2)) Bm1 = padd(Bm1, own(w, qidx(1, 2)));
+                        P Bm2 = own(w, qidx(2, 0));
+                        if (kvalid<ORDER>(2, 0, 1)) Bm2 = pfmas(own(w, qidx(2, 1)), -cz, Bm2);
+                        const P s6 = pmul(pmuls(Bm0, (T)6), wm), s2 = pmul(pmuls(Bm1, (T)-2), wm);
+                        ewall[0] = s6; ewall[1] = s2; ewall[2] = pmul(s6, sgp); ewall[3] = pmuls(s6, cz);
+                        ewall[4] = pmul(pmuls(padd(Bm0, Bm2), (T)2), wm); ewall[5] = s6; ewall[6] = s6;
+                        ewall[7] = pmul(s2, sgp); ewall[8] = pmuls(s2, cz); ewall[9] = pmuls(pmul(s6, sgp), cz);
+                    }
+                }
             }
         }
 
@@ -1051,6 +1075,10 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             m[7] = tt1[4];                                               // 110
             m[5] = tt1[5];                                               // 020
             if (WALLY) { m[3] = padd(m[3], kwall[0]); m[6] = padd(m[6], kwall[1]); m[8] = padd(m[8], kwall[2]); m[9] = padd(m[9], kwall[3]); }
+            if (WALLY && WALLZ && edge) {
+#pragma unroll
+                for (int k = 0; k < TSLB_NF; ++k) m[k] = psub(m[k], ewall[k]);
+            }
 
             // ---- a8: finalise the two rows from their 216-scaled raw moments (m[1..3] lack their base 216 u), Eq. 12 ------
             // x/216 as x*hi + x*lo: unbiased to ~1 ulp (a rounded 1/216 alone would be a systematic gain)
@@ -1187,13 +1215,13 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 bool tslb_tile_supported(const tslb_ctx *c, const char **why)
 {
-    // bounce-back walls are handled on the y faces or on the z faces (walls on x, or on two axes: gather kernel); the z-wall
+    // bounce-back walls are handled on the y faces, on the z faces, or on both (walls on x: gather kernel); the z-wall
     // instantiations exist for the plain case only (no sponge layer)
     bool wall_ax[3] = {false, false, false};
     for (int f = 0; f < 6; ++f)
         if (c->kind[f] == TSLB_BC_BOUNCE_BACK) wall_ax[f >> 1] = true;
-    if (wall_ax[0] || (wall_ax[1] && wall_ax[2])) {
-        if (why) *why = "bounce-back walls on x faces or on two axes";
+    if (wall_ax[0]) {
+        if (why) *why = "bounce-back walls on x faces";
         return false;
     }
     if (wall_ax[2] && (c->beta_z_host || c->nz < 4 || c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS))) {
@@ -1256,7 +1284,8 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     }
     e = cudaSuccess;
 #define TSLB_SMEM_ATTR_Z(T, O)                                                                                                  \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 2, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 2, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 3, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES)
     TSLB_SMEM_ATTR_Z(float, 3); TSLB_SMEM_ATTR_Z(float, 2); TSLB_SMEM_ATTR_Z(double, 3); TSLB_SMEM_ATTR_Z(double, 2);
 #undef TSLB_SMEM_ATTR_Z
 #define TSLB_SMEM_ATTR(T, W, O, G)                                                                                              \
@@ -1298,7 +1327,7 @@ static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 // fp32 has two tile geometries: the one with the smaller estimated duration is taken (a lattice that cannot fill 148
 // large CTAs, or whose width / height the large tile pads badly, runs on the small one)
 // z walls: the large geometry, plain store warp, no sponge (tslb_tile_supported / make_tile see to it)
-template <typename T, int ORDER>
+template <typename T, int ORDER, int WALLV>
 static void launch_tile_zwall(tslb_ctx *c, cudaStream_t st)
 {
     dim3 grid;
@@ -1309,7 +1338,7 @@ static void launch_tile_zwall(tslb_ctx *c, cudaStream_t st)
     fp.L = c->L;
     fp.tnext = c->t + 1;
     for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
-    sweep_tile_kernel<T, 2, ORDER, false, false, 0><<<grid, TileDims<T, 0>::THREADS, TileDims<T, 0>::SMEM_BYTES, st>>>(
+    sweep_tile_kernel<T, WALLV, ORDER, false, false, 0><<<grid, TileDims<T, 0>::THREADS, TileDims<T, 0>::SMEM_BYTES, st>>>(
         c->tm_main[0][a], c->tm_row[0][a], c->tm_store[0][b], (T *)c->buf[b], p, fp);
 }
 
@@ -1333,11 +1362,13 @@ cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
     const bool wallz = c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK;
     const bool o3 = c->order >= 3;
     if (c->dtype == TSLB_F32) {
-        if (wallz) { if (o3) launch_tile_zwall<float, 3>(c, st); else launch_tile_zwall<float, 2>(c, st); }
+        if (wallz && wally) { if (o3) launch_tile_zwall<float, 3, 3>(c, st); else launch_tile_zwall<float, 2, 3>(c, st); }
+        else if (wallz) { if (o3) launch_tile_zwall<float, 3, 2>(c, st); else launch_tile_zwall<float, 2, 2>(c, st); }
         else if (wally) { if (o3) launch_tile<float, 1, 3>(c, st); else launch_tile<float, 1, 2>(c, st); }
         else { if (o3) launch_tile<float, 0, 3>(c, st); else launch_tile<float, 0, 2>(c, st); }
     } else {
-        if (wallz) { if (o3) launch_tile_zwall<double, 3>(c, st); else launch_tile_zwall<double, 2>(c, st); }
+        if (wallz && wally) { if (o3) launch_tile_zwall<double, 3, 3>(c, st); else launch_tile_zwall<double, 2, 3>(c, st); }
+        else if (wallz) { if (o3) launch_tile_zwall<double, 3, 2>(c, st); else launch_tile_zwall<double, 2, 2>(c, st); }
         else if (wally) { if (o3) launch_tile<double, 1, 3>(c, st); else launch_tile<double, 1, 2>(c, st); }
         else { if (o3) launch_tile<double, 0, 3>(c, st); else launch_tile<double, 0, 2>(c, st); }
     }

@@ -63,6 +63,7 @@ BC_SETS = {
     "walls_z": dict(faces={W.FACE_ZLO: W.BC_BOUNCE_BACK, W.FACE_ZHI: W.BC_BOUNCE_BACK}),
     "walls_x": dict(faces={W.FACE_XLO: W.BC_BOUNCE_BACK, W.FACE_XHI: W.BC_BOUNCE_BACK}, g=(0, 1e-4, 0)),
     "walls_xyz": dict(faces={f: W.BC_BOUNCE_BACK for f in range(6)}, g=(1e-4, 1e-4, -1e-4)),
+    "walls_yz_duct": dict(faces={f: W.BC_BOUNCE_BACK for f in (2, 3, 4, 5)}, g=(2e-4, 1e-4, -1e-4)),
     "jet_like": dict(faces={W.FACE_ZLO: W.BC_VELOCITY_INLET, **{f: W.BC_OUTLET_ZERO_GRADIENT for f in (0, 1, 2, 3, 5)}},
                      inlet_face=W.FACE_ZLO),
     "inlet_x_walls_y": dict(faces={W.FACE_XLO: W.BC_VELOCITY_INLET, W.FACE_XHI: W.BC_OUTLET_ZERO_GRADIENT,
@@ -264,6 +265,7 @@ def test_tile_kernel_is_bitwise_repeatable(B, dtype):
              "small_geometry": W.random_state(64, 9, 24, seed=72, dtype=dtype, tau=0.6),
              "walls_y": with_faces(W.random_state(124, 37, 30, seed=73, dtype=dtype, tau=0.6), **BC_SETS["walls_y+force"]),
              "walls_z": with_faces(W.random_state(124, 37, 30, seed=74, dtype=dtype, tau=0.6), **BC_SETS["walls_z"]),
+             "duct": with_faces(W.random_state(124, 37, 30, seed=77, dtype=dtype, tau=0.6), **BC_SETS["walls_yz_duct"]),
              "jet_fused": with_faces(W.random_state(124, 38, 30, seed=75, dtype=dtype, tau=0.6), **BC_SETS["jet_like"]),
              "inlet_x_walls_y": with_faces(W.random_state(124, 37, 30, seed=76, dtype=dtype, tau=0.6), **BC_SETS["inlet_x_walls_y"])}
     for name, w in cases.items():
@@ -290,9 +292,10 @@ def test_z_walls_and_sponge_across_z_chunks(B, oracle_mod, dtype):
     wz.g = (1e-4, -1e-4, 2e-4)
     wo = with_faces(W.random_state(66, 25, 140, seed=82, dtype=dtype, tau=0.58), **BC_SETS["outlet_y_walls_z"])
     wm = with_faces(W.random_state(30, 13, 135, seed=83, dtype=dtype, tau=0.58), **BC_SETS["mixed_wall_outlet_same_axis"])
+    wd = with_faces(W.random_state(64, 27, 130, seed=85, dtype=dtype, tau=0.6), **BC_SETS["walls_yz_duct"])
     ws = W.random_state(40, 20, 150, seed=84, dtype=dtype, tau=0.54)
     ws.sponge = (100, 1000.0, 3.0)
-    for w in (wz, wo, wm, ws):
+    for w in (wz, wo, wm, wd, ws):
         ks = kernels_for(B, w)
         assert TILE in ks, w.name
         G, R, _ = run_both(oracle_mod, w, 4, TILE)
@@ -302,7 +305,7 @@ def test_z_walls_and_sponge_across_z_chunks(B, oracle_mod, dtype):
 def test_which_boundary_sets_run_on_the_tile_kernel(B):
     """Bounce-back walls on the y faces or on the z faces (also next to open faces) run on the tile kernel; walls on x or on
     two axes fall back to the gather kernel."""
-    want = {"walls_y+force": TILE, "walls_z": TILE, "walls_x": GATHER, "walls_xyz": GATHER, "jet_like": TILE,
+    want = {"walls_y+force": TILE, "walls_z": TILE, "walls_yz_duct": TILE, "walls_x": GATHER, "walls_xyz": GATHER, "jet_like": TILE,
             "inlet_x_walls_y": TILE, "outlet_y_walls_z": TILE, "mixed_wall_outlet_same_axis": TILE}
     for name, k in want.items():
         w = with_faces(W.random_state(70, 31, 12, seed=3, dtype="f32", tau=0.6), **BC_SETS[name])
