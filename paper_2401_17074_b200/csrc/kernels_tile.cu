@@ -1010,9 +1010,12 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         P ewall[TSLB_NF];
         bool edge = false;
         if (WALLY && any_ghost) {
-            const P wsp = pk(ghost_lo ? (T)-1 : (T)1, (T)1);
-            const P wm = pk(ghost_lo ? (T)1 : (T)0, ghost_hi ? (T)1 : (T)0);               // which row of the pack is at a wall
-            const P sgp = pk(ghost_lo ? (T)1 : (T)-1, (T)-1);                              // c_y of the arrival direction
+            // (the flags pass through an opaque asm so that the packs below are rebuilt here, a few selects, instead of being
+            //  hoisted out of the plane loop, where they would occupy 14 registers of every main warp all the time)
+            const bool glo = keep((uint32_t)ghost_lo) != 0u, ghi = keep((uint32_t)ghost_hi) != 0u;
+            const P wsp = pk(glo ? (T)-1 : (T)1, (T)1);
+            const P wm = pk(glo ? (T)1 : (T)0, ghi ? (T)1 : (T)0);                         // which row of the pack is at a wall
+            const P sgp = pk(glo ? (T)1 : (T)-1, (T)-1);                                   // c_y of the arrival direction
             const P w12 = pmuls(wm, (T)12), w36 = pmuls(wm, (T)36), w12s = pmul(w12, sgp), w36s = pmul(w36, sgp);
             // (re-read from this warp's own exchange slots instead of being kept in registers across the passes; lanes 0, 1 of
             //  the wx = 1 warp published in the private columns 62, 63)
