@@ -75,6 +75,10 @@ template <typename P> __device__ __forceinline__ P shfl_dn1(P v)
 // rematerialise through), so the loop carries no address arithmetic beyond the stage / slot offsets.
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ uint32_t keep(uint32_t v) { asm volatile("" : "+r"(v)); return v; }
+// the same for a floating-point value: a loop-invariant parameter that passes through keepf inside the loop is re-read
+// (one constant-bank load) in every iteration instead of being hoisted into registers that stay occupied all the time
+__device__ __forceinline__ float keepf(float v) { asm volatile("" : "+f"(v)); return v; }
+__device__ __forceinline__ double keepf(double v) { asm volatile("" : "+d"(v)); return v; }
 __device__ __forceinline__ void mbar_init(uint32_t bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -275,6 +279,10 @@ template <typename T, int G> struct TileGeom;
 #define TILE_F32_NS 2
 #endif
 // duration of one plane of a small-geometry CTA relative to a large one (measured, profiles/README.md)
+// 1: the main warps re-read beta and g from the parameter bank in every plane (see keepf)
+#ifndef TILE_REREAD_PARAMS
+#define TILE_REREAD_PARAMS 1
+#endif
 #ifndef TILE_SMALL_PLANE
 #define TILE_SMALL_PLANE 0.8
 #endif
@@ -756,8 +764,11 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         P (&dprev)[3] = db[1 - PAR];
         P (&dcur)[3] = db[PAR];
         // 1 - omega of the source plane: uniform, or per plane inside a sponge layer (Eq. 26)
-        T bz = p.beta;
+        T bz = TILE_REREAD_PARAMS ? keepf(p.beta) : p.beta;
         if (SPONGE) bz = __ldg(p.beta_z + zsrc(i));
+        T gz[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) gz[a] = TILE_REREAD_PARAMS ? keepf(p.g[a]) : p.g[a];
         mbar_wait(bring + B_FULL, NS == 2 ? ph : fpar);
 
         // ---- a1: moments of the own rows r0, r0+1 and the velocities of the rows r0-1, r0+2 at this column ------------------
@@ -825,7 +836,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #define TSLB_MAIN_ROUND(KZ)                                                                       \
             {                                                                                     \
                 P A[3][3];                                                                        \
-                hermite_round<KZ, P, T>(rc, bz, p.g, A);                                          \
+                hermite_round<KZ, P, T>(rc, bz, gz, A);                                           \
                 if (WALLZ && wsrc) {                                                              \
                     TSLB_BZ(0, 0, 0, KZ) TSLB_BZ(1, 1, 0, KZ) TSLB_BZ(2, 2, 0, KZ)                \
                     TSLB_BZ(3, 0, 1, KZ) TSLB_BZ(4, 1, 1, KZ) TSLB_BZ(5, 0, 2, KZ)                \
