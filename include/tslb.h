@@ -176,6 +176,21 @@ int tslb_get_timing(tslb_ctx *ctx, int *n_launches, double *total_ms);
  * fixed-order final pass (bitwise reproducible).  TSLB_EINVAL: bad axis or NULL; TSLB_ESTATE: no state. */
 int tslb_plane_statistics(tslb_ctx *ctx, int axis, double *dev_sums, void *stream);
 
+/* The same sums as tslb_plane_statistics, for callers that must not allocate or hand over scratch (CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the per-CTA partial sums live in a file-scope device array of the
+ * library -- [13][TSLB_PLANE_STATISTICS_STATIC_MAX][8] doubles = 832 KiB, held by every GPU that loads the library until
+ * exit -- instead of the workspace.  The call itself allocates nothing (no cudaMalloc / cudaFree, two kernel launches on
+ * `stream`, preceded by the boundary-fill launch when boundary nodes are stale, as in tslb_plane_statistics).
+ * dev_sums: [13][n_axis] doubles in device memory, caller-owned, sums are ADDED as above; same fixed summation order,
+ * hence bitwise the same result as tslb_plane_statistics.
+ * All calls on one device share the array: it keeps the last call's contents (every entry that is read is rewritten
+ * first, so nothing needs clearing), and calls that overlap on the GPU -- different streams without ordering, also from
+ * different contexts -- race on it.
+ * TSLB_EINVAL: bad axis, NULL, or n_axis > TSLB_PLANE_STATISTICS_STATIC_MAX (use tslb_plane_statistics then);
+ * TSLB_ESTATE: no state; TSLB_ECUDA: the array's device address could not be obtained, or a launch failed. */
+#define TSLB_PLANE_STATISTICS_STATIC_MAX 1024
+int tslb_plane_statistics_static(tslb_ctx *ctx, int axis, double *dev_sums, void *stream);
+
 /* Running (r, z)-bin statistics of a round jet along z (Fig. 7-8: centre-line velocity and Eq. 27,
  * half-width, mean axial profile, axial / radial rms, Reynolds stress <u'_z u'_r> on sections z = const).  Reading A27
  * (DESIGN.md): with (xc, yc) the jet axis in node coordinates, dx = x - xc, dy = y - yc, r = sqrt(dx^2 + dy^2), a node

@@ -26,7 +26,9 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_set_moments_host", "tslb_set_boundary", "tslb_set_kernel", "tslb_active_kernel", "tslb_step",
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
-           "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics")
+           "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics",
+           "tslb_plane_statistics_static")
+PLANE_STATISTICS_STATIC_MAX = 1024   # TSLB_PLANE_STATISTICS_STATIC_MAX of include/tslb.h
 
 
 class InletParams(C.Structure):
@@ -74,6 +76,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_export_state.argtypes = [vp, vp, C.POINTER(C.c_longlong), vp]
     lib.tslb_import_state.argtypes = [vp, vp, C.c_longlong, vp]
     lib.tslb_plane_statistics.argtypes = [vp, ip, vp, vp]
+    lib.tslb_plane_statistics_static.argtypes = [vp, ip, vp, vp]
     lib.tslb_radial_statistics.argtypes = [vp, C.c_double, C.c_double, C.c_double, ip, vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
@@ -250,6 +253,17 @@ class TSLB:
             raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
         self._chk(self._lib.tslb_plane_statistics(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
                   "tslb_plane_statistics")
+        return sums
+
+    def plane_statistics_static(self, axis: int, sums, stream=None):
+        """tslb_plane_statistics_static: the same sums with the scratch in a static device array of the library; allocates
+        nothing (the caller passes `sums`), n_axis <= PLANE_STATISTICS_STATIC_MAX, overlapping calls on one GPU race."""
+        import torch
+        n_axis = self.shape[2 - axis]
+        if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == (13, n_axis)):
+            raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
+        self._chk(self._lib.tslb_plane_statistics_static(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
+                  "tslb_plane_statistics_static")
         return sums
 
     def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums=None, stream=None):

@@ -582,3 +582,53 @@ cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cud
     c->launches += 2;
     return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------
+// Allocation-free variant of the plane statistics (tslb_plane_statistics_static in include/tslb.h): the per-CTA partial
+// sums live in a file-scope device array instead of the caller's workspace, so the call needs no scratch from anybody --
+// for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
+//   * Size: [13][TSLB_STATIC_STAT_MAX_AXIS][8] doubles = 832 KiB, held by every GPU that loads the library until exit.
+//   * In host code the array's NAME is a host-side stand-in, not a device address: the kernels get the address that
+//     cudaGetSymbolAddress returns, looked up once per device with that device current (static_scratch_ptr).
+//   * Every call on a device shares the array.  The partial kernel overwrites every entry the final kernel reads
+//     (all 13 x n_axis x 8 of them), so nothing has to be cleared between calls and stale contents of an earlier, larger
+//     call are never read; but two calls that OVERLAP on the GPU (different streams, no ordering) race on it.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_stat_scratch[TSLB_STAT_ROWS * TSLB_STATIC_STAT_MAX_AXIS * TSLB_STAT_PARTS];
+
+#define TSLB_STATIC_MAX_DEVICES 64
+static double *g_static_stat_ptr[TSLB_STATIC_MAX_DEVICES];      // device address of the array, per device ordinal (0 = not looked up)
+
+static cudaError_t static_scratch_ptr(double **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= TSLB_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    double *p = __atomic_load_n(&g_static_stat_ptr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        e = cudaGetSymbolAddress((void **)&p, g_static_stat_scratch);       // the current device's copy of the array
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        __atomic_store_n(&g_static_stat_ptr[dev], p, __ATOMIC_RELEASE);     // (two threads racing here store the same value)
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+// No cudaMalloc / cudaFree / allocating library routine anywhere on this path: two kernel launches on `st`.
+cudaError_t tslb_launch_plane_stats_static(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st)
+{
+    const int na = axis == 0 ? c->nx : (axis == 1 ? c->ny : c->nz);
+    if (na > TSLB_STATIC_STAT_MAX_AXIS) return cudaErrorInvalidValue;       // (the API layer reports this with a message)
+    double *scratch = nullptr;
+    cudaError_t e = static_scratch_ptr(&scratch);
+    if (e != cudaSuccess) return e;
+    dim3 grid(na, TSLB_STAT_PARTS);
+    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, scratch);
+    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, scratch);
+    const int tot = TSLB_STAT_ROWS * na;
+    stats_final_kernel<<<(tot + 127) / 128, 128, 0, st>>>(scratch, na, TSLB_STAT_PARTS, dev_sums);
+    c->launches += 2;
+    return cudaGetLastError();
+}

@@ -458,6 +458,26 @@ int tslb_radial_statistics(tslb_ctx *c, double xc, double yc, double dr, int nr,
     return TSLB_OK;
 }
 
+int tslb_plane_statistics_static(tslb_ctx *c, int axis, double *dev_sums, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (axis < 0 || axis > 2) return fail(c, TSLB_EINVAL, "axis must be 0, 1 or 2");
+    if (!dev_sums) return fail(c, TSLB_EINVAL, "dev_sums == NULL");
+    const int na = axis == 0 ? c->nx : (axis == 1 ? c->ny : c->nz);
+    if (na > TSLB_PLANE_STATISTICS_STATIC_MAX) {
+        snprintf(c->err, sizeof c->err, "tslb_plane_statistics_static: axis %d has %d planes, the static scratch holds %d (use tslb_plane_statistics)",
+                 axis, na, TSLB_PLANE_STATISTICS_STATIC_MAX);
+        return TSLB_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = refresh_boundary(c, false, st);
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_plane_stats_static(c, axis, dev_sums, st);
+    if (e != cudaSuccess) return cuda_fail(c, "plane statistics kernels (static scratch)", e);
+    return TSLB_OK;
+}
+
 long long tslb_step_count(const tslb_ctx *c) { return c && c->have_state ? c->t : -1; }
 long long tslb_launch_count(const tslb_ctx *c) { return c ? c->launches : -1; }
 const char *tslb_last_error(const tslb_ctx *c) { return c ? c->err : g_create_err; }

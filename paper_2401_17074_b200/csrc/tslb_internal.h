@@ -149,3 +149,5 @@ cudaError_t tslb_launch_radial_stats(tslb_ctx *c, double xc, double yc, double d
 
 #define TSLB_STAT_ROWS 13   // 1, u (3), uu (6), uuu (3)
 #define TSLB_STAT_PARTS 8   // CTAs per plane in the statistics reduction
+#define TSLB_STATIC_STAT_MAX_AXIS TSLB_PLANE_STATISTICS_STATIC_MAX   // longest axis the allocation-free variant accepts (include/tslb.h)
+cudaError_t tslb_launch_plane_stats_static(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st);  // scratch in a static device array
