@@ -259,6 +259,16 @@ __device__ __forceinline__ void ycombos(const P (&A)[3][3], T &p0, T &m0, T &p1,
     }
 }
 
+// x-wall combination of the coefficients of one node pack: Bx(ky,kz) = sum_kx t_kx(-c_x) A(kx,ky,kz) = A0 - c_x A1 + A2
+template <int ORDER, int KY, int KZ, typename P, typename T>
+__device__ __forceinline__ P bx_combo(const P (&A)[3][3], T cx)
+{
+    P b = kvalid<ORDER>(0, KY, KZ) ? A[0][KY] : pbc<P, T>((T)0);
+    if (kvalid<ORDER>(1, KY, KZ)) b = pfmas(A[1][KY], -cx, b);
+    if (kvalid<ORDER>(2, KY, KZ)) b = padd(b, A[2][KY]);
+    return b;
+}
+
 // index of group (px,py), px+py <= 2, in the z-march state: (0,0)=0 (1,0)=1 (2,0)=2 (0,1)=3 (1,1)=4 (0,2)=5
 __host__ __device__ constexpr int gidx(int px, int py) { return py == 0 ? px : (py == 1 ? 3 + px : 5); }
 // index of the coefficient group (kx, kz) among the 8 exchanged ones
@@ -403,7 +413,8 @@ __device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32
     }
 }
 
-// WALL: 0 = no bounce-back wall, 1 = walls on y faces, 2 = walls on z faces, 3 = both (a duct); walls on x: gather kernel
+// WALL: 0 = no bounce-back wall, 1 = walls on y faces, 2 = walls on z faces, 3 = both (a duct), 4 = walls on x faces
+// (x walls together with y or z walls: gather kernel)
 template <typename T, int WALL, int ORDER, bool SPONGE, bool FUSE, int GEO>
 __global__ void __maxnreg__((TileDims<T, GEO>::MAXREG))
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
@@ -411,7 +422,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 {
     typedef typename PackOf<T>::type P;
     typedef TileDims<T, GEO> TD;
-    constexpr bool WALLY = (WALL & 1) != 0, WALLZ = (WALL & 2) != 0;
+    constexpr bool WALLY = (WALL & 1) != 0, WALLZ = (WALL & 2) != 0, WALLX = (WALL & 4) != 0;
     constexpr int NS = TD::NS, BXW = TD::BXW, FS = TD::FS, ROWS = TD::ROWS, COLS = TD::COLS, WY = TD::WY, WX = TD::WX;
     constexpr int NPACK = TD::NPACK, NGRP = TD::NGRP, EXW = TD::EXW, XPAD = TD::XPAD;
     constexpr int ES = (int)sizeof(T);
@@ -736,6 +747,20 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
 #pragma unroll
     for (int a = 0; a < 3; ++a) { ub[0][a] = pbc<P, T>((T)0); ub[1][a] = ub[0][a]; db[0][a] = ub[0][a]; db[1][a] = ub[0][a]; }
 
+    // ---- halfway bounce-back on an x face (WALL = 4).  A lane that holds a column beyond the wall sends nothing into the x
+    //      pass (msrc = 0) and enters the x differences with u = 0; the lane that holds the wall column adds, one iteration
+    //      later (when its plane is the target), the nine bounced populations f*_ibar of its own nodes: with
+    //      Bx(ky,kz) = sum_kx t_kx(-c_x) A(kx,ky,kz) and the local sums over y and z the ten corrections are
+    //      36 Bx00 | c_x 36 Bx00 | -12 Bx10 | -12 Bx01 | 36 Bx00 | 12 (Bx00 + Bx20) | 12 (Bx00 + Bx02) | -c_x 12 Bx10 |
+    //      -c_x 12 Bx01 | 4 Bx11   for the moments 000 | 100 | 010 | 001 | 200 | 020 | 002 | 110 | 101 | 011. ---------------------
+    const T cxl = !WALLX ? (T)0 : ((col == 0 && p.kind[0] == TSLB_BC_BOUNCE_BACK) ? (T)1
+                                   : ((col == L.nx - 1 && p.kind[1] == TSLB_BC_BOUNCE_BACK) ? (T)-1 : (T)0));
+    const P msrc = pbc<P, T>((WALLX && ((col < 0 && p.kind[0] == TSLB_BC_BOUNCE_BACK) || (col >= L.nx && p.kind[1] == TSLB_BC_BOUNCE_BACK))) ? (T)0 : (T)1);
+    P bxs[2][6];                                          // Bx of the source planes by parity, used when the plane is the target
+    if (WALLX) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { bxs[0][k] = pbc<P, T>((T)0); bxs[1][k] = bxs[0][k]; }
+    }
     const bool xper = p.kind[0] == TSLB_BC_PERIODIC;
     // periodic x: the node at x = 0 is also the ghost column x = nx, the node at x = nx-1 the ghost column x = -1
     const bool xedge = xper && lane_out && (col == 0 || col == L.nx - 1);
@@ -814,6 +839,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         const bool wsrc_hi = WALLZ && zsrc_raw >= L.nz && p.kind[5] == TSLB_BC_BOUNCE_BACK;
         const bool wsrc = wsrc_lo || wsrc_hi;
         P Bz[6];                                          // (kx,ky) = 00, 10, 20, 01, 11, 02
+        P Bx[6];                                          // (ky,kz) = 00, 10, 20, 01, 11, 02
         const T sz = wsrc_lo ? (T)-1 : (T)1;
         T qP0[NGRP], qM1[NGRP];
         P cen[NGRP];
@@ -841,6 +867,12 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                     TSLB_BZ(0, 0, 0, KZ) TSLB_BZ(1, 1, 0, KZ) TSLB_BZ(2, 2, 0, KZ)                \
                     TSLB_BZ(3, 0, 1, KZ) TSLB_BZ(4, 1, 1, KZ) TSLB_BZ(5, 0, 2, KZ)                \
                 }                                                                                 \
+                if (WALLX) {                                                                      \
+                    if (KZ == 0) { Bx[0] = bx_combo<ORDER, 0, KZ, P, T>(A, cxl); Bx[1] = bx_combo<ORDER, 1, KZ, P, T>(A, cxl); Bx[2] = bx_combo<ORDER, 2, KZ, P, T>(A, cxl); \
+                                   Bx[0] = pfmas(rc[1], (T)-3 * cxl, Bx[0]); Bx[1] = pfmas(rc[2], (T)3, Bx[1]); }                                                        \
+                    if (KZ == 1) { Bx[3] = pfmas(rc[3], (T)3, bx_combo<ORDER, 0, KZ, P, T>(A, cxl)); Bx[4] = bx_combo<ORDER, 1, KZ, P, T>(A, cxl); }                      \
+                    if (KZ == 2) { Bx[5] = bx_combo<ORDER, 0, KZ, P, T>(A, cxl); }                                                                                        \
+                }                                                                                 \
                 TSLB_MAIN_GROUP(0, KZ) TSLB_MAIN_GROUP(1, KZ) TSLB_MAIN_GROUP(2, KZ)              \
             }
             TSLB_MAIN_ROUND(0)
@@ -852,6 +884,11 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
         }
         if (GE::QFLAGS) flag_set(bQown, (uint32_t)(i + 1), lane);
         else warp_arrive(bQown + 8 * PAR, lane);
+
+        if (WALLX) {                                      // kept for the next iteration, when this plane is the target
+#pragma unroll
+            for (int k = 0; k < 6; ++k) bxs[PAR][k] = Bx[k];
+        }
 
         // ---- increment form along y: exact differences of the stored velocities,
         //      Ly = (up - c) + (dn - c), Wy = (up - dn) * sgn with up / dn the neighbour rows (hu = (u(r0-1), u(r0+2)), the
@@ -956,13 +993,15 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             if (kz == 0) {
 #pragma unroll
                 for (int a = 0; a < 2; ++a) {
-                    const P xl = shfl_up1(rc[1 + a]), xr = shfl_dn1(rc[1 + a]);
+                    const P us = WALLX ? pmul(rc[1 + a], msrc) : rc[1 + a];
+                    const P xl = shfl_up1(us), xr = shfl_dn1(us);
                     Lx[a] = pfmas(rc[1 + a], (T)-2, padd(xl, xr));
                     Dx[a] = psub(xl, xr);
                 }
             }
             if (kz == 1) {
-                const P xl = shfl_up1(rc[3]), xr = shfl_dn1(rc[3]);
+                const P us = WALLX ? pmul(rc[3], msrc) : rc[3];
+                const P xl = shfl_up1(us), xr = shfl_dn1(us);
                 Lx[2] = pfmas(rc[3], (T)-2, padd(xl, xr));
                 Dx[2] = psub(xl, xr);
             }
@@ -975,6 +1014,7 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                 if (kvalid<ORDER>(2, 0, kz)) t = padd(t, G1[py][2]);
                 P pp = t, mm = t;
                 if (kvalid<ORDER>(1, 0, kz)) { pp = padd(t, G1[py][1]); mm = psub(t, G1[py][1]); }
+                if (WALLX) { pp = pmul(pp, msrc); mm = pmul(mm, msrc); }
                 const P upP = shfl_up1(pp);   // from column-1  (c_x = +1 pulls from x-1)
                 const P dnM = shfl_dn1(mm);   // from column+1
                 P o[3];
@@ -1089,6 +1129,16 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
             m[7] = tt1[4];                                               // 110
             m[5] = tt1[5];                                               // 020
             if (WALLY) { m[3] = padd(m[3], kwall[0]); m[6] = padd(m[6], kwall[1]); m[8] = padd(m[8], kwall[2]); m[9] = padd(m[9], kwall[3]); }
+            if (WALLX && cxl != (T)0) {                   // (divergent inside an edge warp only: no shuffles in here)
+                const P (&bx)[6] = bxs[1 - PAR];
+                const P b36 = pmuls(bx[0], (T)36), n10 = pmuls(bx[1], (T)-12), n01 = pmuls(bx[3], (T)-12);
+                m[0] = padd(m[0], b36); m[1] = pfmas(b36, cxl, m[1]); m[2] = padd(m[2], n10); m[3] = padd(m[3], n01);
+                m[4] = padd(m[4], b36);
+                m[5] = pfmas(padd(bx[0], bx[2]), (T)12, m[5]);
+                m[6] = pfmas(padd(bx[0], bx[5]), (T)12, m[6]);
+                m[7] = pfmas(n10, cxl, m[7]); m[8] = pfmas(n01, cxl, m[8]);
+                m[9] = pfmas(bx[4], (T)4, m[9]);
+            }
             if (WALLY && WALLZ && edge) {
 #pragma unroll
                 for (int k = 0; k < TSLB_NF; ++k) m[k] = psub(m[k], ewall[k]);
@@ -1211,6 +1261,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
     if (open_k(5) && c->nz - (int)(grid->z - 1) * zc < 2) ok = false;             // z = nz-1 alone in the last chunk
     if (zc < 2) ok = false;
     if (c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK) ok = false;   // z-wall kernels: plain store warp only
+    if (c->kind[0] == TSLB_BC_BOUNCE_BACK || c->kind[1] == TSLB_BC_BOUNCE_BACK) ok = false;   // x-wall kernels likewise
 #ifdef TILE_NO_FUSE
     ok = false;
 #endif
@@ -1229,17 +1280,17 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 
 bool tslb_tile_supported(const tslb_ctx *c, const char **why)
 {
-    // bounce-back walls are handled on the y faces, on the z faces, or on both (walls on x: gather kernel); the z-wall
-    // instantiations exist for the plain case only (no sponge layer)
+    // bounce-back walls are handled on the y faces, on the z faces, on both, or on the x faces alone (x walls together with
+    // other walls: gather kernel); the x- and z-wall instantiations exist for the plain case only (no sponge layer)
     bool wall_ax[3] = {false, false, false};
     for (int f = 0; f < 6; ++f)
         if (c->kind[f] == TSLB_BC_BOUNCE_BACK) wall_ax[f >> 1] = true;
-    if (wall_ax[0]) {
-        if (why) *why = "bounce-back walls on x faces";
+    if (wall_ax[0] && (wall_ax[1] || wall_ax[2])) {
+        if (why) *why = "bounce-back walls on x faces together with walls on another axis";
         return false;
     }
-    if (wall_ax[2] && (c->beta_z_host || c->nz < 4 || c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS))) {
-        if (why) *why = "z walls together with a sponge layer, or fewer rows than one large tile";
+    if ((wall_ax[2] || wall_ax[0]) && (c->beta_z_host || c->nz < 4 || c->ny < (c->dtype == TSLB_F64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS))) {
+        if (why) *why = "x or z walls together with a sponge layer, or fewer rows than one large tile";
         return false;
     }
     // every tile is full: the last tile of the y axis is shifted back, which needs at least one tile height of rows
@@ -1299,7 +1350,8 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     e = cudaSuccess;
 #define TSLB_SMEM_ATTR_Z(T, O)                                                                                                  \
     if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 2, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES); \
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 3, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 3, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_tile_kernel<T, 4, O, false, false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TileDims<T, 0>::SMEM_BYTES)
     TSLB_SMEM_ATTR_Z(float, 3); TSLB_SMEM_ATTR_Z(float, 2); TSLB_SMEM_ATTR_Z(double, 3); TSLB_SMEM_ATTR_Z(double, 2);
 #undef TSLB_SMEM_ATTR_Z
 #define TSLB_SMEM_ATTR(T, W, O, G)                                                                                              \
@@ -1340,7 +1392,7 @@ static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 
 // fp32 has two tile geometries: the one with the smaller estimated duration is taken (a lattice that cannot fill 148
 // large CTAs, or whose width / height the large tile pads badly, runs on the small one)
-// z walls: the large geometry, plain store warp, no sponge (tslb_tile_supported / make_tile see to it)
+// x or z walls (WALLV = 2, 3, 4): the large geometry, plain store warp, no sponge (tslb_tile_supported / make_tile see to it)
 template <typename T, int ORDER, int WALLV>
 static void launch_tile_zwall(tslb_ctx *c, cudaStream_t st)
 {
@@ -1374,8 +1426,12 @@ cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st)
 {
     const bool wally = c->kind[2] == TSLB_BC_BOUNCE_BACK || c->kind[3] == TSLB_BC_BOUNCE_BACK;
     const bool wallz = c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK;
+    const bool wallx = c->kind[0] == TSLB_BC_BOUNCE_BACK || c->kind[1] == TSLB_BC_BOUNCE_BACK;
     const bool o3 = c->order >= 3;
-    if (c->dtype == TSLB_F32) {
+    if (wallx) {
+        if (c->dtype == TSLB_F32) { if (o3) launch_tile_zwall<float, 3, 4>(c, st); else launch_tile_zwall<float, 2, 4>(c, st); }
+        else { if (o3) launch_tile_zwall<double, 3, 4>(c, st); else launch_tile_zwall<double, 2, 4>(c, st); }
+    } else if (c->dtype == TSLB_F32) {
         if (wallz && wally) { if (o3) launch_tile_zwall<float, 3, 3>(c, st); else launch_tile_zwall<float, 2, 3>(c, st); }
         else if (wallz) { if (o3) launch_tile_zwall<float, 3, 2>(c, st); else launch_tile_zwall<float, 2, 2>(c, st); }
         else if (wally) { if (o3) launch_tile<float, 1, 3>(c, st); else launch_tile<float, 1, 2>(c, st); }

@@ -266,6 +266,7 @@ def test_tile_kernel_is_bitwise_repeatable(B, dtype):
              "walls_y": with_faces(W.random_state(124, 37, 30, seed=73, dtype=dtype, tau=0.6), **BC_SETS["walls_y+force"]),
              "walls_z": with_faces(W.random_state(124, 37, 30, seed=74, dtype=dtype, tau=0.6), **BC_SETS["walls_z"]),
              "duct": with_faces(W.random_state(124, 37, 30, seed=77, dtype=dtype, tau=0.6), **BC_SETS["walls_yz_duct"]),
+             "walls_x": with_faces(W.random_state(124, 37, 30, seed=78, dtype=dtype, tau=0.6), **BC_SETS["walls_x"]),
              "jet_fused": with_faces(W.random_state(124, 38, 30, seed=75, dtype=dtype, tau=0.6), **BC_SETS["jet_like"]),
              "inlet_x_walls_y": with_faces(W.random_state(124, 37, 30, seed=76, dtype=dtype, tau=0.6), **BC_SETS["inlet_x_walls_y"])}
     for name, w in cases.items():
@@ -295,7 +296,9 @@ def test_z_walls_and_sponge_across_z_chunks(B, oracle_mod, dtype):
     wd = with_faces(W.random_state(64, 27, 130, seed=85, dtype=dtype, tau=0.6), **BC_SETS["walls_yz_duct"])
     ws = W.random_state(40, 20, 150, seed=84, dtype=dtype, tau=0.54)
     ws.sponge = (100, 1000.0, 3.0)
-    for w in (wz, wo, wm, wd, ws):
+    wx = with_faces(W.random_state(130, 26, 70, seed=86, dtype=dtype, tau=0.6), **BC_SETS["walls_x"])
+    wx.g = (1e-4, 2e-4, -1e-4)
+    for w in (wz, wo, wm, wd, wx, ws):
         ks = kernels_for(B, w)
         assert TILE in ks, w.name
         G, R, _ = run_both(oracle_mod, w, 4, TILE)
@@ -305,7 +308,7 @@ def test_z_walls_and_sponge_across_z_chunks(B, oracle_mod, dtype):
 def test_which_boundary_sets_run_on_the_tile_kernel(B):
     """Bounce-back walls on the y faces or on the z faces (also next to open faces) run on the tile kernel; walls on x or on
     two axes fall back to the gather kernel."""
-    want = {"walls_y+force": TILE, "walls_z": TILE, "walls_yz_duct": TILE, "walls_x": GATHER, "walls_xyz": GATHER, "jet_like": TILE,
+    want = {"walls_y+force": TILE, "walls_z": TILE, "walls_yz_duct": TILE, "walls_x": TILE, "walls_xyz": GATHER, "jet_like": TILE,
             "inlet_x_walls_y": TILE, "outlet_y_walls_z": TILE, "mixed_wall_outlet_same_axis": TILE}
     for name, k in want.items():
         w = with_faces(W.random_state(70, 31, 12, seed=3, dtype="f32", tau=0.6), **BC_SETS[name])
