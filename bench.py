@@ -70,6 +70,9 @@ class ClockSampler:
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._read, daemon=True)
             self.thr.start()
+            t0 = time.time()                      # nvidia-smi needs a moment to start: wait for its first sample, so that even
+            while not self.lines and time.time() - t0 < 2.0:   # a timed region shorter than the sampling period has a reading
+                time.sleep(0.01)
         except OSError:
             self.proc = None
 

@@ -463,7 +463,6 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) { mbar_init(sb + B_FULL + 8 * s, 1); mbar_init(sb + B_EMPTY + 8 * s, TD::WARPS); }
-#pragma unroll
         if (TileGeom<T, GEO>::QFLAGS) {
             for (int s = 0; s < 4 * (NPACK + 1); ++s)                               // published flags: 4 bytes per warp, zero = nothing yet
                 asm volatile("st.shared.u32 [%0], %1;" ::"r"(sb + B_Q + 4 * s), "r"(0u) : "memory");
