@@ -34,7 +34,12 @@
  * viscous decay, forced Poiseuille curvature, shear stress Pi_xy = -(tau/3) rho du/dy, lattice
  * symmetries, brute-vs-closed; open faces: the populations pulled from inlet / outlet nodes equal Eq. 23 as printed
  * (built with independent numpy Hermite tensors, two time levels), uniform through-flow is a fixed point; diagnostics
- * equal the plain numpy sums.  Still PARITY UNPINNED (readings, nothing in the paper or the mathematics fixes them):
+ * equal the plain numpy sums; sponge layer (Eq. 26): K = 0 identity, the profile at the paper's numbers, equivalence with a
+ * population code that relaxes every node with its own omega, decay rates of a two-region layer; pressure outlet: Eq. 23
+ * with the imposed density, through-flow fixed point; NEQ no-slip wall: Poiseuille parabola through u = 0 at the wall
+ * nodes; Gaussian noise: the Box-Muller identity through the pinned mixer and the sample moments of a unit normal; plane
+ * statistics: closed-form Taylor-Green sums, numpy central moments; (r,z)-ring statistics: an analytic swirling jet via
+ * numpy hypot / bincount, the axis node, rotation invariance.  Still PARITY UNPINNED (readings, nothing in the paper or the mathematics fixes them):
  * A13's nozzle geometry (top-hat disc on a full inlet plane), A14's noise law (uniform, relative) and A16's clamp rule
  * where several open faces meet.
  *
