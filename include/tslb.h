@@ -52,7 +52,9 @@ enum {
     TSLB_BC_VELOCITY_INLET = 2,       /* nodes ON the face: u imposed, rho and Pi_neq from x_F          */
     TSLB_BC_OUTLET_ZERO_GRADIENT = 3, /* nodes ON the face: all 10 moments copied from x_F              */
     TSLB_BC_BODY_FORCE = 4,           /* not a face kind: sets the body acceleration g (face ignored)   */
-    TSLB_BC_OUTLET_PRESSURE = 5       /* nodes ON the face: rho imposed, u and Pi_neq copied from x_F    */
+    TSLB_BC_OUTLET_PRESSURE = 5,      /* nodes ON the face: rho imposed, u and Pi_neq copied from x_F    */
+    TSLB_BC_EXCHANGE = 6              /* z faces only: nodes ON the face are the ghost plane of a slab     */
+                                      /* decomposition, supplied by tslb_import_face (below)               */
 };
 /* Bit 8 of tslb_inlet_params.noise_component_mask: Gaussian noise law instead of the uniform one (below). */
 #define TSLB_NOISE_GAUSSIAN 0x100
@@ -103,7 +105,7 @@ int tslb_set_moments(tslb_ctx *ctx, const void *dev_src, void *stream);
 int tslb_set_moments_host(tslb_ctx *ctx, const void *host_src, void *stream);
 
 /* Set the kind of one face, or the body force.
- *   PERIODIC / BOUNCE_BACK / OUTLET_ZERO_GRADIENT : params == NULL.
+ *   PERIODIC / BOUNCE_BACK / OUTLET_ZERO_GRADIENT / EXCHANGE (z faces only) : params == NULL.
  *   VELOCITY_INLET : params -> tslb_inlet_params.
  *   OUTLET_PRESSURE: params -> const double rho_out (> 0): density imposed on the face nodes, u and Pi_neq from x_F
  *                    (PAPER.md:187 "either momentum or density/pressure", :202).
@@ -202,6 +204,27 @@ int tslb_plane_statistics_static(tslb_ctx *ctx, int axis, double *dev_sums, void
  * fp64 without fused multiply-adds (identical on every IEEE machine); the additions use atomics, so repeated runs agree
  * to rounding, not bitwise.  TSLB_EINVAL: NULL, dr <= 0, non-finite arguments, nr outside [1, 512]; TSLB_ESTATE: no state. */
 int tslb_radial_statistics(tslb_ctx *ctx, double xc, double yc, double dr, int nr, double *dev_sums, void *stream);
+
+/* Slab decomposition along z (PAPER.md:318 names multi-GPU domain decomposition as the next step).
+ * A rank owns planes [z_lo, z_hi) of the global lattice and holds them in a context of its own whose z axis is extended by
+ * one GHOST plane per cut face: face kind TSLB_BC_EXCHANGE on TSLB_FACE_ZLO and/or TSLB_FACE_ZHI.  The nodes of a ghost plane
+ * are never filled by the library and what a sweep writes there is meaningless; their time-t moments are the caller's to
+ * supply before every tslb_step (n = 1 per exchange): because a sweep reads only time-t nearest neighbours (Eq. 6, :157), the
+ * owned planes then advance exactly -- bit for bit -- as they would in the undivided lattice.  Per step and cut face:
+ *     tslb_export_face(face)  the 10 moments of the outermost OWNED plane (z = 1 for ZLO, z = nz - 2 for ZHI) at the current
+ *                             time, as held internally ([10][ny][nx], x fastest, field 0 = rho - 1: no rounding), after the
+ *                             open-face boundary nodes of that plane have been filled for the current time;
+ *     (transport: the caller's -- NCCL send/recv over NVLink in paper_2401_17074_b200/slab.py, a device copy on one GPU)
+ *     tslb_import_face(face)  such an array into the ghost plane (z = 0 for ZLO, z = nz - 1 for ZHI) of the current state,
+ *                             ghost columns included.
+ * Both are asynchronous on `stream`; face_bytes = 10 * ny * nx * sizeof(dtype) (tslb_face_bytes).  Ghost planes are left out
+ * of tslb_diagnostics, so the sums of the ranks add up to those of the undivided lattice.  The seeded inlet noise is keyed
+ * on the node's index in the context's own lattice: an inlet on the z = 0 face of the first slab draws the numbers of the
+ * undivided run, inlets on faces the cuts cross do not.
+ * TSLB_EINVAL: face is not ZLO / ZHI or not of kind EXCHANGE, NULL pointer; TSLB_ESTATE: no state. */
+size_t tslb_face_bytes(const tslb_ctx *ctx);
+int tslb_export_face(tslb_ctx *ctx, int face, void *dev_dst, void *stream);
+int tslb_import_face(tslb_ctx *ctx, int face, const void *dev_src, void *stream);
 
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libtslb.so")
 TSLB_F32, TSLB_F64 = 0, 1
 TSLB_OK, TSLB_EINVAL, TSLB_ENOMEM, TSLB_ECUDA, TSLB_ESTATE = range(5)
 FACE_XLO, FACE_XHI, FACE_YLO, FACE_YHI, FACE_ZLO, FACE_ZHI = range(6)
-BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE, BC_OUTLET_PRESSURE = range(6)
+BC_PERIODIC, BC_BOUNCE_BACK, BC_VELOCITY_INLET, BC_OUTLET_ZERO_GRADIENT, BC_BODY_FORCE, BC_OUTLET_PRESSURE, BC_EXCHANGE = range(7)
 NOISE_GAUSSIAN = 0x100
 KERNEL_AUTO, KERNEL_GATHER, KERNEL_TILE = range(3)
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_GATHER: "gather", KERNEL_TILE: "tile"}
@@ -27,7 +27,7 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
            "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics",
-           "tslb_plane_statistics_static")
+           "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face")
 PLANE_STATISTICS_STATIC_MAX = 1024   # TSLB_PLANE_STATISTICS_STATIC_MAX of include/tslb.h
 
 
@@ -78,6 +78,10 @@ def load_library(path: Optional[str] = None):
     lib.tslb_plane_statistics.argtypes = [vp, ip, vp, vp]
     lib.tslb_plane_statistics_static.argtypes = [vp, ip, vp, vp]
     lib.tslb_radial_statistics.argtypes = [vp, C.c_double, C.c_double, C.c_double, ip, vp, vp]
+    lib.tslb_face_bytes.argtypes = [vp]
+    lib.tslb_face_bytes.restype = C.c_size_t
+    lib.tslb_export_face.argtypes = [vp, ip, vp, vp]
+    lib.tslb_import_face.argtypes = [vp, ip, vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
@@ -236,6 +240,24 @@ class TSLB:
         self._check_tensor(S, "state", (10,) + self.shape)
         self._chk(self._lib.tslb_import_state(self._h, C.c_void_p(S.data_ptr()), int(step_count), _stream_ptr(stream)), "tslb_import_state")
 
+    def face_bytes(self) -> int:
+        return int(self._lib.tslb_face_bytes(self._h))
+
+    def export_face(self, face: int, out=None, stream=None):
+        """The outermost owned plane next to the EXCHANGE face `face` (FACE_ZLO / FACE_ZHI), raw internal values [10][ny][nx]."""
+        import torch
+        shape = (10,) + self.shape[1:]
+        if out is None:
+            out = torch.empty(shape, dtype=self.torch_dtype, device="cuda")
+        self._check_tensor(out, "out", shape)
+        self._chk(self._lib.tslb_export_face(self._h, int(face), C.c_void_p(out.data_ptr()), _stream_ptr(stream)), "tslb_export_face")
+        return out
+
+    def import_face(self, face: int, plane, stream=None):
+        """Load the ghost plane of the EXCHANGE face `face` from an array as written by export_face."""
+        self._check_tensor(plane, "plane", (10,) + self.shape[1:])
+        self._chk(self._lib.tslb_import_face(self._h, int(face), C.c_void_p(plane.data_ptr()), _stream_ptr(stream)), "tslb_import_face")
+
     def diagnostics(self, stream=None):
         """(mass, px, py, pz, kinetic energy) as a CUDA fp64 tensor of 5."""
         import torch
@@ -263,7 +285,7 @@ class TSLB:
         if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == (13, n_axis)):
             raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
         self._chk(self._lib.tslb_plane_statistics_static(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
-                  "tslb_plane_statistics_static")
+                  "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face")
         return sums
 
     def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums=None, stream=None):

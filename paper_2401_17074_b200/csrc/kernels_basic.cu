@@ -254,6 +254,32 @@ __global__ void fill_boundary_kernel(T *__restrict__ M, FillParams p)
 }
 
 // ---------------------------------------------------------------------------------------------
+// Slab decomposition along z (include/tslb.h, tslb_export_face / tslb_import_face): plane z of the internal buffer <-> a dense
+// array [10][ny][nx], values unchanged (field 0 stays rho - 1).  The import also writes the ghost columns x = -1 and x = nx of
+// the plane (periodic image, else the clamped node: only has to be finite), so that no halo launch is needed after it.
+// 40 B/node of a plane each way: 10.5 MB for 512^2 fp32, a few microseconds at HBM speed.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int DIR>
+__global__ void face_kernel(T *__restrict__ M, T *__restrict__ dense, Layout L, int z, int xper)
+{
+    const int w = L.nx + 2;
+    const long long tot = (long long)TSLB_NF * L.ny * w;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += stride) {
+        const int x = (int)(i % w) - 1;
+        const long long r = i / w;
+        const int y = (int)(r % L.ny), f = (int)(r / L.ny);
+        int xs = x;
+        if (x < 0) xs = xper ? L.nx - 1 : 0;
+        if (x >= L.nx) xs = xper ? 0 : L.nx - 1;
+        const long long im = f * L.field + lay_idx(L, x, y, z);
+        const long long id = ((long long)f * L.ny + y) * L.nx + xs;
+        if (DIR > 0) M[im] = dense[id];
+        else if (x == xs) dense[id] = M[im];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Ghost-column refresh: the cells x = -1 and x = nx of every row take the 10 moments of the
 // node obtained by wrapping x on a periodic axis (clamping it otherwise).  The TMA-staged sweep reads its x neighbours
 // through these columns (a TMA row is contiguous and cannot wrap); it keeps them current itself, so this kernel runs
@@ -324,7 +350,8 @@ __global__ void __launch_bounds__(TSLB_DIAG_THREADS) diag_partial_kernel(const T
     for (int row = blockIdx.x * wpb + (threadIdx.x >> 5); row < nrows; row += gridDim.x * wpb) {
         const int y = row % p.L.ny, z = row / p.L.ny;
         if ((y == 0 && is_open_kind(p.kind[2])) || (y == p.L.ny - 1 && is_open_kind(p.kind[3])) ||
-            (z == 0 && is_open_kind(p.kind[4])) || (z == p.L.nz - 1 && is_open_kind(p.kind[5]))) continue;
+            (z == 0 && (is_open_kind(p.kind[4]) || p.kind[4] == TSLB_BC_EXCHANGE)) ||      // ghost planes of a slab belong to
+            (z == p.L.nz - 1 && (is_open_kind(p.kind[5]) || p.kind[5] == TSLB_BC_EXCHANGE))) continue;   // the neighbouring rank
         const T *r = A + lay_idx(p.L, 0, y, z);
         const int x0 = open_x0 ? 1 : 0, x1 = open_x1 ? p.L.nx - 1 : p.L.nx;
         for (int x = x0 + lane_; x < x1; x += 32) {
@@ -529,6 +556,24 @@ cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st)
     if (blocks > (long long)c->sm_count * 16) blocks = (long long)c->sm_count * 16;
     if (c->dtype == TSLB_F32) halo_kernel<float><<<(unsigned)blocks, 256, 0, st>>>((float *)buf, make_fill(c));
     else halo_kernel<double><<<(unsigned)blocks, 256, 0, st>>>((double *)buf, make_fill(c));
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tslb_launch_face(tslb_ctx *c, int dir, int z, void *dense, cudaStream_t st)
+{
+    const long long tot = (long long)TSLB_NF * c->ny * (c->nx + 2);
+    long long blocks = (tot + 255) / 256;
+    if (blocks > (long long)c->sm_count * 16) blocks = (long long)c->sm_count * 16;
+    const int xper = c->kind[0] == TSLB_BC_PERIODIC;
+    void *buf = c->buf[c->cur];
+    if (c->dtype == TSLB_F32) {
+        if (dir > 0) face_kernel<float, +1><<<(unsigned)blocks, 256, 0, st>>>((float *)buf, (float *)dense, c->L, z, xper);
+        else face_kernel<float, -1><<<(unsigned)blocks, 256, 0, st>>>((float *)buf, (float *)dense, c->L, z, xper);
+    } else {
+        if (dir > 0) face_kernel<double, +1><<<(unsigned)blocks, 256, 0, st>>>((double *)buf, (double *)dense, c->L, z, xper);
+        else face_kernel<double, -1><<<(unsigned)blocks, 256, 0, st>>>((double *)buf, (double *)dense, c->L, z, xper);
+    }
     c->launches++;
     return cudaGetLastError();
 }

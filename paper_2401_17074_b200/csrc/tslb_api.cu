@@ -258,7 +258,9 @@ int tslb_set_boundary(tslb_ctx *c, int face, int kind, const void *params)
         return TSLB_OK;
     }
     if (face < 0 || face > 5) return fail(c, TSLB_EINVAL, "unknown face");
-    if (kind < 0 || kind > TSLB_BC_OUTLET_PRESSURE) return fail(c, TSLB_EINVAL, "unknown boundary kind");
+    if (kind < 0 || kind > TSLB_BC_EXCHANGE) return fail(c, TSLB_EINVAL, "unknown boundary kind");
+    if (kind == TSLB_BC_EXCHANGE && face != TSLB_FACE_ZLO && face != TSLB_FACE_ZHI)
+        return fail(c, TSLB_EINVAL, "EXCHANGE (slab ghost plane) exists on the z faces only");
     if (kind == TSLB_BC_OUTLET_PRESSURE) {
         if (!params) return fail(c, TSLB_EINVAL, "OUTLET_PRESSURE needs params -> double rho_out");
         const double rho = *(const double *)params;
@@ -416,6 +418,43 @@ int tslb_import_state(tslb_ctx *c, const void *dev_src, long long step_count, vo
     cudaError_t e = tslb_launch_import_raw(c, dev_src, c->buf[0], (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
     c->cur = 0; c->t = step_count; c->have_state = 1; c->halo_valid = 0;
+    return TSLB_OK;
+}
+
+size_t tslb_face_bytes(const tslb_ctx *c)
+{
+    return c ? (size_t)TSLB_NF * c->ny * c->nx * tslb_elem(c) : 0;
+}
+
+static int face_check(tslb_ctx *c, int face, const void *ptr)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (face != TSLB_FACE_ZLO && face != TSLB_FACE_ZHI) return fail(c, TSLB_EINVAL, "face must be TSLB_FACE_ZLO or TSLB_FACE_ZHI");
+    if (c->kind[face] != TSLB_BC_EXCHANGE) return fail(c, TSLB_EINVAL, "face is not of kind TSLB_BC_EXCHANGE");
+    if (!ptr) return fail(c, TSLB_EINVAL, "face array == NULL");
+    return TSLB_OK;
+}
+
+int tslb_export_face(tslb_ctx *c, int face, void *dev_dst, void *stream)
+{
+    int rc = face_check(c, face, dev_dst);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = refresh_boundary(c, false, st);      // lateral open-face nodes of the owned plane, at the current time
+    if (e != cudaSuccess) return cuda_fail(c, "fill kernel", e);
+    e = tslb_launch_face(c, -1, face == TSLB_FACE_ZLO ? 1 : c->nz - 2, dev_dst, st);
+    if (e != cudaSuccess) return cuda_fail(c, "face export kernel", e);
+    return TSLB_OK;
+}
+
+int tslb_import_face(tslb_ctx *c, int face, const void *dev_src, void *stream)
+{
+    int rc = face_check(c, face, dev_src);
+    if (rc) return rc;
+    // the plane's ghost columns are written with it, so halo_valid keeps its value
+    cudaError_t e = tslb_launch_face(c, +1, face == TSLB_FACE_ZLO ? 0 : c->nz - 1, (void *)dev_src, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "face import kernel", e);
     return TSLB_OK;
 }
 

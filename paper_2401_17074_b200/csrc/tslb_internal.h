@@ -143,6 +143,7 @@ cudaError_t tslb_launch_import(tslb_ctx *c, const void *src, void *dst, cudaStre
 cudaError_t tslb_launch_export(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // internal -> API
 cudaError_t tslb_launch_import_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);  // the same without the rho <-> rho - 1 shift
 cudaError_t tslb_launch_export_raw(tslb_ctx *c, const void *src, void *dst, cudaStream_t st);
+cudaError_t tslb_launch_face(tslb_ctx *c, int dir, int z, void *dense, cudaStream_t st);   // slab ghost planes: dir +1 dense -> plane z of buf[cur], -1 back
 cudaError_t tslb_launch_diag(tslb_ctx *c, double *dev_out5, cudaStream_t st);
 cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st);
 cudaError_t tslb_launch_radial_stats(tslb_ctx *c, double xc, double yc, double dr, int nr, double *dev_sums, cudaStream_t st);

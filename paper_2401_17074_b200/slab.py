@@ -1,0 +1,228 @@
+"""Slab decomposition of one lattice along z over several GPUs.
+
+Host-side orchestration only: every number is produced by the kernels behind the C ABI.  A rank owns the planes
+[z_lo, z_hi) of the global lattice in a context of its own (`binding.TSLB`) whose z axis carries one ghost plane per cut
+face (face kind BC_EXCHANGE, include/tslb.h "Slab decomposition").  One step is
+
+    sweep of the slab (tslb_step)  ->  tslb_export_face of the outermost owned planes  ->  transport  ->  tslb_import_face
+
+and because a sweep reads time-t nearest neighbours only (PAPER.md:68 Eq. 6, :157), the owned planes advance bit for bit
+as in the undivided lattice.  Transport: `torch.distributed` point-to-point (NCCL over NVLink / NVSwitch: one 40 B/node
+plane per cut face and direction, 10.5 MB for 512^2 fp32, i.e. ~12 us at 900 GB/s against a ~2.3 ms sweep -- the
+exchange is not overlapped with the sweep, there is nothing to win yet), or plain device copies between slabs that live
+in one process on one GPU (`exchange_local`, what the 1-GPU parity test uses; the slabs never wait on one another).
+
+Limits (checked, with an error): the seeded inlet noise is keyed on a context's own node index, so a noisy inlet must sit
+on the global z = 0 / z = nz-1 face of a first / last slab whose z offset is zero (the jet's inlet does); a sponge layer
+(Eq. 26) must lie inside the last slab; statistics calls are per slab (ghost planes included -- strip them with
+`Slab.owned`).
+"""
+from __future__ import annotations
+
+import dataclasses
+from dataclasses import dataclass
+from typing import List, Optional, Sequence
+
+from . import workloads as W
+
+BC_EXCHANGE = 6   # TSLB_BC_EXCHANGE (include/tslb.h)
+
+
+@dataclass(frozen=True)
+class SlabPlan:
+    """Planes [z_lo, z_hi) of an nz-plane lattice on `rank` of `world`; lo_rank / hi_rank = -1 where the slab ends on a
+    face of the global lattice (which then keeps its own boundary kind)."""
+    rank: int
+    world: int
+    nz: int
+    z_lo: int
+    z_hi: int
+    lo_rank: int
+    hi_rank: int
+
+    @property
+    def ghost_lo(self) -> bool:
+        return self.lo_rank >= 0
+
+    @property
+    def ghost_hi(self) -> bool:
+        return self.hi_rank >= 0
+
+    @property
+    def owned(self) -> int:
+        return self.z_hi - self.z_lo
+
+    @property
+    def nz_local(self) -> int:
+        return self.owned + int(self.ghost_lo) + int(self.ghost_hi)
+
+    @property
+    def z_offset(self) -> int:
+        """global z of local plane 0"""
+        return self.z_lo - int(self.ghost_lo)
+
+
+def plan_slabs(nz: int, world: int, periodic_z: bool) -> List[SlabPlan]:
+    """Balanced split: the first nz % world ranks own one plane more.  Every slab owns at least one plane and its context
+    at least three (tslb_create's minimum)."""
+    if world < 1 or nz < world:
+        raise ValueError("cannot split %d planes over %d ranks" % (nz, world))
+    base, rem = divmod(nz, world)
+    plans, z = [], 0
+    for r in range(world):
+        n = base + (1 if r < rem else 0)
+        if world == 1:
+            lo = hi = -1                       # undivided: the z faces keep their kinds (periodic wraps inside the kernel)
+        elif periodic_z:
+            lo, hi = (r - 1) % world, (r + 1) % world
+        else:
+            lo, hi = (r - 1 if r > 0 else -1), (r + 1 if r < world - 1 else -1)
+        p = SlabPlan(r, world, nz, z, z + n, lo, hi)
+        if p.nz_local < 3:
+            raise ValueError("slab of rank %d would have %d planes (< 3): use fewer ranks" % (r, p.nz_local))
+        plans.append(p)
+        z += n
+    return plans
+
+
+def local_workload(w: W.Workload, plan: SlabPlan) -> W.Workload:
+    """The slab's own Workload: the global initial state cut to the slab's planes (ghost planes included, wrapped on a
+    periodic axis), EXCHANGE on the cut faces, everything else as in `w`."""
+    import numpy as np
+    periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
+    zs = np.arange(plan.z_offset, plan.z_offset + plan.nz_local)
+    if periodic_z:
+        zs = zs % w.nz
+    faces = dict(w.faces)
+    if plan.world > 1:
+        faces[W.FACE_ZLO] = BC_EXCHANGE if plan.ghost_lo else w.faces.get(W.FACE_ZLO, W.BC_PERIODIC)
+        faces[W.FACE_ZHI] = BC_EXCHANGE if plan.ghost_hi else w.faces.get(W.FACE_ZHI, W.BC_PERIODIC)
+    inlet = w.inlet
+    if inlet is not None and plan.world > 1:
+        if inlet.face == W.FACE_ZLO and plan.ghost_lo:
+            inlet = None                                        # the inlet face belongs to the first slab
+        elif inlet.face == W.FACE_ZHI and plan.ghost_hi:
+            inlet = None
+        elif inlet.face == W.FACE_ZHI and inlet.noise_amp != 0.0 and plan.z_offset != 0:
+            raise NotImplementedError("noisy inlet on z = nz-1 of a slab with a z offset (noise is keyed on local indices)")
+        elif inlet.face < W.FACE_ZLO:
+            if inlet.noise_amp != 0.0:
+                raise NotImplementedError("noisy inlet on a face the slab cuts cross (noise is keyed on local indices)")
+            up = inlet.u_plane                                  # [3][nz][n_a]: cut to the slab's planes
+            inlet = dataclasses.replace(inlet, u_plane=np.ascontiguousarray(up[:, zs, :]))
+    sponge = w.sponge
+    if sponge is not None and plan.world > 1:
+        z_start, K, p = sponge
+        if plan.z_hi != w.nz:
+            if z_start < plan.z_hi + 1:                         # the layer reaches this slab's planes or its upper ghost plane
+                raise NotImplementedError("sponge layer starts below the last slab")
+            sponge = None
+        else:
+            if z_start <= plan.z_offset:
+                raise NotImplementedError("sponge layer starts below the last slab")
+            sponge = (z_start - plan.z_offset, K, p)            # nz_local - z_start_local = nz - z_start: same profile
+    return dataclasses.replace(w, name="%s_slab%dof%d" % (w.name, plan.rank, plan.world), nz=plan.nz_local,
+                               moments=np.ascontiguousarray(w.moments[:, zs]), faces=faces, inlet=inlet, sponge=sponge)
+
+
+def exchange_planes(plan: SlabPlan, send_lo, send_hi, recv_lo, recv_hi, group=None) -> None:
+    """Point-to-point exchange of the cut-face planes with the neighbouring ranks (any device `torch.distributed` serves:
+    NCCL for CUDA tensors, gloo for CPU ones).  send_lo / send_hi: this rank's outermost owned planes; recv_lo / recv_hi:
+    what becomes its ghost planes.  With two ranks on a periodic axis both neighbours are the same peer: messages between
+    a pair are matched in the order they are issued (NCCL has no tags), so the low plane is always sent first and the
+    matching receive -- the neighbour's LOW plane is this rank's HIGH ghost -- is issued first."""
+    import torch.distributed as dist
+    ops = []
+    if plan.ghost_lo:
+        ops.append(dist.P2POp(dist.isend, send_lo, plan.lo_rank, group, tag=0))
+    if plan.ghost_hi:
+        ops.append(dist.P2POp(dist.isend, send_hi, plan.hi_rank, group, tag=1))
+    if plan.ghost_hi:
+        ops.append(dist.P2POp(dist.irecv, recv_hi, plan.hi_rank, group, tag=0))
+    if plan.ghost_lo:
+        ops.append(dist.P2POp(dist.irecv, recv_lo, plan.lo_rank, group, tag=1))
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+
+
+class Slab:
+    """One rank's part of a slab-decomposed lattice on the current CUDA device."""
+
+    def __init__(self, w: W.Workload, plan: SlabPlan, kernel: int = 0):
+        import torch
+        from . import binding
+        self.plan = plan
+        self.local = local_workload(w, plan)
+        self.sim = binding.from_workload(self.local, kernel)
+        self.sim.set_moments(torch.from_numpy(self.local.moments).to("cuda"))
+        shape = (10, w.ny, w.nx)
+        mk = lambda: torch.empty(shape, dtype=self.sim.torch_dtype, device="cuda")
+        self.send_lo, self.recv_lo = (mk(), mk()) if plan.ghost_lo else (None, None)
+        self.send_hi, self.recv_hi = (mk(), mk()) if plan.ghost_hi else (None, None)
+
+    # the three phases of one exchange (tslb_export_face / transport / tslb_import_face)
+    def export_faces(self, stream=None):
+        if self.plan.ghost_lo:
+            self.sim.export_face(W.FACE_ZLO, self.send_lo, stream)
+        if self.plan.ghost_hi:
+            self.sim.export_face(W.FACE_ZHI, self.send_hi, stream)
+
+    def import_faces(self, stream=None):
+        if self.plan.ghost_lo:
+            self.sim.import_face(W.FACE_ZLO, self.recv_lo, stream)
+        if self.plan.ghost_hi:
+            self.sim.import_face(W.FACE_ZHI, self.recv_hi, stream)
+
+    def exchange(self, group=None):
+        self.export_faces()
+        exchange_planes(self.plan, self.send_lo, self.send_hi, self.recv_lo, self.recv_hi, group)
+        self.import_faces()
+
+    def step(self, n: int = 1, group=None):
+        """n time steps of the whole lattice as seen from this rank (collective: every rank calls it)."""
+        for _ in range(n):
+            self.sim.step(1)
+            self.exchange(group)
+
+    def owned(self, M):
+        """Cut the ghost planes off an array whose axis 1 is the slab's z axis (get_moments, export_state)."""
+        return M[:, int(self.plan.ghost_lo): self.plan.nz_local - int(self.plan.ghost_hi)]
+
+    def owned_moments(self):
+        return self.owned(self.sim.get_moments())
+
+    def diagnostics(self, group=None, reduce: bool = True):
+        """(mass, momentum[3], kinetic energy) of the whole lattice: the slabs' sums (ghost planes left out) added up."""
+        import torch.distributed as dist
+        d = self.sim.diagnostics()
+        if reduce and self.plan.world > 1:
+            dist.all_reduce(d, op=dist.ReduceOp.SUM, group=group)
+        return d
+
+
+def exchange_local(slabs: Sequence[Slab]) -> None:
+    """The exchange between slabs that live in one process on one GPU: export everywhere, then copy plane to plane on the
+    current stream, then import.  Serial launches of one stream: no kernel ever waits on another."""
+    for s in slabs:
+        s.export_faces()
+    for s in slabs:
+        if s.plan.ghost_lo:
+            s.recv_lo.copy_(slabs[s.plan.lo_rank].send_hi)
+        if s.plan.ghost_hi:
+            s.recv_hi.copy_(slabs[s.plan.hi_rank].send_lo)
+    for s in slabs:
+        s.import_faces()
+
+
+def step_local(slabs: Sequence[Slab], n: int = 1) -> None:
+    for _ in range(n):
+        for s in slabs:
+            s.sim.step(1)
+        exchange_local(slabs)
+
+
+def gather_local(slabs: Sequence[Slab]):
+    """The whole lattice's moments [10][nz][ny][nx] from slabs of one process, in rank order."""
+    import torch
+    return torch.cat([s.owned_moments() for s in slabs], dim=1)

@@ -61,6 +61,14 @@ def test_host_only_state_machine(lib):
         s.set_body_force((float("inf"), 0, 0))
     s.set_body_force((1e-6, 0, 0))
     s.set_boundary(B.FACE_YLO, B.BC_BOUNCE_BACK)
+    # slab ghost planes exist on the z faces only; face export / import need a state
+    with pytest.raises(B.TSLBError) as e:
+        s.set_boundary(B.FACE_XLO, B.BC_EXCHANGE)
+    assert e.value.code == B.TSLB_EINVAL
+    s.set_boundary(B.FACE_ZHI, B.BC_EXCHANGE)
+    assert s.face_bytes() == 10 * 6 * 8 * 8
+    assert s._lib.tslb_export_face(s._h, B.FACE_ZHI, C.c_void_p(0x1000), None) == B.TSLB_ESTATE
+    assert s._lib.tslb_import_face(s._h, B.FACE_ZHI, C.c_void_p(0x1000), None) == B.TSLB_ESTATE
     with pytest.raises(B.TSLBError):
         s.set_kernel(5)
     # misaligned / undersized workspace

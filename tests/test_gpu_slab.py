@@ -1,0 +1,100 @@
+"""Slab decomposition along z (include/tslb.h tslb_export_face / tslb_import_face): several
+slabs of one lattice, each in a context of its own, advanced on ONE GPU with the ghost planes exchanged by device copies
+(slab.step_local: serial launches on one stream, no kernel waits on another), against (1) the fp64 oracle of the UNDIVIDED
+lattice, element by element, at the tolerances of the other parity tests, and (2) the undivided CUDA run, bit for bit --
+a node's arithmetic does not depend on where the lattice was cut.  The transport over torch.distributed is covered on CPU
+(tests/test_slab_host.py, gloo, world_size 2)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2401_17074_b200 import slab as S
+from paper_2401_17074_b200 import workloads as W
+from tests.parity_util import assert_parity, gpu_state, make_gpu, make_oracle
+from tests.test_gpu_parity import BC_SETS, B, kernels_for, with_faces  # noqa: F401  (B is the fixture)
+
+pytestmark = pytest.mark.gpu
+
+
+def run_slabs(w, world, steps, kernel):
+    import torch
+    periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
+    slabs = [S.Slab(w, p, kernel) for p in S.plan_slabs(w.nz, world, periodic_z)]
+    S.step_local(slabs, steps)
+    G = S.gather_local(slabs)
+    torch.cuda.synchronize()
+    return slabs, G.cpu().numpy()
+
+
+def lateral_inlet(dt):
+    """Inlet on a face the cuts cross (its imposed-velocity plane is cut with the slabs); noise off, see slab.py."""
+    w = with_faces(W.random_state(40, 16, 17, seed=55, dtype=dt, tau=0.6), **BC_SETS["outlet_y_walls_z"])
+    w.inlet = dataclasses.replace(w.inlet, noise_amp=0.0, noise_mask=0)
+    return w
+
+
+CASES = {
+    "periodic": lambda dt: W.random_state(70, 27, 23, seed=51, dtype=dt, tau=0.58),
+    "channel": lambda dt: with_faces(W.random_state(66, 15, 21, seed=52, dtype=dt, tau=0.6), **BC_SETS["walls_y+force"]),
+    "jet_like": lambda dt: with_faces(W.random_state(24, 17, 30, seed=53, dtype=dt, tau=0.55), **BC_SETS["jet_like"]),
+    "walls_z": lambda dt: with_faces(W.random_state(64, 12, 19, seed=54, dtype=dt, tau=0.6), **BC_SETS["walls_z"]),
+    "inlet_y_walls_z": lambda dt: lateral_inlet(dt),
+    "wall_outlet_z": lambda dt: with_faces(W.random_state(33, 17, 14, seed=56, dtype=dt, tau=0.6),
+                                           **BC_SETS["mixed_wall_outlet_same_axis"]),
+}
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_slabs_match_oracle_and_undivided_run(B, oracle_mod, case, world, dtype):
+    w = CASES[case](dtype)
+    steps = 6
+    o = make_oracle(oracle_mod, w)
+    o.step(steps)
+    R = o.get_moments()
+    for k in kernels_for(B, w):
+        slabs, G = run_slabs(w, world, steps, k)
+        assert all(s.sim.step_count == steps for s in slabs)
+        assert_parity(w, G.astype(np.float64), R, "%s, %d slabs, kernel %d" % (case, world, k))
+        one = make_gpu(w, k)
+        one.step(steps)
+        G1 = one.get_moments().cpu().numpy()
+        assert np.array_equal(G, G1), "%s: %d slabs differ from the undivided run (kernel %d), max %.3e" % (
+            case, world, k, np.abs(G.astype(np.float64) - G1).max())
+        # the slabs' diagnostics add up to the undivided lattice's (ghost planes are left out)
+        d = sum(s.diagnostics(reduce=False).cpu().numpy() for s in slabs)
+        d1 = one.diagnostics().cpu().numpy()
+        np.testing.assert_allclose(d, d1, rtol=1e-12, atol=1e-12 * abs(d1[0]))
+        one.close()
+        for s in slabs:
+            s.sim.close()
+
+
+def test_jet_with_inlet_noise_and_sponge_in_slabs(B, oracle_mod):
+    """configs[3]'s own boundary set, reduced: the noisy inlet sits on the first slab, the sponge layer in the last one."""
+    w = W.jet(24, 20, 40, steps=12, dtype="f32", D=6.0)
+    w.sponge = (32, 1000.0, 3.0)
+    o = make_oracle(oracle_mod, w)
+    o.step(w.steps)
+    R = o.get_moments()
+    for world in (2, 3):
+        slabs, G = run_slabs(w, world, w.steps, B.KERNEL_AUTO)
+        assert_parity(w, G.astype(np.float64), R, "jet, %d slabs" % world)
+        one = make_gpu(w, B.KERNEL_AUTO)
+        one.step(w.steps)
+        assert np.array_equal(G, one.get_moments().cpu().numpy())
+        one.close()
+
+
+def test_face_calls_reject_other_faces(B):
+    w = W.random_state(16, 8, 9, seed=3, dtype="f32")
+    s = S.Slab(w, S.plan_slabs(w.nz, 2, True)[0])
+    with pytest.raises(B.TSLBError) as e:
+        s.sim._chk(s.sim._lib.tslb_export_face(s.sim._h, B.FACE_XLO, 0x1000, None), "tslb_export_face")
+    assert e.value.code == B.TSLB_EINVAL
+    one = make_gpu(w, B.KERNEL_AUTO)                      # periodic z: not an EXCHANGE face
+    with pytest.raises(B.TSLBError):
+        one.export_face(B.FACE_ZLO)
+    one.close()
