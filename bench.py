@@ -44,6 +44,12 @@ def parse_args(argv=None):
     ap.add_argument("--kernel", default="auto", choices=["auto", "gather", "tile"])
     ap.add_argument("--order", type=int, default=3, choices=[2, 3],
                     help="Hermite order of the reconstruction: 3 = the paper's high-order TSLB (the headline), 2 = Eq. 8")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="opt-in: ONE lattice cut into this many z slabs (paper_2401_17074_b200/slab.py) instead of replicas: "
+                         "under torchrun one slab per rank (must equal the world size, NCCL point-to-point exchange, strong "
+                         "scaling); on one GPU all slabs on it with device-copy exchange (cost of the decomposition path)")
+    ap.add_argument("--staged", action="store_true",
+                    help="with --slabs: ghost planes through tslb_export_face / tslb_import_face instead of in place (tslb_face_planes)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
@@ -355,10 +361,109 @@ def run_ours(args):
     return 0
 
 
+def run_slabs(args):
+    """--slabs S: the same workload as one lattice cut into S slabs along z.  Not the default: the
+    north_star's path is one GPU / replicas; this leg measures what the decomposition costs."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2401_17074_b200 import binding as B
+    from paper_2401_17074_b200 import build as BLD
+    from paper_2401_17074_b200 import slab as S
+    from paper_2401_17074_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the TSLB path has no CPU fallback")
+    if world > 1 and args.slabs != world:
+        raise SystemExit("bench.py: --slabs must equal the world size under torchrun (one slab per rank)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    BLD.build_lib()
+    kernel = {"auto": B.KERNEL_AUTO, "gather": B.KERNEL_GATHER, "tile": B.KERNEL_TILE}[args.kernel]
+    w = make_workload(args)
+    w.order = args.order
+    plans = S.plan_slabs(w.nz, args.slabs, w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC)
+    slabs = [S.Slab(w, p, kernel, args.staged) for p in (plans if world == 1 else [plans[rank]])]
+    owned_sites = float(sum(s.plan.owned for s in slabs)) * w.nx * w.ny
+    stream = torch.cuda.current_stream()
+
+    def advance(n):
+        if world > 1:
+            slabs[0].step(n)
+        else:
+            S.step_local(slabs, n)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    advance(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    l0 = sum(s.sim.launch_count for s in slabs)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    advance(args.steps)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sum(s.sim.launch_count for s in slabs) - l0
+    clocks = sampler.stop() if rank == 0 else None
+    ms_max, units = aggregate(ms, owned_sites * args.steps, dist if world > 1 else None, "cuda")
+    d = sum(s.diagnostics(reduce=False) for s in slabs)
+    if world > 1:
+        dist.all_reduce(d)
+    d = d.cpu().numpy()
+    assert np.isfinite(d).all() and (args.workload == "jet" or abs(d[0] / w.sites - 1) < 1e-5), d
+    # the sweeps alone (event pairs around each sweep launch of every local slab), after the timed region
+    nt = max(1, min(args.steps, 20))
+    for s in slabs:
+        s.sim.set_timing(nt)
+    advance(nt)
+    torch.cuda.synchronize()
+    sweep_ms = sum(s.sim.get_timing()[1] for s in slabs) / nt
+    for s in slabs:
+        s.sim.set_timing(0)
+    if rank == 0:
+        peak, peak_src = hbm_peak()
+        step_ms = ms_max / args.steps
+        achieved = BYTES_PER_SITE[args.dtype] * (units / args.steps) / (step_ms * 1e-3) / 1e9
+        cfg = dict(workload_config(args), order=args.order, kernel=B.KERNEL_NAMES[slabs[0].sim.active_kernel()])
+        cfg["parallelism"] = ("one lattice in %d z slabs, " % args.slabs) + (
+            "one slab per GPU, ghost planes by NCCL point-to-point" if world > 1 else "all on one GPU, ghost planes by device copies")
+        cfg["slab_planes"] = [p.owned for p in plans]
+        cfg["transport"] = "staged (tslb_export_face / tslb_import_face)" if args.staged else "in place (tslb_face_planes)"
+        line = {"metric": "GLUPS", "value": glups(units, ms_max), "unit": "GLUPS", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": args.dtype, "data": "synthetic", "config": cfg,
+                "roofline": {"bound": "hbm", "kernel": "whole step: sweep of every local slab + face export / transport / import",
+                             "achieved": achieved, "peak": (peak * world) if peak else None, "unit": "GB/s",
+                             "frac": achieved / (peak * world) if peak else None, "peak_source": peak_src,
+                             "algorithmic_bytes_per_site": BYTES_PER_SITE[args.dtype], "traffic": None,
+                             "sweep_ms_per_step_rank0": sweep_ms, "exchange_ms_per_step_rank0": ms / args.steps - sweep_ms},
+                "clocks": clocks, "e2e": None, "gpu_launches": int(launches)}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main(argv=None):
     args = parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
+    if args.slabs > 1:
+        return run_slabs(args)
     return run_ours(args)
 
 

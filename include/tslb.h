@@ -225,6 +225,19 @@ int tslb_radial_statistics(tslb_ctx *ctx, double xc, double yc, double dr, int n
 size_t tslb_face_bytes(const tslb_ctx *ctx);
 int tslb_export_face(tslb_ctx *ctx, int face, void *dev_dst, void *stream);
 int tslb_import_face(tslb_ctx *ctx, int face, const void *dev_src, void *stream);
+/* Zero-copy form of the same exchange, for transports that can read and write the workspace in place (NCCL send / recv,
+ * peer-to-peer or same-device copies): where the two planes of an EXCHANGE face live in the CURRENT moment buffer.
+ * *dev_owned / *dev_ghost: field 0 of the outermost owned plane / of the ghost plane; field f of either starts
+ * f * *field_stride_bytes further on and is one contiguous run of *plane_bytes bytes (the plane's rows with their padding and
+ * ghost columns).  Two contexts with the same nx, ny and dtype have the same plane layout, so copying the
+ * ten runs of a neighbour's owned plane onto this context's ghost plane is the whole exchange: no staging, ghost columns
+ * included.  Before returning, the call enqueues on `stream` whatever completes the owned plane for the current time (fill
+ * of lateral open-face nodes, ghost-column refresh).  The pointers are valid until the next tslb_step / set_moments /
+ * import_state of this context (the buffers ping-pong): ask again after every step.  The ghost plane must be written
+ * before the next tslb_step and after the sweep that precedes it has finished (stream order does that).
+ * Same error codes as tslb_export_face. */
+int tslb_face_planes(tslb_ctx *ctx, int face, void **dev_owned, void **dev_ghost, size_t *plane_bytes,
+                     size_t *field_stride_bytes, void *stream);
 
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);

@@ -27,7 +27,7 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
            "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics",
-           "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face")
+           "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face", "tslb_face_planes")
 PLANE_STATISTICS_STATIC_MAX = 1024   # TSLB_PLANE_STATISTICS_STATIC_MAX of include/tslb.h
 
 
@@ -82,6 +82,7 @@ def load_library(path: Optional[str] = None):
     lib.tslb_face_bytes.restype = C.c_size_t
     lib.tslb_export_face.argtypes = [vp, ip, vp, vp]
     lib.tslb_import_face.argtypes = [vp, ip, vp, vp]
+    lib.tslb_face_planes.argtypes = [vp, ip, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
@@ -165,6 +166,7 @@ class TSLB:
         self._chk(self._lib.tslb_bind_workspace(self._h, C.c_void_p(workspace.data_ptr()), workspace.numel()),
                   "tslb_bind_workspace")
         self._keep["ws"] = workspace
+        self._keep.pop("ws_typed", None)
 
     def set_moments(self, M, stream=None):
         """M: CUDA tensor [10][nz][ny][nx] of the context dtype."""
@@ -258,6 +260,22 @@ class TSLB:
         self._check_tensor(plane, "plane", (10,) + self.shape[1:])
         self._chk(self._lib.tslb_import_face(self._h, int(face), C.c_void_p(plane.data_ptr()), _stream_ptr(stream)), "tslb_import_face")
 
+    def face_planes(self, face: int, stream=None):
+        """tslb_face_planes as two tensors [10][plane elements] that alias the workspace: (outermost owned plane, ghost plane)
+        of the EXCHANGE face `face` in the current buffer; row f is contiguous.  Valid until the next step of this context."""
+        import torch
+        owned, ghost, pb, fs = C.c_void_p(), C.c_void_p(), C.c_size_t(), C.c_size_t()
+        self._chk(self._lib.tslb_face_planes(self._h, int(face), C.byref(owned), C.byref(ghost), C.byref(pb), C.byref(fs),
+                                             _stream_ptr(stream)), "tslb_face_planes")
+        ws = self._keep["ws"]
+        es = 4 if self.dtype == "f32" else 8
+        typed = self._keep.get("ws_typed")
+        if typed is None:
+            typed = self._keep["ws_typed"] = ws[: ws.numel() - ws.numel() % es].view(self.torch_dtype)
+        view = lambda ptr: torch.as_strided(typed, (10, pb.value // es), (fs.value // es, 1),
+                                            typed.storage_offset() + (ptr.value - typed.data_ptr()) // es)
+        return view(owned), view(ghost)
+
     def diagnostics(self, stream=None):
         """(mass, px, py, pz, kinetic energy) as a CUDA fp64 tensor of 5."""
         import torch
@@ -285,7 +303,7 @@ class TSLB:
         if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == (13, n_axis)):
             raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
         self._chk(self._lib.tslb_plane_statistics_static(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
-                  "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face")
+                  "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face", "tslb_face_planes")
         return sums
 
     def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums=None, stream=None):

@@ -458,6 +458,25 @@ int tslb_import_face(tslb_ctx *c, int face, const void *dev_src, void *stream)
     return TSLB_OK;
 }
 
+int tslb_face_planes(tslb_ctx *c, int face, void **dev_owned, void **dev_ghost, size_t *plane_bytes,
+                     size_t *field_stride_bytes, void *stream)
+{
+    int rc = face_check(c, face, dev_owned);
+    if (rc) return rc;
+    if (!dev_ghost || !plane_bytes || !field_stride_bytes) return fail(c, TSLB_EINVAL, "NULL output argument");
+    const char *why = "";
+    cudaError_t e = refresh_boundary(c, pick_kernel(c, &why) == TSLB_KERNEL_TILE, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "fill/halo kernel", e);
+    const size_t es = tslb_elem(c);
+    char *base = (char *)c->buf[c->cur];
+    const int zo = face == TSLB_FACE_ZLO ? 1 : c->nz - 2, zg = face == TSLB_FACE_ZLO ? 0 : c->nz - 1;
+    *dev_owned = base + (size_t)zo * c->L.plane * es;
+    *dev_ghost = base + (size_t)zg * c->L.plane * es;
+    *plane_bytes = (size_t)c->L.plane * es;
+    *field_stride_bytes = (size_t)c->L.field * es;
+    return TSLB_OK;
+}
+
 int tslb_diagnostics(tslb_ctx *c, double *dev_out5, void *stream)
 {
     int rc = check_ready(c, true);

@@ -4,7 +4,8 @@ Host-side orchestration only: every number is produced by the kernels behind the
 [z_lo, z_hi) of the global lattice in a context of its own (`binding.TSLB`) whose z axis carries one ghost plane per cut
 face (face kind BC_EXCHANGE, include/tslb.h "Slab decomposition").  One step is
 
-    sweep of the slab (tslb_step)  ->  tslb_export_face of the outermost owned planes  ->  transport  ->  tslb_import_face
+    sweep of the slab (tslb_step)  ->  transport of the outermost owned planes into the neighbours' ghost planes
+    (zero copy: in place in the workspaces, tslb_face_planes; or staged: tslb_export_face -> transport -> tslb_import_face)
 
 and because a sweep reads time-t nearest neighbours only (PAPER.md:68 Eq. 6, :157), the owned planes advance bit for bit
 as in the undivided lattice.  Transport: `torch.distributed` point-to-point (NCCL over NVLink / NVSwitch: one 40 B/node
@@ -125,43 +126,51 @@ def local_workload(w: W.Workload, plan: SlabPlan) -> W.Workload:
                                moments=np.ascontiguousarray(w.moments[:, zs]), faces=faces, inlet=inlet, sponge=sponge)
 
 
+def _chunks(t):
+    return [] if t is None else (list(t) if isinstance(t, (list, tuple)) else [t])
+
+
 def exchange_planes(plan: SlabPlan, send_lo, send_hi, recv_lo, recv_hi, group=None) -> None:
     """Point-to-point exchange of the cut-face planes with the neighbouring ranks (any device `torch.distributed` serves:
     NCCL for CUDA tensors, gloo for CPU ones).  send_lo / send_hi: this rank's outermost owned planes; recv_lo / recv_hi:
-    what becomes its ghost planes.  With two ranks on a periodic axis both neighbours are the same peer: messages between
-    a pair are matched in the order they are issued (NCCL has no tags), so the low plane is always sent first and the
-    matching receive -- the neighbour's LOW plane is this rank's HIGH ghost -- is issued first."""
+    what becomes its ghost planes; each a contiguous tensor or a list of contiguous chunks (the ten field runs of a plane
+    inside the workspace, for the zero-copy path).  With two ranks on a periodic axis both neighbours are the same peer:
+    messages between a pair are matched in the order they are issued (NCCL has no tags), so the low plane is always sent
+    first and the matching receive -- the neighbour's LOW plane is this rank's HIGH ghost -- is issued first."""
     import torch.distributed as dist
     ops = []
     if plan.ghost_lo:
-        ops.append(dist.P2POp(dist.isend, send_lo, plan.lo_rank, group, tag=0))
+        ops += [dist.P2POp(dist.isend, c, plan.lo_rank, group, tag=i) for i, c in enumerate(_chunks(send_lo))]
     if plan.ghost_hi:
-        ops.append(dist.P2POp(dist.isend, send_hi, plan.hi_rank, group, tag=1))
+        ops += [dist.P2POp(dist.isend, c, plan.hi_rank, group, tag=64 + i) for i, c in enumerate(_chunks(send_hi))]
     if plan.ghost_hi:
-        ops.append(dist.P2POp(dist.irecv, recv_hi, plan.hi_rank, group, tag=0))
+        ops += [dist.P2POp(dist.irecv, c, plan.hi_rank, group, tag=i) for i, c in enumerate(_chunks(recv_hi))]
     if plan.ghost_lo:
-        ops.append(dist.P2POp(dist.irecv, recv_lo, plan.lo_rank, group, tag=1))
+        ops += [dist.P2POp(dist.irecv, c, plan.lo_rank, group, tag=64 + i) for i, c in enumerate(_chunks(recv_lo))]
     if ops:
         for req in dist.batch_isend_irecv(ops):
             req.wait()
 
 
 class Slab:
-    """One rank's part of a slab-decomposed lattice on the current CUDA device."""
+    """One rank's part of a slab-decomposed lattice on the current CUDA device.  staged = False (default): the transport
+    reads the owned planes and writes the ghost planes in place in the workspace (tslb_face_planes, zero copy);
+    staged = True: through dense arrays (tslb_export_face / tslb_import_face)."""
 
-    def __init__(self, w: W.Workload, plan: SlabPlan, kernel: int = 0):
+    def __init__(self, w: W.Workload, plan: SlabPlan, kernel: int = 0, staged: bool = False):
         import torch
         from . import binding
         self.plan = plan
+        self.staged = staged
         self.local = local_workload(w, plan)
         self.sim = binding.from_workload(self.local, kernel)
         self.sim.set_moments(torch.from_numpy(self.local.moments).to("cuda"))
         shape = (10, w.ny, w.nx)
         mk = lambda: torch.empty(shape, dtype=self.sim.torch_dtype, device="cuda")
-        self.send_lo, self.recv_lo = (mk(), mk()) if plan.ghost_lo else (None, None)
-        self.send_hi, self.recv_hi = (mk(), mk()) if plan.ghost_hi else (None, None)
+        self.send_lo, self.recv_lo = (mk(), mk()) if plan.ghost_lo and staged else (None, None)
+        self.send_hi, self.recv_hi = (mk(), mk()) if plan.ghost_hi and staged else (None, None)
 
-    # the three phases of one exchange (tslb_export_face / transport / tslb_import_face)
+    # staged path: the three phases of one exchange (tslb_export_face / transport / tslb_import_face)
     def export_faces(self, stream=None):
         if self.plan.ghost_lo:
             self.sim.export_face(W.FACE_ZLO, self.send_lo, stream)
@@ -174,10 +183,21 @@ class Slab:
         if self.plan.ghost_hi:
             self.sim.import_face(W.FACE_ZHI, self.recv_hi, stream)
 
+    # zero-copy path: (owned_lo, ghost_lo, owned_hi, ghost_hi) as views [10][plane] of the workspace, None where uncut
+    def planes(self, stream=None):
+        olo, glo = self.sim.face_planes(W.FACE_ZLO, stream) if self.plan.ghost_lo else (None, None)
+        ohi, ghi = self.sim.face_planes(W.FACE_ZHI, stream) if self.plan.ghost_hi else (None, None)
+        return olo, glo, ohi, ghi
+
     def exchange(self, group=None):
-        self.export_faces()
-        exchange_planes(self.plan, self.send_lo, self.send_hi, self.recv_lo, self.recv_hi, group)
-        self.import_faces()
+        if self.staged:
+            self.export_faces()
+            exchange_planes(self.plan, self.send_lo, self.send_hi, self.recv_lo, self.recv_hi, group)
+            self.import_faces()
+        else:
+            rows = lambda v: None if v is None else [v[f] for f in range(v.shape[0])]     # ten contiguous runs
+            olo, glo, ohi, ghi = self.planes()
+            exchange_planes(self.plan, rows(olo), rows(ohi), rows(glo), rows(ghi), group)
 
     def step(self, n: int = 1, group=None):
         """n time steps of the whole lattice as seen from this rank (collective: every rank calls it)."""
@@ -202,17 +222,26 @@ class Slab:
 
 
 def exchange_local(slabs: Sequence[Slab]) -> None:
-    """The exchange between slabs that live in one process on one GPU: export everywhere, then copy plane to plane on the
-    current stream, then import.  Serial launches of one stream: no kernel ever waits on another."""
-    for s in slabs:
-        s.export_faces()
-    for s in slabs:
+    """The exchange between slabs that live in one process on one GPU: plane-to-plane device copies on the current stream
+    (zero-copy path: straight from workspace to workspace; staged path: export everywhere, copy, import).  Serial launches
+    of one stream: no kernel ever waits on another."""
+    if slabs and slabs[0].staged:
+        for s in slabs:
+            s.export_faces()
+        for s in slabs:
+            if s.plan.ghost_lo:
+                s.recv_lo.copy_(slabs[s.plan.lo_rank].send_hi)
+            if s.plan.ghost_hi:
+                s.recv_hi.copy_(slabs[s.plan.hi_rank].send_lo)
+        for s in slabs:
+            s.import_faces()
+        return
+    views = [s.planes() for s in slabs]                    # also completes every owned plane for the current time
+    for s, (_, glo, _, ghi) in zip(slabs, views):
         if s.plan.ghost_lo:
-            s.recv_lo.copy_(slabs[s.plan.lo_rank].send_hi)
+            glo.copy_(views[s.plan.lo_rank][2])            # the HIGH owned plane of the slab below
         if s.plan.ghost_hi:
-            s.recv_hi.copy_(slabs[s.plan.hi_rank].send_lo)
-    for s in slabs:
-        s.import_faces()
+            ghi.copy_(views[s.plan.hi_rank][0])            # the LOW owned plane of the slab above
 
 
 def step_local(slabs: Sequence[Slab], n: int = 1) -> None:

@@ -17,10 +17,10 @@ from tests.test_gpu_parity import BC_SETS, B, kernels_for, with_faces  # noqa: F
 pytestmark = pytest.mark.gpu
 
 
-def run_slabs(w, world, steps, kernel):
+def run_slabs(w, world, steps, kernel, staged=False):
     import torch
     periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
-    slabs = [S.Slab(w, p, kernel) for p in S.plan_slabs(w.nz, world, periodic_z)]
+    slabs = [S.Slab(w, p, kernel, staged) for p in S.plan_slabs(w.nz, world, periodic_z)]
     S.step_local(slabs, steps)
     G = S.gather_local(slabs)
     torch.cuda.synchronize()
@@ -55,7 +55,11 @@ def test_slabs_match_oracle_and_undivided_run(B, oracle_mod, case, world, dtype)
     o.step(steps)
     R = o.get_moments()
     for k in kernels_for(B, w):
-        slabs, G = run_slabs(w, world, steps, k)
+        slabs_st, G_st = run_slabs(w, world, steps, k, staged=True)        # tslb_export_face / tslb_import_face
+        slabs, G = run_slabs(w, world, steps, k)                           # tslb_face_planes (zero copy)
+        assert np.array_equal(G, G_st)
+        for s in slabs_st:
+            s.sim.close()
         assert all(s.sim.step_count == steps for s in slabs)
         assert_parity(w, G.astype(np.float64), R, "%s, %d slabs, kernel %d" % (case, world, k))
         one = make_gpu(w, k)

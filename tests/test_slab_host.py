@@ -84,16 +84,21 @@ mk = lambda v: torch.full(shape, float(v))
 # plane value = 10 * owner + (0 low plane | 1 high plane)
 send_lo, send_hi = mk(10 * rank), mk(10 * rank + 1)
 recv_lo, recv_hi = mk(-1), mk(-1)
+chunked = sys.argv[4] == "1"        # the zero-copy path hands over the ten field runs of a plane one by one
+if chunked:
+    send_lo += torch.arange(10.0).view(10, 1, 1) / 100; send_hi += torch.arange(10.0).view(10, 1, 1) / 100
+rows = lambda t: [t[f] for f in range(10)] if chunked else t
 for it in range(3):            # several exchanges in a row: the pairing must not drift
-    S.exchange_planes(plan, send_lo if plan.ghost_lo else None, send_hi if plan.ghost_hi else None,
-                      recv_lo if plan.ghost_lo else None, recv_hi if plan.ghost_hi else None)
+    S.exchange_planes(plan, rows(send_lo) if plan.ghost_lo else None, rows(send_hi) if plan.ghost_hi else None,
+                      rows(recv_lo) if plan.ghost_lo else None, rows(recv_hi) if plan.ghost_hi else None)
     other = 1 - rank
+    field = (torch.arange(10.0).view(10, 1, 1) / 100) if chunked else 0.0
     if plan.ghost_lo:          # my low ghost plane is the HIGH plane of the rank below
-        assert (recv_lo == 10 * other + 1).all(), (rank, it, recv_lo.flatten()[0])
+        assert (recv_lo == 10 * other + 1 + field).all(), (rank, it, recv_lo.flatten()[0])
     else:
         assert (recv_lo == -1).all()
     if plan.ghost_hi:          # my high ghost plane is the LOW plane of the rank above
-        assert (recv_hi == 10 * other).all(), (rank, it, recv_hi.flatten()[0])
+        assert (recv_hi == 10 * other + field).all(), (rank, it, recv_hi.flatten()[0])
     else:
         assert (recv_hi == -1).all()
     recv_lo.fill_(-1); recv_hi.fill_(-1)
@@ -102,15 +107,16 @@ print("ok", rank)
 """
 
 
+@pytest.mark.parametrize("chunked", [False, True])
 @pytest.mark.parametrize("periodic", [True, False])
-def test_exchange_planes_world_size_2_gloo(tmp_path, periodic):
+def test_exchange_planes_world_size_2_gloo(tmp_path, periodic, chunked):
     """Two ranks: on a periodic axis both neighbours are the same peer (the pairing of the two messages is what can go
     wrong); on a bounded axis each rank has one neighbour only."""
     import socket
     s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
     script = tmp_path / "worker.py"
     script.write_text(WORKER % ROOT)
-    procs = [subprocess.Popen([sys.executable, str(script), str(r), str(port), "1" if periodic else "0"],
+    procs = [subprocess.Popen([sys.executable, str(script), str(r), str(port), "1" if periodic else "0", "1" if chunked else "0"],
                               stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for r in range(2)]
     outs = [p.communicate(timeout=240)[0] for p in procs]
     for p, o in zip(procs, outs):
