@@ -50,6 +50,9 @@ def parse_args(argv=None):
                          "scaling); on one GPU all slabs on it with device-copy exchange (cost of the decomposition path)")
     ap.add_argument("--staged", action="store_true",
                     help="with --slabs: ghost planes through tslb_export_face / tslb_import_face instead of in place (tslb_face_planes)")
+    ap.add_argument("--connected", action="store_true",
+                    help="with --slabs on one GPU: no exchange at all, the tile kernel reads the neighbouring slabs' planes in place "
+                         "(tslb_set_neighbor)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
@@ -392,9 +395,16 @@ def run_slabs(args):
     owned_sites = float(sum(s.plan.owned for s in slabs)) * w.nx * w.ny
     stream = torch.cuda.current_stream()
 
+    if args.connected:
+        if world > 1:
+            raise SystemExit("bench.py: --connected needs the slabs in one process (mutually addressable buffers)")
+        S.connect_local(slabs)
+
     def advance(n):
         if world > 1:
             slabs[0].step(n)
+        elif args.connected:
+            S.step_connected(slabs, n)
         else:
             S.step_local(slabs, n)
 
@@ -442,7 +452,8 @@ def run_slabs(args):
         cfg["parallelism"] = ("one lattice in %d z slabs, " % args.slabs) + (
             "one slab per GPU, ghost planes by NCCL point-to-point" if world > 1 else "all on one GPU, ghost planes by device copies")
         cfg["slab_planes"] = [p.owned for p in plans]
-        cfg["transport"] = "staged (tslb_export_face / tslb_import_face)" if args.staged else "in place (tslb_face_planes)"
+        cfg["transport"] = ("none: neighbours read in place by the sweep's TMA producer (tslb_set_neighbor)" if args.connected else
+                            "staged (tslb_export_face / tslb_import_face)" if args.staged else "in place (tslb_face_planes)")
         line = {"metric": "GLUPS", "value": glups(units, ms_max), "unit": "GLUPS", "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong",
                 "vs_baseline": None, "dtype": args.dtype, "data": "synthetic", "config": cfg,

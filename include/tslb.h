@@ -239,6 +239,30 @@ int tslb_import_face(tslb_ctx *ctx, int face, const void *dev_src, void *stream)
 int tslb_face_planes(tslb_ctx *ctx, int face, void **dev_owned, void **dev_ghost, size_t *plane_bytes,
                      size_t *field_stride_bytes, void *stream);
 
+/* Fused form of the exchange: no exchange at all.  After tslb_set_neighbor the tile kernel's TMA producer loads the source
+ * plane ON the EXCHANGE face `face` -- this context's ghost plane -- straight from the neighbouring slab's current moment
+ * buffer (its outermost owned plane), tile by tile while it sweeps: peer memory over NVLink when the neighbour lives on another
+ * GPU (peer access enabled, or its buffers mapped through CUDA IPC), plain global memory when it lives on the same one.  The
+ * ghost plane of this context is then never read and nothing has to be copied between steps.
+ *   peer_buf   the neighbour's two moment buffers as tslb_buffers reports them (addresses valid on THIS device), or NULL to
+ *              detach (back to tslb_import_face / tslb_face_planes);
+ *   peer_nz    the neighbour context's nz (its own ghost planes included); nx, ny and dtype must equal this context's;
+ *   peer_cur   which of the two buffers holds the neighbour's current time level now.
+ * Contract: from here on both contexts take their steps in lockstep (tslb_step(n = 1) on each, then the next step), so
+ * that the neighbour's current buffer alternates with this context's; the caller orders the work so that (a) the neighbour's
+ * state of time t is complete (its sweep of the previous step has finished and tslb_refresh has run on it) before this
+ * context's sweep of step t starts, and (b) that sweep has finished before the neighbour's sweep of step t+1 starts (it
+ * overwrites the buffer being read): one stream, or one barrier per step between neighbours.  tslb_set_moments,
+ * tslb_import_state and tslb_bind_workspace detach every neighbour.  Tile kernel only: tslb_step fails with TSLB_EINVAL if
+ * the gather kernel would run while a neighbour is attached.
+ * TSLB_EINVAL: face not ZLO / ZHI or not EXCHANGE, peer_nz < 3, peer_cur not 0 / 1, NULL buffer; TSLB_ESTATE: no state;
+ * TSLB_ECUDA: the TMA descriptors could not be built. */
+int tslb_buffers(const tslb_ctx *ctx, void *dev_buf[2], int *cur);
+int tslb_set_neighbor(tslb_ctx *ctx, int face, void *const peer_buf[2], int peer_nz, int peer_cur);
+/* Enqueue on `stream` whatever completes the current state (open-face boundary nodes of the current time, ghost columns):
+ * what tslb_step does first.  For callers that let another context read this one's planes (tslb_set_neighbor). */
+int tslb_refresh(tslb_ctx *ctx, void *stream);
+
 /* Steps taken since the last set_moments, or -1. */
 long long tslb_step_count(const tslb_ctx *ctx);
 /* Number of kernels this context has launched so far (all kinds), for bench.py's gpu_launches. */

@@ -27,7 +27,8 @@ SYMBOLS = ("tslb_create", "tslb_destroy", "tslb_workspace_bytes", "tslb_bind_wor
            "tslb_get_moments", "tslb_get_moments_host", "tslb_diagnostics", "tslb_step_count",
            "tslb_launch_count", "tslb_last_error", "tslb_version", "tslb_set_timing", "tslb_get_timing", "tslb_set_order", "tslb_plane_statistics",
            "tslb_export_state", "tslb_import_state", "tslb_set_sponge", "tslb_radial_statistics",
-           "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face", "tslb_face_planes")
+           "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face", "tslb_face_planes",
+           "tslb_buffers", "tslb_set_neighbor", "tslb_refresh")
 PLANE_STATISTICS_STATIC_MAX = 1024   # TSLB_PLANE_STATISTICS_STATIC_MAX of include/tslb.h
 
 
@@ -83,6 +84,9 @@ def load_library(path: Optional[str] = None):
     lib.tslb_export_face.argtypes = [vp, ip, vp, vp]
     lib.tslb_import_face.argtypes = [vp, ip, vp, vp]
     lib.tslb_face_planes.argtypes = [vp, ip, C.POINTER(vp), C.POINTER(vp), C.POINTER(C.c_size_t), C.POINTER(C.c_size_t), vp]
+    lib.tslb_buffers.argtypes = [vp, C.POINTER(vp), C.POINTER(ip)]
+    lib.tslb_set_neighbor.argtypes = [vp, ip, C.POINTER(vp), ip, ip]
+    lib.tslb_refresh.argtypes = [vp, vp]
     lib.tslb_set_timing.argtypes = [vp, ip]
     lib.tslb_get_timing.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
     lib.tslb_step_count.argtypes = [vp]
@@ -276,6 +280,24 @@ class TSLB:
                                             typed.storage_offset() + (ptr.value - typed.data_ptr()) // es)
         return view(owned), view(ghost)
 
+    def buffers(self):
+        """(address of moment buffer 0, of buffer 1, index of the one that holds the current time level)."""
+        arr, cur = (C.c_void_p * 2)(), C.c_int(0)
+        self._chk(self._lib.tslb_buffers(self._h, arr, C.byref(cur)), "tslb_buffers")
+        return int(arr[0]), int(arr[1]), cur.value
+
+    def set_neighbor(self, face: int, peer_bufs=None, peer_nz: int = 0, peer_cur: int = 0):
+        """tslb_set_neighbor: read the ghost plane of the EXCHANGE face `face` in place from the neighbouring slab's buffers
+        (two addresses valid on this device, as the neighbour's buffers() reports them); peer_bufs = None detaches."""
+        if peer_bufs is None:
+            self._chk(self._lib.tslb_set_neighbor(self._h, int(face), None, 0, 0), "tslb_set_neighbor")
+            return
+        arr = (C.c_void_p * 2)(C.c_void_p(int(peer_bufs[0])), C.c_void_p(int(peer_bufs[1])))
+        self._chk(self._lib.tslb_set_neighbor(self._h, int(face), arr, int(peer_nz), int(peer_cur)), "tslb_set_neighbor")
+
+    def refresh(self, stream=None):
+        self._chk(self._lib.tslb_refresh(self._h, _stream_ptr(stream)), "tslb_refresh")
+
     def diagnostics(self, stream=None):
         """(mass, px, py, pz, kinetic energy) as a CUDA fp64 tensor of 5."""
         import torch
@@ -303,7 +325,7 @@ class TSLB:
         if not (sums.is_cuda and sums.dtype == torch.float64 and sums.is_contiguous() and tuple(sums.shape) == (13, n_axis)):
             raise ValueError("sums must be a contiguous CUDA float64 tensor of shape (13, %d)" % n_axis)
         self._chk(self._lib.tslb_plane_statistics_static(self._h, int(axis), C.c_void_p(sums.data_ptr()), _stream_ptr(stream)),
-                  "tslb_plane_statistics_static", "tslb_face_bytes", "tslb_export_face", "tslb_import_face", "tslb_face_planes")
+                  "tslb_plane_statistics_static")
         return sums
 
     def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums=None, stream=None):

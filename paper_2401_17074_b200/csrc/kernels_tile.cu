@@ -29,6 +29,7 @@
 // passes.  A pass with taps (t-, t0, t+) applied to B*u gives (t- + t0 + t+) B u(x) + B [t- (u(x-1) - u(x)) + t+ (u(x+1) - u(x))];
 // only the bracket (exact differences of stored velocities) is added at each stage, and the product of the tap sums,
 // 216 u_a(x), is re-attached in closed form at the end:  u' = u + (J_small - u dR) / (216 + dR).
+#include <string.h>
 #include <type_traits>
 #include "tslb_internal.h"
 
@@ -170,6 +171,15 @@ struct TileParams {
     const T *beta_z;   // sponge layer (Eq. 26): 1 - omega of the nodes of plane z, [nz] (SPONGE instantiations only)
     int zchunk;  // planes per z chunk
     int fuse;    // the store warp writes the open-face boundary nodes of time t+1 itself (FUSE instantiations)
+};
+// Slab neighbours read in place (tslb_set_neighbor, include/tslb.h): the source plane ON an EXCHANGE face -- the ghost plane of
+// a slab -- is loaded by TMA straight from the neighbouring slab's current buffer (its outermost owned plane: peer memory over
+// NVLink, or the same device) instead of from this lattice's ghost plane.  Same plane layout (equal nx, ny, dtype), so the
+// boxes, the halo rows and the ghost columns are those of the peer's plane.
+struct NbParams {
+    CUtensorMap main[2], row[2];   // [0]: the slab below (face ZLO), [1]: the slab above (face ZHI); the peer's CURRENT buffer
+    int on[2];
+    int z[2];                      // the peer's outermost owned plane on that side
 };
 // fused boundary fill (a6): what the store warp needs to impose inlet velocities / outlet densities
 struct FuseParams {
@@ -418,7 +428,8 @@ __device__ __noinline__ void tile_impose(const FuseParams &p, uint32_t a, uint32
 template <typename T, int WALL, int ORDER, bool SPONGE, bool FUSE, int GEO>
 __global__ void __maxnreg__((TileDims<T, GEO>::MAXREG))
 sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_constant__ CUtensorMap tmRow,
-                  const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p, const __grid_constant__ FuseParams fp)
+                  const __grid_constant__ CUtensorMap tmStore, T *__restrict__ Bbuf, TileParams<T> p, const __grid_constant__ FuseParams fp,
+                  const __grid_constant__ NbParams nb)
 {
     typedef typename PackOf<T>::type P;
     typedef TileDims<T, GEO> TD;
@@ -600,9 +611,13 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
                 if (j >= NS) mbar_wait(sb + B_EMPTY + 8 * s, (uint32_t)((j / NS - 1) & 1));
                 const uint32_t dst = sb + s * STAGE_BYTES, bar = sb + B_FULL + 8 * s;
                 mbar_expect_tx(bar, (uint32_t)TD::STAGE_TX);
-                tma_load_4d(dst, &tmMain, bar, x0, row0, zs, 0);
-                tma_load_4d(dst + TD::MAIN_ELEMS * ES, &tmRow, bar, x0, ylo, zs, 0);
-                tma_load_4d(dst + (TD::MAIN_ELEMS + TD::HALO_ELEMS) * ES, &tmRow, bar, x0, yhi, zs, 0);
+                // the ghost plane of a slab whose neighbour is attached: the neighbour's own plane, in place
+                const CUtensorMap *mm = &tmMain, *mr = &tmRow;
+                if (zs == 0 && nb.on[0]) { mm = &nb.main[0]; mr = &nb.row[0]; zs = nb.z[0]; }
+                else if (zs == L.nz - 1 && nb.on[1]) { mm = &nb.main[1]; mr = &nb.row[1]; zs = nb.z[1]; }
+                tma_load_4d(dst, mm, bar, x0, row0, zs, 0);
+                tma_load_4d(dst + TD::MAIN_ELEMS * ES, mr, bar, x0, ylo, zs, 0);
+                tma_load_4d(dst + (TD::MAIN_ELEMS + TD::HALO_ELEMS) * ES, mr, bar, x0, yhi, zs, 0);
             }
         } else {
             // output plane m of this chunk (z = z0 + m) sits in output tile m % NOUT; its k-th use completes phase k of the
@@ -1370,6 +1385,54 @@ cudaError_t tslb_tile_prepare(tslb_ctx *c)
     return cudaSuccess;
 }
 
+// Neighbour slabs (tslb_set_neighbor): load descriptors over the peer's two moment buffers (its own nz, same nx / ny / dtype).
+cudaError_t tslb_tile_prepare_neighbor(tslb_ctx *c, int side)
+{
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    const Layout &L = c->L;
+    const size_t es = tslb_elem(c);
+    const bool f64 = c->dtype == TSLB_F64;
+    const cuuint32_t bxw = f64 ? TileDims<double>::BXW : TileDims<float>::BXW;
+    const cuuint32_t rows_g[2] = {(cuuint32_t)(f64 ? TileDims<double>::ROWS : TileDims<float, 0>::ROWS),
+                                  (cuuint32_t)(f64 ? TileDims<double>::ROWS : TileDims<float, 1>::ROWS)};
+    const long long pnz = c->nb_nz[side];
+    const cuuint64_t strides[3] = {(cuuint64_t)L.px * es, (cuuint64_t)L.plane * es, (cuuint64_t)L.plane * pnz * es};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint64_t dims_ld[4] = {(cuuint64_t)L.px, (cuuint64_t)L.ny, (cuuint64_t)pnz, TSLB_NF};
+    for (int g = 0; g < 2; ++g)
+    for (int b = 0; b < 2; ++b) {
+        const cuuint32_t box_main[4] = {bxw, rows_g[g], 1, TSLB_NF}, box_row[4] = {bxw, 1, 1, TSLB_NF};
+        CUresult r = ((EncodeTiledFn)fn)(&c->nb_main[side][g][b], dt, 4, c->nb_buf[side][b], dims_ld, strides, box_main, estr,
+                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r == CUDA_SUCCESS)
+            r = ((EncodeTiledFn)fn)(&c->nb_row[side][g][b], dt, 4, c->nb_buf[side][b], dims_ld, strides, box_row, estr,
+                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, TSLB_L2PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    return cudaSuccess;
+}
+
+static NbParams make_nb(const tslb_ctx *c, int geo)
+{
+    NbParams nb;
+    memset(&nb, 0, sizeof nb);
+    for (int s = 0; s < 2; ++s) {
+        if (!c->nb_on[s]) continue;
+        // the peer alternates its buffers in lockstep with this context (include/tslb.h)
+        const int b = (int)((c->nb_cur0[s] + (c->t - c->nb_t0[s])) & 1);
+        nb.on[s] = 1;
+        nb.main[s] = c->nb_main[s][geo][b];
+        nb.row[s] = c->nb_row[s][geo][b];
+        nb.z[s] = s == 0 ? c->nb_nz[s] - 2 : 1;
+    }
+    return nb;
+}
+
 template <typename T, int WALLY, int ORDER, int GEO>
 static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
 {
@@ -1381,9 +1444,10 @@ static void launch_tile_geo(tslb_ctx *c, cudaStream_t st)
     fp.L = c->L;
     fp.tnext = c->t + 1;
     for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
+    const NbParams nb = make_nb(c, GEO);
 #define TSLB_TILE_LAUNCH(S, F)                                                                                                            \
     sweep_tile_kernel<T, WALLY, ORDER, S, F, GEO><<<grid, TileDims<T, GEO>::THREADS, TileDims<T, GEO>::SMEM_BYTES, st>>>(                    \
-        c->tm_main[GEO][a], c->tm_row[GEO][a], c->tm_store[GEO][b], (T *)c->buf[b], p, fp)
+        c->tm_main[GEO][a], c->tm_row[GEO][a], c->tm_store[GEO][b], (T *)c->buf[b], p, fp, nb)
     if (p.beta_z) { if (p.fuse) TSLB_TILE_LAUNCH(true, true); else TSLB_TILE_LAUNCH(true, false); }
     else { if (p.fuse) TSLB_TILE_LAUNCH(false, true); else TSLB_TILE_LAUNCH(false, false); }
 #undef TSLB_TILE_LAUNCH
@@ -1403,8 +1467,9 @@ static void launch_tile_zwall(tslb_ctx *c, cudaStream_t st)
     fp.L = c->L;
     fp.tnext = c->t + 1;
     for (int f = 0; f < 6; ++f) { fp.kind[f] = c->kind[f]; fp.inlet[f] = c->inlet[f]; fp.rho_out[f] = c->rho_out[f]; }
+    const NbParams nb = make_nb(c, 0);
     sweep_tile_kernel<T, WALLV, ORDER, false, false, 0><<<grid, TileDims<T, 0>::THREADS, TileDims<T, 0>::SMEM_BYTES, st>>>(
-        c->tm_main[0][a], c->tm_row[0][a], c->tm_store[0][b], (T *)c->buf[b], p, fp);
+        c->tm_main[0][a], c->tm_row[0][a], c->tm_store[0][b], (T *)c->buf[b], p, fp, nb);
 }
 
 template <typename T, int WALLY, int ORDER>

@@ -201,6 +201,7 @@ int tslb_bind_workspace(tslb_ctx *c, void *dev_ptr, size_t bytes)
     c->beta_z = (char *)dev_ptr + 2 * buffer_bytes(c) + scratch_bytes(c);
     c->sponge_dirty = c->beta_z_host != nullptr;
     c->cur = 0; c->t = 0; c->have_state = 0; c->halo_valid = 0;
+    c->nb_on[0] = c->nb_on[1] = 0;
     // padding cells are never written by the kernels: give them a defined (zero) value once
     e = cudaMemset(dev_ptr, 0, 2 * buffer_bytes(c));
     if (e != cudaSuccess) return cuda_fail(c, "cudaMemset(workspace)", e);
@@ -226,6 +227,7 @@ int tslb_set_moments(tslb_ctx *c, const void *dev_src, void *stream)
     cudaError_t e = tslb_launch_import(c, dev_src, c->buf[0], (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
     c->cur = 0; c->t = 0; c->have_state = 1; c->halo_valid = 0;
+    c->nb_on[0] = c->nb_on[1] = 0;
     return TSLB_OK;
 }
 
@@ -243,6 +245,7 @@ int tslb_set_moments_host(tslb_ctx *c, const void *host_src, void *stream)
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(c, "cudaStreamSynchronize", e);
     c->cur = 0; c->t = 0; c->have_state = 1; c->halo_valid = 0;
+    c->nb_on[0] = c->nb_on[1] = 0;
     return TSLB_OK;
 }
 
@@ -341,6 +344,8 @@ int tslb_step(tslb_ctx *c, int n, void *stream)
     const char *why = "";
     const int k = pick_kernel(c, &why);
     if (k < 0) return fail(c, TSLB_EINVAL, "TSLB_KERNEL_TILE does not cover this configuration: %s", why);
+    if (k != TSLB_KERNEL_TILE && (c->nb_on[0] || c->nb_on[1]))
+        return fail(c, TSLB_EINVAL, "a neighbour is attached (tslb_set_neighbor) but the gather kernel would run: %s", why);
     cudaStream_t st = (cudaStream_t)stream;
     if (c->sponge_dirty) {               // per-plane relaxation table of the sponge layer
         cudaError_t e = cudaMemcpyAsync(c->beta_z, c->beta_z_host, (size_t)c->nz * tslb_elem(c), cudaMemcpyHostToDevice, st);
@@ -418,6 +423,7 @@ int tslb_import_state(tslb_ctx *c, const void *dev_src, long long step_count, vo
     cudaError_t e = tslb_launch_import_raw(c, dev_src, c->buf[0], (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(c, "import kernel", e);
     c->cur = 0; c->t = step_count; c->have_state = 1; c->halo_valid = 0;
+    c->nb_on[0] = c->nb_on[1] = 0;
     return TSLB_OK;
 }
 
@@ -474,6 +480,44 @@ int tslb_face_planes(tslb_ctx *c, int face, void **dev_owned, void **dev_ghost, 
     *dev_ghost = base + (size_t)zg * c->L.plane * es;
     *plane_bytes = (size_t)c->L.plane * es;
     *field_stride_bytes = (size_t)c->L.field * es;
+    return TSLB_OK;
+}
+
+int tslb_buffers(const tslb_ctx *c, void *dev_buf[2], int *cur)
+{
+    if (!c || !dev_buf || !cur) return TSLB_EINVAL;
+    if (!c->ws) return TSLB_ESTATE;
+    dev_buf[0] = c->buf[0]; dev_buf[1] = c->buf[1];
+    *cur = c->cur;
+    return TSLB_OK;
+}
+
+int tslb_set_neighbor(tslb_ctx *c, int face, void *const peer_buf[2], int peer_nz, int peer_cur)
+{
+    if (!c) return TSLB_EINVAL;
+    if (face != TSLB_FACE_ZLO && face != TSLB_FACE_ZHI) return fail(c, TSLB_EINVAL, "face must be TSLB_FACE_ZLO or TSLB_FACE_ZHI");
+    const int side = face == TSLB_FACE_ZLO ? 0 : 1;
+    if (!peer_buf) { c->nb_on[side] = 0; return TSLB_OK; }
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    if (c->kind[face] != TSLB_BC_EXCHANGE) return fail(c, TSLB_EINVAL, "face is not of kind TSLB_BC_EXCHANGE");
+    if (!peer_buf[0] || !peer_buf[1]) return fail(c, TSLB_EINVAL, "peer buffer == NULL");
+    if (peer_nz < 3 || (peer_cur != 0 && peer_cur != 1)) return fail(c, TSLB_EINVAL, "peer_nz < 3 or peer_cur not 0 / 1");
+    c->nb_buf[side][0] = peer_buf[0]; c->nb_buf[side][1] = peer_buf[1];
+    c->nb_nz[side] = peer_nz; c->nb_cur0[side] = peer_cur; c->nb_t0[side] = c->t;
+    cudaError_t e = tslb_tile_prepare_neighbor(c, side);
+    if (e != cudaSuccess) return cuda_fail(c, "TMA descriptors of the neighbour", e);
+    c->nb_on[side] = 1;
+    return TSLB_OK;
+}
+
+int tslb_refresh(tslb_ctx *c, void *stream)
+{
+    int rc = check_ready(c, true);
+    if (rc) return rc;
+    const char *why = "";
+    cudaError_t e = refresh_boundary(c, pick_kernel(c, &why) == TSLB_KERNEL_TILE, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(c, "fill/halo kernel", e);
     return TSLB_OK;
 }
 

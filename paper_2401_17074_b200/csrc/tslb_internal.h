@@ -112,6 +112,11 @@ struct tslb_ctx {
     int last_fused;      // the last tile launch wrote the open-face boundary nodes of its output itself (fused fill)
     CUtensorMap tm_main[2][2], tm_row[2][2], tm_store[2][2];  // TMA descriptors [tile geometry][buffer]: tile rows, one halo row, output tile
     int tmap_ok;
+    // neighbouring slabs read in place (tslb_set_neighbor): side 0 = below ZLO, 1 = above ZHI
+    int nb_on[2], nb_nz[2], nb_cur0[2];
+    long long nb_t0[2];              // this context's step count when the neighbour was attached
+    void *nb_buf[2][2];              // the peer's two moment buffers
+    CUtensorMap nb_main[2][2][2], nb_row[2][2][2];   // [side][tile geometry][peer buffer]
     int cur;          // buf[cur] holds time t
     long long t;
     int have_state;
@@ -136,6 +141,7 @@ static inline size_t tslb_sites(const tslb_ctx *c) { return (size_t)c->nx * c->n
 cudaError_t tslb_launch_gather(tslb_ctx *c, cudaStream_t st);
 cudaError_t tslb_launch_tile(tslb_ctx *c, cudaStream_t st);
 bool tslb_tile_supported(const tslb_ctx *c, const char **why);
+cudaError_t tslb_tile_prepare_neighbor(tslb_ctx *c, int side);                            // TMA descriptors over a neighbouring slab's buffers
 cudaError_t tslb_tile_prepare(tslb_ctx *c);                                               // TMA descriptors, smem opt-in
 cudaError_t tslb_launch_fill(tslb_ctx *c, void *buf, cudaStream_t st);                    // open-face boundary nodes at time t
 cudaError_t tslb_launch_halo(tslb_ctx *c, void *buf, cudaStream_t st);                    // ghost layers

@@ -7,6 +7,9 @@ face (face kind BC_EXCHANGE, include/tslb.h "Slab decomposition").  One step is
     sweep of the slab (tslb_step)  ->  transport of the outermost owned planes into the neighbours' ghost planes
     (zero copy: in place in the workspaces, tslb_face_planes; or staged: tslb_export_face -> transport -> tslb_import_face)
 
+or, where the slabs' buffers are mutually addressable (one process; `connect_local` / `step_connected`), no transport at
+all: the tile kernel's TMA producer loads the ghost planes from the neighbours' buffers while it sweeps (tslb_set_neighbor)
+
 and because a sweep reads time-t nearest neighbours only (PAPER.md:68 Eq. 6, :157), the owned planes advance bit for bit
 as in the undivided lattice.  Transport: `torch.distributed` point-to-point (NCCL over NVLink / NVSwitch: one 40 B/node
 plane per cut face and direction, 10.5 MB for 512^2 fp32, i.e. ~12 us at 900 GB/s against a ~2.3 ms sweep -- the
@@ -242,6 +245,29 @@ def exchange_local(slabs: Sequence[Slab]) -> None:
             glo.copy_(views[s.plan.lo_rank][2])            # the HIGH owned plane of the slab below
         if s.plan.ghost_hi:
             ghi.copy_(views[s.plan.hi_rank][0])            # the LOW owned plane of the slab above
+
+
+def connect_local(slabs: Sequence[Slab]) -> None:
+    """Fused form (tslb_set_neighbor): every slab's tile kernel reads its ghost planes in place from the neighbouring slabs'
+    current buffers while it sweeps; nothing is exchanged between steps.  Slabs of one process whose buffers are mutually
+    addressable: one GPU, or several GPUs of one process with peer access enabled.  Tile kernel only (tslb_step refuses
+    otherwise).  Call after the states are loaded, with all slabs at the same step count; advance with step_connected."""
+    for s in slabs:
+        for face, on, nb in ((W.FACE_ZLO, s.plan.ghost_lo, s.plan.lo_rank), (W.FACE_ZHI, s.plan.ghost_hi, s.plan.hi_rank)):
+            if on:
+                b0, b1, cur = slabs[nb].sim.buffers()
+                s.sim.set_neighbor(face, (b0, b1), slabs[nb].plan.nz_local, cur)
+
+
+def step_connected(slabs: Sequence[Slab], n: int = 1) -> None:
+    """n steps of connected slabs on one stream: first every slab's state of time t is completed (tslb_refresh: lateral
+    open-face nodes, ghost columns), then every slab is swept -- each sweep reads only time-t buffers and writes its own
+    time-(t+1) buffer, so stream order is all the synchronisation there is."""
+    for _ in range(n):
+        for s in slabs:
+            s.sim.refresh()
+        for s in slabs:
+            s.sim.step(1)
 
 
 def step_local(slabs: Sequence[Slab], n: int = 1) -> None:

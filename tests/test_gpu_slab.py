@@ -76,6 +76,50 @@ def test_slabs_match_oracle_and_undivided_run(B, oracle_mod, case, world, dtype)
             s.sim.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_connected_slabs_read_their_neighbours_in_place(B, case, world, dtype):
+    """tslb_set_neighbor: the tile kernel loads the ghost planes from the neighbouring slabs' buffers; no exchange between
+    steps.  Bitwise equal to the undivided run (whose parity with the oracle the test above and test_gpu_parity.py hold).
+    The ghost planes of the contexts are poisoned first: nothing may read them."""
+    import torch
+    w = CASES[case](dtype)
+    if TILE_ONLY(B, w) is False:
+        pytest.skip("gather-only lattice")
+    steps = 7
+    periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
+    slabs = [S.Slab(w, p, B.KERNEL_TILE) for p in S.plan_slabs(w.nz, world, periodic_z)]
+    for s in slabs:                                        # poison the ghost planes of the loaded state
+        M = s.sim.export_state()[0]
+        if s.plan.ghost_lo:
+            M[:, 0] = float("nan")
+        if s.plan.ghost_hi:
+            M[:, -1] = float("nan")
+        s.sim.import_state(M, 0)
+    S.connect_local(slabs)
+    l0 = sum(s.sim.launch_count for s in slabs)
+    S.step_connected(slabs, steps)
+    G = S.gather_local(slabs)
+    torch.cuda.synchronize()
+    one = make_gpu(w, B.KERNEL_TILE)
+    one.step(steps)
+    G1 = one.get_moments()
+    assert torch.equal(G, G1), "max %.3e" % (G.double() - G1.double()).abs().max().item()
+    # reloading a state detaches the neighbours; the gather kernel refuses to run with a neighbour attached
+    S.connect_local(slabs)
+    slabs[0].sim.set_kernel(B.KERNEL_GATHER)
+    with pytest.raises(B.TSLBError):
+        slabs[0].sim.step(1)
+    one.close()
+    for s in slabs:
+        s.sim.close()
+
+
+def TILE_ONLY(B, w):
+    return len(kernels_for(B, w)) == 2
+
+
 def test_jet_with_inlet_noise_and_sponge_in_slabs(B, oracle_mod):
     """configs[3]'s own boundary set, reduced: the noisy inlet sits on the first slab, the sponge layer in the last one."""
     w = W.jet(24, 20, 40, steps=12, dtype="f32", D=6.0)
@@ -89,6 +133,12 @@ def test_jet_with_inlet_noise_and_sponge_in_slabs(B, oracle_mod):
         one = make_gpu(w, B.KERNEL_AUTO)
         one.step(w.steps)
         assert np.array_equal(G, one.get_moments().cpu().numpy())
+        # the same with the neighbours read in place
+        periodic_z = False
+        slabs = [S.Slab(w, p, B.KERNEL_TILE) for p in S.plan_slabs(w.nz, world, periodic_z)]
+        S.connect_local(slabs)
+        S.step_connected(slabs, w.steps)
+        assert np.array_equal(S.gather_local(slabs).cpu().numpy(), G)
         one.close()
 
 
