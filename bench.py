@@ -450,7 +450,8 @@ def run_slabs(args):
         achieved = BYTES_PER_SITE[args.dtype] * (units / args.steps) / (step_ms * 1e-3) / 1e9
         cfg = dict(workload_config(args), order=args.order, kernel=B.KERNEL_NAMES[slabs[0].sim.active_kernel()])
         cfg["parallelism"] = ("one lattice in %d z slabs, " % args.slabs) + (
-            "one slab per GPU, ghost planes by NCCL point-to-point" if world > 1 else "all on one GPU, ghost planes by device copies")
+            "one slab per GPU, ghost planes by NCCL point-to-point" if world > 1 else
+            "all on one GPU, " + ("no exchange" if args.connected else "ghost planes by device copies"))
         cfg["slab_planes"] = [p.owned for p in plans]
         cfg["transport"] = ("none: neighbours read in place by the sweep's TMA producer (tslb_set_neighbor)" if args.connected else
                             "staged (tslb_export_face / tslb_import_face)" if args.staged else "in place (tslb_face_planes)")
