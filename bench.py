@@ -51,8 +51,8 @@ def parse_args(argv=None):
     ap.add_argument("--staged", action="store_true",
                     help="with --slabs: ghost planes through tslb_export_face / tslb_import_face instead of in place (tslb_face_planes)")
     ap.add_argument("--connected", action="store_true",
-                    help="with --slabs on one GPU: no exchange at all, the tile kernel reads the neighbouring slabs' planes in place "
-                         "(tslb_set_neighbor)")
+                    help="with --slabs: no exchange at all, the tile kernel reads the neighbouring slabs' planes in place "
+                         "(tslb_set_neighbor; under torchrun through CUDA IPC mappings of the neighbours' workspaces)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
@@ -391,17 +391,20 @@ def run_slabs(args):
     w = make_workload(args)
     w.order = args.order
     plans = S.plan_slabs(w.nz, args.slabs, w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC)
-    slabs = [S.Slab(w, p, kernel, args.staged) for p in (plans if world == 1 else [plans[rank]])]
+    slabs = [S.Slab(w, p, kernel, args.staged, ipc=args.connected and world > 1) for p in (plans if world == 1 else [plans[rank]])]
     owned_sites = float(sum(s.plan.owned for s in slabs)) * w.nx * w.ny
     stream = torch.cuda.current_stream()
 
     if args.connected:
         if world > 1:
-            raise SystemExit("bench.py: --connected needs the slabs in one process (mutually addressable buffers)")
-        S.connect_local(slabs)
+            S.connect_ipc(slabs[0])         # the neighbours' workspaces mapped through CUDA IPC (NVLink peer memory)
+        else:
+            S.connect_local(slabs)
 
     def advance(n):
-        if world > 1:
+        if world > 1 and args.connected:
+            S.step_connected_dist(slabs[0], n)
+        elif world > 1:
             slabs[0].step(n)
         elif args.connected:
             S.step_connected(slabs, n)
@@ -450,7 +453,8 @@ def run_slabs(args):
         achieved = BYTES_PER_SITE[args.dtype] * (units / args.steps) / (step_ms * 1e-3) / 1e9
         cfg = dict(workload_config(args), order=args.order, kernel=B.KERNEL_NAMES[slabs[0].sim.active_kernel()])
         cfg["parallelism"] = ("one lattice in %d z slabs, " % args.slabs) + (
-            "one slab per GPU, ghost planes by NCCL point-to-point" if world > 1 else
+            ("one slab per GPU, " + ("neighbours' planes read over CUDA IPC peer memory, one NCCL all-reduce per step as barrier"
+                                     if args.connected else "ghost planes by NCCL point-to-point")) if world > 1 else
             "all on one GPU, " + ("no exchange" if args.connected else "ghost planes by device copies"))
         cfg["slab_planes"] = [p.owned for p in plans]
         cfg["transport"] = ("none: neighbours read in place by the sweep's TMA producer (tslb_set_neighbor)" if args.connected else

@@ -371,10 +371,13 @@ def _host_ptr(M, ctx: TSLB, shape):
     return C.c_void_p(M.ctypes.data), M
 
 
-def from_workload(w, kernel: int = KERNEL_AUTO) -> TSLB:
-    """Context configured (boundary set, force, kernel choice) for a workloads.Workload; state not loaded."""
+def from_workload(w, kernel: int = KERNEL_AUTO, workspace=None) -> TSLB:
+    """Context configured (boundary set, force, kernel choice) for a workloads.Workload; state not loaded.
+    workspace: None (a torch allocation) or a callable nbytes -> object with data_ptr() / numel() to bind instead."""
     import torch
-    sim = TSLB(w.nx, w.ny, w.nz, w.tau, w.dtype)
+    sim = TSLB(w.nx, w.ny, w.nz, w.tau, w.dtype, bind=workspace is None)
+    if workspace is not None:
+        sim.bind_workspace(workspace(sim.workspace_bytes()))
     for face, kind in w.faces.items():
         if w.inlet is not None and face == w.inlet.face:
             up = torch.from_numpy(w.inlet.u_plane).to("cuda")

@@ -155,18 +155,59 @@ def exchange_planes(plan: SlabPlan, send_lo, send_hi, recv_lo, recv_hi, group=No
             req.wait()
 
 
+def _cudart():
+    from cuda.bindings import runtime as rt
+    return rt
+
+
+class RawWorkspace:
+    """Device memory straight from cudaMalloc (not torch's caching allocator, whose blocks share allocations): its CUDA IPC
+    handle names exactly this workspace.  Quacks like the tensor binding.TSLB.bind_workspace expects."""
+
+    def __init__(self, nbytes: int):
+        import torch
+        torch.empty(1, device="cuda")          # torch's current device is the runtime's current device from here on
+        rt = _cudart()
+        err, ptr = rt.cudaMalloc(int(nbytes))
+        if int(err) != 0:
+            raise RuntimeError("cudaMalloc(%d) failed: %s" % (nbytes, err))
+        self._ptr, self._n = int(ptr), int(nbytes)
+
+    def data_ptr(self) -> int:
+        return self._ptr
+
+    def numel(self) -> int:
+        return self._n
+
+    def ipc_handle(self) -> bytes:
+        err, h = _cudart().cudaIpcGetMemHandle(self._ptr)
+        if int(err) != 0:
+            raise RuntimeError("cudaIpcGetMemHandle failed: %s" % err)
+        return bytes(h.reserved)
+
+    def __del__(self):
+        try:
+            if self._ptr:
+                _cudart().cudaFree(self._ptr)
+                self._ptr = 0
+        except Exception:
+            pass
+
+
 class Slab:
     """One rank's part of a slab-decomposed lattice on the current CUDA device.  staged = False (default): the transport
     reads the owned planes and writes the ghost planes in place in the workspace (tslb_face_planes, zero copy);
     staged = True: through dense arrays (tslb_export_face / tslb_import_face)."""
 
-    def __init__(self, w: W.Workload, plan: SlabPlan, kernel: int = 0, staged: bool = False):
+    def __init__(self, w: W.Workload, plan: SlabPlan, kernel: int = 0, staged: bool = False, ipc: bool = False):
         import torch
         from . import binding
         self.plan = plan
         self.staged = staged
         self.local = local_workload(w, plan)
-        self.sim = binding.from_workload(self.local, kernel)
+        # ipc: the workspace is a cudaMalloc allocation of its own, so that other processes can map it (connect_ipc)
+        self.sim = binding.from_workload(self.local, kernel, RawWorkspace if ipc else None)
+        self._opened = {}          # rank -> base address of that rank's workspace mapped into this process
         self.sim.set_moments(torch.from_numpy(self.local.moments).to("cuda"))
         shape = (10, w.ny, w.nx)
         mk = lambda: torch.empty(shape, dtype=self.sim.torch_dtype, device="cuda")
@@ -222,6 +263,73 @@ class Slab:
         if reduce and self.plan.world > 1:
             dist.all_reduce(d, op=dist.ReduceOp.SUM, group=group)
         return d
+
+
+def _rank_barrier(group=None) -> None:
+    """One ordering point between the ranks' GPU work.  NCCL: a one-element all-reduce on the current stream (device side:
+    it completes when every rank's preceding sweep has, and the following sweep waits for it; the host does not block).
+    Other backends (gloo in the tests): synchronise the device, then a host barrier."""
+    import torch
+    import torch.distributed as dist
+    if dist.get_backend(group) == "nccl":
+        dist.all_reduce(torch.zeros(1, device="cuda"), group=group)
+    else:
+        torch.cuda.synchronize()
+        dist.barrier(group)
+
+
+def connect_ipc(slab: Slab, group=None) -> None:
+    """connect_local across processes (one slab per rank, Slab(..., ipc=True)): every rank publishes the CUDA IPC handle of
+    its workspace and where its two moment buffers sit in it, maps its neighbours' workspaces (cudaIpcOpenMemHandle with
+    lazy peer access: NVLink peer memory when the neighbour is another GPU of the node) and attaches them
+    (tslb_set_neighbor).  Collective; all ranks at the same step count.  Advance with step_connected_dist."""
+    import os
+    import torch.distributed as dist
+    rt = _cudart()
+    ws = slab.sim._keep["ws"]
+    if not isinstance(ws, RawWorkspace):
+        raise ValueError("connect_ipc needs Slab(..., ipc=True)")
+    b0, b1, cur = slab.sim.buffers()
+    mine = (ws.ipc_handle(), b0 - ws.data_ptr(), b1 - ws.data_ptr(), slab.plan.nz_local, cur, os.getpid())
+    infos = [None] * slab.plan.world
+    dist.all_gather_object(infos, mine, group=group)
+    for face, on, nb in ((W.FACE_ZLO, slab.plan.ghost_lo, slab.plan.lo_rank), (W.FACE_ZHI, slab.plan.ghost_hi, slab.plan.hi_rank)):
+        if not on:
+            continue
+        handle, o0, o1, nz, pcur, _ = infos[nb]
+        if nb not in slab._opened:
+            h = rt.cudaIpcMemHandle_t()
+            h.reserved = handle
+            err, base = rt.cudaIpcOpenMemHandle(h, rt.cudaIpcMemLazyEnablePeerAccess)
+            if int(err) != 0:
+                raise RuntimeError("cudaIpcOpenMemHandle (rank %d) failed: %s" % (nb, err))
+            slab._opened[nb] = int(base)
+        base = slab._opened[nb]
+        slab.sim.set_neighbor(face, (base + o0, base + o1), nz, pcur)
+    _rank_barrier(group)
+
+
+def step_connected_dist(slab: Slab, n: int = 1, group=None) -> None:
+    """n steps of IPC-connected slabs, one rank each: complete the own state of time t, one ordering point (every rank's
+    state of time t complete, every sweep of step t-1 finished: the buffer it read may be overwritten), sweep.  The
+    closing ordering point keeps the buffers of the last step alive until every neighbour has read them."""
+    for _ in range(n):
+        slab.sim.refresh()
+        _rank_barrier(group)
+        slab.sim.step(1)
+    _rank_barrier(group)
+
+
+def disconnect_ipc(slab: Slab, group=None) -> None:
+    """Detach the neighbours and unmap their workspaces (collective: nobody may still be sweeping)."""
+    _rank_barrier(group)
+    for face, on in ((W.FACE_ZLO, slab.plan.ghost_lo), (W.FACE_ZHI, slab.plan.ghost_hi)):
+        if on:
+            slab.sim.set_neighbor(face, None)
+    for base in slab._opened.values():
+        _cudart().cudaIpcCloseMemHandle(base)
+    slab._opened.clear()
+    _rank_barrier(group)
 
 
 def exchange_local(slabs: Sequence[Slab]) -> None:

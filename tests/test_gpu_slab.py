@@ -5,6 +5,9 @@ lattice, element by element, at the tolerances of the other parity tests, and (2
 a node's arithmetic does not depend on where the lattice was cut.  The transport over torch.distributed is covered on CPU
 (tests/test_slab_host.py, gloo, world_size 2)."""
 import dataclasses
+import os
+import subprocess
+import sys
 
 import numpy as np
 import pytest
@@ -152,3 +155,55 @@ def test_face_calls_reject_other_faces(B):
     with pytest.raises(B.TSLBError):
         one.export_face(B.FACE_ZLO)
     one.close()
+
+
+IPC_WORKER = r"""
+import os, sys
+sys.path.insert(0, %r)
+import numpy as np, torch, torch.distributed as dist
+from paper_2401_17074_b200 import binding as B, slab as S, workloads as W
+rank, port, world, case = int(sys.argv[1]), sys.argv[2], int(sys.argv[3]), sys.argv[4]
+torch.cuda.set_device(0)
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:" + port, rank=rank, world_size=world)
+if case == "periodic":
+    w = W.random_state(70, 27, 23, seed=61, dtype="f32", tau=0.58)
+else:
+    w = W.jet(24, 20, 40, steps=9, dtype="f32", D=6.0)
+steps = 9
+plan = S.plan_slabs(w.nz, world, case == "periodic")[rank]
+s = S.Slab(w, plan, B.KERNEL_TILE, ipc=True)
+M = s.sim.export_state()[0]                      # poison the ghost planes: nothing may read them
+if plan.ghost_lo: M[:, 0] = float("nan")
+if plan.ghost_hi: M[:, -1] = float("nan")
+s.sim.import_state(M, 0)
+S.connect_ipc(s)
+l0 = s.sim.launch_count
+S.step_connected_dist(s, steps)
+G = s.owned_moments()
+one = B.from_workload(w, B.KERNEL_TILE)
+one.set_moments(torch.from_numpy(w.moments).to("cuda"))
+one.step(steps)
+G1 = one.get_moments()[:, plan.z_lo:plan.z_hi]
+assert torch.equal(G, G1), (rank, (G.double() - G1.double()).abs().max().item())
+S.disconnect_ipc(s)
+dist.barrier(); dist.destroy_process_group()
+print("ok", rank, "launches per step", (s.sim.launch_count - l0) / steps)
+"""
+
+
+@pytest.mark.parametrize("case,world", [("periodic", 2), ("periodic", 3), ("jet", 2)])
+def test_ipc_connected_slabs_in_separate_processes(B, tmp_path, case, world):
+    """One slab per PROCESS, all on this GPU: each maps its neighbours' workspaces through CUDA IPC (slab.connect_ipc), the tile
+    kernel reads their planes in place, the processes meet at one host barrier per step (their kernels never wait on one
+    another), and every rank's owned planes equal the undivided run bit for bit.  The path bench.py --slabs N --connected
+    takes under torchrun, except that there the neighbour is another GPU and the barrier is a stream-ordered NCCL all-reduce."""
+    import socket
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
+    script = tmp_path / "ipc_worker.py"
+    script.write_text(IPC_WORKER % root)
+    procs = [subprocess.Popen([sys.executable, str(script), str(r), str(port), str(world), case], stdout=subprocess.PIPE,
+                              stderr=subprocess.STDOUT, text=True) for r in range(world)]
+    outs = [p.communicate(timeout=600)[0] for p in procs]
+    for p, o in zip(procs, outs):
+        assert p.returncode == 0 and "ok" in o, o
