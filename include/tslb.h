@@ -218,7 +218,8 @@ int tslb_radial_statistics(tslb_ctx *ctx, double xc, double yc, double dr, int n
  *     tslb_import_face(face)  such an array into the ghost plane (z = 0 for ZLO, z = nz - 1 for ZHI) of the current state,
  *                             ghost columns included.
  * Both are asynchronous on `stream`; face_bytes = 10 * ny * nx * sizeof(dtype) (tslb_face_bytes).  Ghost planes are left out
- * of tslb_diagnostics, so the sums of the ranks add up to those of the undivided lattice.  The seeded inlet noise is keyed
+ * of tslb_diagnostics and tslb_plane_statistics(_static) (on axis 2 their rows stay as they were), so the sums of the ranks add up
+ * to those of the undivided lattice; tslb_radial_statistics is per plane: drop the ghost planes' rows.  The seeded inlet noise is keyed
  * on the node's index in the context's own lattice: an inlet on the z = 0 face of the first slab draws the numbers of the
  * undivided run, inlets on faces the cuts cross do not.
  * TSLB_EINVAL: face is not ZLO / ZHI or not of kind EXCHANGE, NULL pointer; TSLB_ESTATE: no state. */

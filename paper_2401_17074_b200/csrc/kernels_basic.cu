@@ -390,8 +390,11 @@ __global__ void diag_final_kernel(const double *__restrict__ partial, int nblock
 // in a fixed order to the caller's running sums.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(256) stats_partial_kernel(const T *__restrict__ A, Layout L, int axis, double *__restrict__ partial)
+__global__ void __launch_bounds__(256) stats_partial_kernel(const T *__restrict__ A, Layout L, int axis, double *__restrict__ partial,
+                                                            int zlo, int zhi)
 {
+    // [zlo, zhi): the planes that count -- all of them, except the ghost planes of a slab (EXCHANGE faces), which belong to the
+    // neighbouring rank and may hold anything: they add nothing to the planes of axis 0 / 1 and give zero rows on axis 2
     const int j = blockIdx.x, part = blockIdx.y, nparts = gridDim.y;
     const int n[3] = {L.nx, L.ny, L.nz};
     const int a = (axis == 0) ? 1 : 0;              // fastest in-plane axis
@@ -403,6 +406,7 @@ __global__ void __launch_bounds__(256) stats_partial_kernel(const T *__restrict_
     for (long long i = (long long)part * blockDim.x + threadIdx.x; i < cnt; i += (long long)nparts * blockDim.x) {
         int q[3];
         q[axis] = j; q[a] = (int)(i % n[a]); q[b] = (int)(i / n[a]);
+        if (q[2] < zlo || q[2] >= zhi) continue;
         const long long idx = lay_idx(L, q[0], q[1], q[2]);
         const double ux = A[L.field + idx], uy = A[2 * L.field + idx], uz = A[3 * L.field + idx];
         acc[0] += 1.0;
@@ -611,12 +615,15 @@ cudaError_t tslb_launch_radial_stats(tslb_ctx *c, double xc, double yc, double d
     return cudaGetLastError();
 }
 
+static int stat_zlo(const tslb_ctx *c) { return c->kind[TSLB_FACE_ZLO] == TSLB_BC_EXCHANGE ? 1 : 0; }
+static int stat_zhi(const tslb_ctx *c) { return c->kind[TSLB_FACE_ZHI] == TSLB_BC_EXCHANGE ? c->nz - 1 : c->nz; }
+
 cudaError_t tslb_launch_plane_stats(tslb_ctx *c, int axis, double *dev_sums, cudaStream_t st)
 {
     const int na = axis == 0 ? c->nx : (axis == 1 ? c->ny : c->nz);
     dim3 grid(na, TSLB_STAT_PARTS);
-    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, c->scratch);
-    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, c->scratch);
+    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, c->scratch, stat_zlo(c), stat_zhi(c));
+    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, c->scratch, stat_zlo(c), stat_zhi(c));
     const int tot = TSLB_STAT_ROWS * na;
     stats_final_kernel<<<(tot + 127) / 128, 128, 0, st>>>(c->scratch, na, TSLB_STAT_PARTS, dev_sums);
     c->launches += 2;
@@ -665,8 +672,8 @@ cudaError_t tslb_launch_plane_stats_static(tslb_ctx *c, int axis, double *dev_su
     cudaError_t e = static_scratch_ptr(&scratch);
     if (e != cudaSuccess) return e;
     dim3 grid(na, TSLB_STAT_PARTS);
-    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, scratch);
-    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, scratch);
+    if (c->dtype == TSLB_F32) stats_partial_kernel<float><<<grid, 256, 0, st>>>((const float *)c->buf[c->cur], c->L, axis, scratch, stat_zlo(c), stat_zhi(c));
+    else stats_partial_kernel<double><<<grid, 256, 0, st>>>((const double *)c->buf[c->cur], c->L, axis, scratch, stat_zlo(c), stat_zhi(c));
     const int tot = TSLB_STAT_ROWS * na;
     stats_final_kernel<<<(tot + 127) / 128, 128, 0, st>>>(scratch, na, TSLB_STAT_PARTS, dev_sums);
     c->launches += 2;

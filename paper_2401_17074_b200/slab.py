@@ -18,8 +18,8 @@ in one process on one GPU (`exchange_local`, what the 1-GPU parity test uses; th
 
 Limits (checked, with an error): the seeded inlet noise is keyed on a context's own node index, so a noisy inlet must sit
 on the global z = 0 / z = nz-1 face of a first / last slab whose z offset is zero (the jet's inlet does); a sponge layer
-(Eq. 26) must lie inside the last slab; statistics calls are per slab (ghost planes included -- strip them with
-`Slab.owned`).
+(Eq. 26) must lie inside the last slab.  `Slab.plane_statistics` / `radial_statistics` / `diagnostics` give the sums of
+the undivided lattice (ghost planes left out).
 """
 from __future__ import annotations
 
@@ -255,6 +255,29 @@ class Slab:
 
     def owned_moments(self):
         return self.owned(self.sim.get_moments())
+
+    def plane_statistics(self, axis: int, sums, group=None, reduce: bool = False):
+        """One sample of the plane sums (tslb_plane_statistics) of this slab's OWNED planes added to `sums`, the array of
+        the whole lattice ([13][n_axis of the undivided lattice], CUDA fp64): planes of constant x or y get this slab's
+        share, planes of constant z land in rows z_lo .. z_hi.  reduce = True adds the ranks up (collective; then every
+        rank must pass an array that holds only its own contribution, e.g. zeros)."""
+        import torch
+        loc = self.sim.plane_statistics(axis)                      # ghost planes are left out by the library
+        if axis == 2:
+            sums[:, self.plan.z_lo:self.plan.z_hi] += self.owned(loc)
+        else:
+            sums += loc
+        if reduce and self.plan.world > 1:
+            import torch.distributed as dist
+            dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
+        return sums
+
+    def radial_statistics(self, xc: float, yc: float, dr: float, nr: int, sums):
+        """One sample of the (r, z)-ring sums (tslb_radial_statistics) of the owned planes added to rows z_lo .. z_hi of
+        `sums` ([8][nz of the undivided lattice][nr], CUDA fp64)."""
+        loc = self.sim.radial_statistics(xc, yc, dr, nr)
+        sums[:, self.plan.z_lo:self.plan.z_hi] += self.owned(loc)
+        return sums
 
     def diagnostics(self, group=None, reduce: bool = True):
         """(mass, momentum[3], kinetic energy) of the whole lattice: the slabs' sums (ghost planes left out) added up."""

@@ -145,6 +145,38 @@ def test_jet_with_inlet_noise_and_sponge_in_slabs(B, oracle_mod):
         one.close()
 
 
+@pytest.mark.parametrize("connected", [False, True])
+def test_statistics_of_slabs_add_up_to_the_undivided_lattice(B, connected):
+    """Plane sums on all three axes and the jet's (r, z)-ring sums: the slabs' contributions (ghost planes left out, which in
+    the connected form hold whatever the sweep wrote there) against the undivided CUDA run, whose parity with the oracle
+    test_gpu_parity.py holds."""
+    import torch
+    w = W.jet(24, 20, 40, steps=8, dtype="f32", D=6.0)
+    one = make_gpu(w, B.KERNEL_AUTO)
+    one.step(w.steps)
+    slabs = [S.Slab(w, p, B.KERNEL_AUTO) for p in S.plan_slabs(w.nz, 3, False)]
+    if connected:
+        S.connect_local(slabs)
+        S.step_connected(slabs, w.steps)
+    else:
+        S.step_local(slabs, w.steps)
+    for axis, n in ((0, w.nx), (1, w.ny), (2, w.nz)):
+        ref = one.plane_statistics(axis)
+        tot = torch.zeros((13, n), dtype=torch.float64, device="cuda")
+        for s in slabs:
+            s.plane_statistics(axis, tot)
+        assert torch.isfinite(tot).all()
+        torch.testing.assert_close(tot, ref, rtol=1e-12, atol=1e-13)
+        assert tot[0].sum().item() == w.sites                       # every node counted once
+    xc, yc = (w.nx - 1) / 2.0, (w.ny - 1) / 2.0
+    ref = one.radial_statistics(xc, yc, 1.5, 8)
+    tot = torch.zeros_like(ref)
+    for s in slabs:
+        s.radial_statistics(xc, yc, 1.5, 8, tot)
+    torch.testing.assert_close(tot, ref, rtol=1e-12, atol=1e-13)
+    one.close()
+
+
 def test_face_calls_reject_other_faces(B):
     w = W.random_state(16, 8, 9, seed=3, dtype="f32")
     s = S.Slab(w, S.plan_slabs(w.nz, 2, True)[0])
