@@ -170,6 +170,7 @@ struct TileParams {
     T beta, g[3];
     const T *beta_z;   // sponge layer (Eq. 26): 1 - omega of the nodes of plane z, [nz] (SPONGE instantiations only)
     int zchunk;  // planes per z chunk
+    int zbeg, zend;   // planes that are advanced: all of them, without the ghost planes of a slab (EXCHANGE faces)
     int fuse;    // the store warp writes the open-face boundary nodes of time t+1 itself (FUSE instantiations)
 };
 // Slab neighbours read in place (tslb_set_neighbor, include/tslb.h): the source plane ON an EXCHANGE face -- the ghost plane of
@@ -460,8 +461,8 @@ sweep_tile_kernel(const __grid_constant__ CUtensorMap tmMain, const __grid_const
     // rows are computed twice, to identical values)
     const int x0 = blockIdx.x * COLS;
     const int row0 = min((int)blockIdx.y * ROWS, L.ny - ROWS);
-    const int z0 = blockIdx.z * p.zchunk;
-    const int z1 = min(z0 + p.zchunk, L.nz);
+    const int z0 = p.zbeg + blockIdx.z * p.zchunk;
+    const int z1 = min(z0 + p.zchunk, p.zend);
     const int nplanes = z1 - z0 + 2;                     // source planes z0-1 .. z1
     // z of the i-th source plane (wrapped on a periodic axis; beyond a wall / open face the plane is zero-filled and the
     // index only has to be valid): needed for the per-plane relaxation of a sponge layer
@@ -1238,14 +1239,18 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
     // in z until the halo rows / columns that neighbouring tiles share have left L2 before their second reader arrives
     // (measured at 512^3 fp32: DRAM reads 7.09 / 6.62 / 6.13 GB per step for chunks of 128 / 64 / 32 planes, 5.4 GB
     // algorithmic; profiles/README.md).
+    // (the ghost planes of a slab -- EXCHANGE faces -- are sources only: the march covers the owned planes)
+    p.zbeg = c->kind[4] == TSLB_BC_EXCHANGE ? 1 : 0;
+    p.zend = c->kind[5] == TSLB_BC_EXCHANGE ? c->nz - 1 : c->nz;
+    const int nzs = p.zend - p.zbeg;
     const long long cols = (long long)gx * gy;
     int best = 1;
     double best_cost = 1e300;
-    for (int k = 1; k <= c->nz; ++k) {
-        const int zc = (c->nz + k - 1) / k;
+    for (int k = 1; k <= nzs; ++k) {
+        const int zc = (nzs + k - 1) / k;
         if (k > 1 && zc < 8) break;
-        if (zc > TILE_ZC_MAX && (c->nz + k) / (k + 1) >= 8) continue;
-        const long long ctas = cols * ((c->nz + zc - 1) / zc);
+        if (zc > TILE_ZC_MAX && (nzs + k) / (k + 1) >= 8) continue;
+        const long long ctas = cols * ((nzs + zc - 1) / zc);
         const long long slots = (long long)c->sm_count * TDH::G::CTAS;
         const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (zc + 2 + 3);      // + ring fill latency of a fresh CTA, in plane units
@@ -1253,9 +1258,9 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
     }
     // a plane of a small CTA (4 rows, two CTAs per SM) takes about TILE_SMALL_PLANE of a large one's (12 rows)
     if (cost_out) *cost_out = (c->ny < TDH::ROWS) ? 1e300 : best_cost * (GEO == 1 ? TILE_SMALL_PLANE : 1.0);
-    int zc = (c->nz + best - 1) / best;
+    int zc = (nzs + best - 1) / best;
     p.zchunk = zc;
-    *grid = dim3(gx, gy, (c->nz + zc - 1) / zc);
+    *grid = dim3(gx, gy, (nzs + zc - 1) / zc);
     // Fused boundary fill: possible when every open-face boundary node shares a tile and a z chunk with the interior node
     // x_F it copies (the store warp patches the output tile in shared memory), the row tail and the periodic ghost
     // columns -- stored from the main warps' registers, unpatched -- do not hold boundary values, and open axes are
@@ -1272,7 +1277,7 @@ TileParams<T> make_tile(const tslb_ctx *c, dim3 *grid, double *cost_out)
     if (c->kind[0] == TSLB_BC_PERIODIC) ok = false;                               // ghost-column images of boundary rows
     if (c->nx % (int)(16 / sizeof(T)) != 0) ok = false;                           // row tail stored from registers
     if (open_k(1) && (c->nx - 1) % TDH::COLS == 0) ok = false;            // x = nx-1 alone in the last tile column
-    if (open_k(5) && c->nz - (int)(grid->z - 1) * zc < 2) ok = false;             // z = nz-1 alone in the last chunk
+    if (open_k(5) && p.zend - (p.zbeg + (int)(grid->z - 1) * zc) < 2) ok = false;   // z = nz-1 alone in the last chunk
     if (zc < 2) ok = false;
     if (c->kind[4] == TSLB_BC_BOUNCE_BACK || c->kind[5] == TSLB_BC_BOUNCE_BACK) ok = false;   // z-wall kernels: plain store warp only
     if (c->kind[0] == TSLB_BC_BOUNCE_BACK || c->kind[1] == TSLB_BC_BOUNCE_BACK) ok = false;   // x-wall kernels likewise
