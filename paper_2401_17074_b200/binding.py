@@ -272,6 +272,8 @@ class TSLB:
         self._chk(self._lib.tslb_face_planes(self._h, int(face), C.byref(owned), C.byref(ghost), C.byref(pb), C.byref(fs),
                                              _stream_ptr(stream)), "tslb_face_planes")
         ws = self._keep["ws"]
+        if not hasattr(ws, "untyped_storage"):
+            raise TypeError("face_planes returns views of a torch workspace; this context is bound to %s" % type(ws).__name__)
         es = 4 if self.dtype == "f32" else 8
         typed = self._keep.get("ws_typed")
         if typed is None:

@@ -88,7 +88,7 @@ def test_connected_slabs_read_their_neighbours_in_place(B, case, world, dtype):
     The ghost planes of the contexts are poisoned first: nothing may read them."""
     import torch
     w = CASES[case](dtype)
-    if TILE_ONLY(B, w) is False:
+    if not runs_on_tile(B, w):
         pytest.skip("gather-only lattice")
     steps = 7
     periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
@@ -119,8 +119,40 @@ def test_connected_slabs_read_their_neighbours_in_place(B, case, world, dtype):
         s.sim.close()
 
 
-def TILE_ONLY(B, w):
+def runs_on_tile(B, w):
     return len(kernels_for(B, w)) == 2
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_thin_slabs_of_one_and_two_planes(B, oracle_mod, dtype):
+    """The smallest slabs there are: one owned plane between two ghost planes (its low and its high export are the same
+    plane), next to slabs of two; ragged split (the first ranks own one plane more); all three transports."""
+    import torch
+    cases = [(W.random_state(62, 13, 5, seed=71, dtype=dtype, tau=0.6), 4),                     # periodic: 2, 1, 1, 1 planes
+             (with_faces(W.random_state(30, 16, 7, seed=72, dtype=dtype, tau=0.57), **BC_SETS["jet_like"]), 3)]   # 3, 2, 2
+    for w, world in cases:
+        steps = 5
+        o = make_oracle(oracle_mod, w)
+        o.step(steps)
+        R = o.get_moments()
+        one = make_gpu(w, B.KERNEL_TILE)
+        one.step(steps)
+        G1 = one.get_moments()
+        for mode in ("staged", "in place", "connected"):
+            periodic_z = w.faces.get(W.FACE_ZLO, W.BC_PERIODIC) == W.BC_PERIODIC
+            slabs = [S.Slab(w, p, B.KERNEL_TILE, staged=(mode == "staged")) for p in S.plan_slabs(w.nz, world, periodic_z)]
+            assert min(s.plan.owned for s in slabs) <= 2
+            if mode == "connected":
+                S.connect_local(slabs)
+                S.step_connected(slabs, steps)
+            else:
+                S.step_local(slabs, steps)
+            G = S.gather_local(slabs)
+            assert torch.equal(G, G1), "%s, %s" % (w.name, mode)
+            for s in slabs:
+                s.sim.close()
+        assert_parity(w, G1.cpu().numpy().astype(np.float64), R, "thin slabs")
+        one.close()
 
 
 def test_jet_with_inlet_noise_and_sponge_in_slabs(B, oracle_mod):
