@@ -121,3 +121,19 @@ def test_exchange_planes_world_size_2_gloo(tmp_path, periodic, chunked):
     outs = [p.communicate(timeout=240)[0] for p in procs]
     for p, o in zip(procs, outs):
         assert p.returncode == 0 and "ok" in o, o
+
+
+def test_local_workload_cuts_a_lateral_inlet_plane_and_refuses_its_noise():
+    """An inlet on a face the cuts cross: its imposed-velocity plane [3][nz][nx] is cut to the slab's planes (ghost planes
+    included); with noise it is refused (the noise stream is keyed on a context's own node index)."""
+    w = W.random_state(6, 5, 12, seed=4)
+    up = np.random.default_rng(1).uniform(-0.03, 0.03, (3, w.nz, w.nx))
+    w.faces = {W.FACE_YHI: W.BC_VELOCITY_INLET, W.FACE_YLO: W.BC_OUTLET_ZERO_GRADIENT}
+    w.inlet = W.Inlet(W.FACE_YHI, up, 0.0, 9, 0)
+    for p in S.plan_slabs(w.nz, 3, True):
+        lw = S.local_workload(w, p)
+        zs = np.arange(p.z_offset, p.z_offset + p.nz_local) % w.nz
+        assert lw.inlet.u_plane.shape == (3, p.nz_local, w.nx) and np.array_equal(lw.inlet.u_plane, up[:, zs, :])
+    w.inlet = W.Inlet(W.FACE_YHI, up, 0.05, 9, 0b111)
+    with pytest.raises(NotImplementedError):
+        S.local_workload(w, S.plan_slabs(w.nz, 3, True)[1])
