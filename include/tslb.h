@@ -208,7 +208,7 @@ int tslb_radial_statistics(tslb_ctx *ctx, double xc, double yc, double dr, int n
 /* Slab decomposition along z (PAPER.md:318 names multi-GPU domain decomposition as the next step).
  * A rank owns planes [z_lo, z_hi) of the global lattice and holds them in a context of its own whose z axis is extended by
  * one GHOST plane per cut face: face kind TSLB_BC_EXCHANGE on TSLB_FACE_ZLO and/or TSLB_FACE_ZHI.  The nodes of a ghost plane
- * are never filled by the library and what a sweep writes there is meaningless; their time-t moments are the caller's to
+ * are never filled by the library (the tile kernel does not write them, what the gather kernel writes there is meaningless); their time-t moments are the caller's to
  * supply before every tslb_step (n = 1 per exchange): because a sweep reads only time-t nearest neighbours (Eq. 6, :157), the
  * owned planes then advance exactly -- bit for bit -- as they would in the undivided lattice.  Per step and cut face:
  *     tslb_export_face(face)  the 10 moments of the outermost OWNED plane (z = 1 for ZLO, z = nz - 2 for ZHI) at the current
